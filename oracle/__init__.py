@@ -1,0 +1,146 @@
+"""CPU oracle for the hot path of arXiv 2506.02121 — TEST INFRASTRUCTURE ONLY.
+
+numpy-facing wrappers (argument marshalling only) around oracle/liboracle.so, which is
+compiled from oracle/mlcc_oracle.c.  Only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this package.  It imports nothing from the
+product package and the product never imports it.
+"""
+import ctypes as C
+
+import numpy as np
+
+from .build import build as _build
+
+_lib = None
+
+_d = np.float64
+_pd = np.ctypeslib.ndpointer(dtype=np.float64, flags="C_CONTIGUOUS")
+_pi32 = np.ctypeslib.ndpointer(dtype=np.int32, flags="C_CONTIGUOUS")
+_pi64 = np.ctypeslib.ndpointer(dtype=np.int64, flags="C_CONTIGUOUS")
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(_build())
+        L.orc_critical_curves.argtypes = [_pd, _pd, C.c_int64, C.c_double, C.c_double, C.c_int64,
+                                          C.c_double, C.c_int, _pd, _pi32, _pi32]
+        for f in (L.orc_critical_curve_rows, L.orc_critical_curve_rows_ld):
+            f.argtypes = [_pd, _pd, C.c_int64, C.c_double, C.c_double, C.c_int64, C.c_int64,
+                          _pi64, C.c_int64, C.c_double, C.c_int, C.c_void_p, _pd, _pi32, _pi32]
+        for f in (L.orc_caustics, L.orc_caustics_ld):
+            f.argtypes = [_pd, _pd, C.c_int64, C.c_double, C.c_double, _pd, C.c_int64, _pd]
+        for f in (L.orc_residuals, L.orc_residuals_ld):
+            f.argtypes = [_pd, _pd, C.c_int64, C.c_double, C.c_double, C.c_double, C.c_double,
+                          _pd, C.c_int64, _pd]
+        L.orc_match_root_sets.argtypes = [_pd, _pd, C.c_int64, C.c_int64, C.c_double, _pd, _pi32]
+        L.orc_star_field.argtypes = [C.c_uint64, C.c_int64, C.c_double, C.c_int, C.c_void_p,
+                                     _pd, _pd, C.POINTER(C.c_double)]
+        L.orc_philox4x32_10.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32),
+                                        C.POINTER(C.c_uint32)]
+        L.orc_philox4x32_10.restype = None
+        L.orc_num_threads.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise RuntimeError(f"oracle {what} failed with code {rc}")
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
+
+
+def philox4x32_10(ctr, key):
+    c = (C.c_uint32 * 4)(*[int(x) & 0xFFFFFFFF for x in ctr])
+    k = (C.c_uint32 * 2)(*[int(x) & 0xFFFFFFFF for x in key])
+    o = (C.c_uint32 * 4)()
+    lib().orc_philox4x32_10(c, k, o)
+    return [int(x) for x in o]
+
+
+def star_field(seed, N, kappa_star, mass_model=0, mass_params=None):
+    """-> (star_xy [N,2] f64, masses [N] f64, R)."""
+    xy = np.empty((N, 2), _d)
+    m = np.empty(N, _d)
+    R = C.c_double(0.0)
+    pp = None
+    if mass_params is not None:
+        arr = np.ascontiguousarray(mass_params, _d)
+        pp = arr.ctypes.data_as(C.c_void_p)
+    _check(lib().orc_star_field(int(seed), int(N), float(kappa_star), int(mass_model), pp, xy, m,
+                                C.byref(R)), "star_field")
+    return xy, m, R.value
+
+
+def _stars(star_xy, masses):
+    xy = np.ascontiguousarray(star_xy, _d).reshape(-1, 2)
+    m = np.ascontiguousarray(masses, _d).reshape(-1)
+    assert xy.shape[0] == m.shape[0]
+    return xy, m, xy.shape[0]
+
+
+def critical_curves(star_xy, masses, kappa_s, gamma, num_phi, tol=1e-12, max_iter=50):
+    """Sequential continuation over the whole grid. -> (roots [num_phi,2N,2], iters, unconverged)."""
+    xy, m, N = _stars(star_xy, masses)
+    out = np.empty((num_phi, 2 * N, 2), _d)
+    it = np.zeros(num_phi, np.int32)
+    un = np.zeros(num_phi, np.int32)
+    _check(lib().orc_critical_curves(xy, m, N, float(kappa_s), float(gamma), int(num_phi),
+                                     float(tol), int(max_iter), out, it, un), "critical_curves")
+    return out, it, un
+
+
+def critical_curve_rows(star_xy, masses, kappa_s, gamma, num_phi_total, rows, tol=1e-12,
+                        max_iter=50, j_offset=0, init_roots=None, long_double=False):
+    """Listed rows; first from cold seeds (or init_roots), each next from the previous listed row."""
+    xy, m, N = _stars(star_xy, masses)
+    rows = np.ascontiguousarray(rows, np.int64)
+    out = np.empty((len(rows), 2 * N, 2), _d)
+    it = np.zeros(len(rows), np.int32)
+    un = np.zeros(len(rows), np.int32)
+    ip = None
+    if init_roots is not None:
+        init = np.ascontiguousarray(init_roots, _d).reshape(2 * N, 2)
+        ip = init.ctypes.data_as(C.c_void_p)
+    f = lib().orc_critical_curve_rows_ld if long_double else lib().orc_critical_curve_rows
+    _check(f(xy, m, N, float(kappa_s), float(gamma), int(num_phi_total), int(j_offset), rows,
+             len(rows), float(tol), int(max_iter), ip, out, it, un), "critical_curve_rows")
+    return out, it, un
+
+
+def caustics(star_xy, masses, kappa_s, gamma, points, long_double=False):
+    xy, m, N = _stars(star_xy, masses)
+    pts = np.ascontiguousarray(points, _d)
+    shape = pts.shape
+    flat = pts.reshape(-1, 2)
+    out = np.empty_like(flat)
+    f = lib().orc_caustics_ld if long_double else lib().orc_caustics
+    _check(f(xy, m, N, float(kappa_s), float(gamma), flat, flat.shape[0], out), "caustics")
+    return out.reshape(shape)
+
+
+def residuals(star_xy, masses, kappa_s, gamma, phi_index, num_phi_total, points, long_double=True):
+    """-> dict(F complex, Fp complex, inv_mu, newton = |F|/|F'|) at the points, phase 2 pi phi_index/num_phi_total."""
+    xy, m, N = _stars(star_xy, masses)
+    flat = np.ascontiguousarray(points, _d).reshape(-1, 2)
+    out = np.empty((flat.shape[0], 6), _d)
+    f = lib().orc_residuals_ld if long_double else lib().orc_residuals
+    _check(f(xy, m, N, float(kappa_s), float(gamma), float(phi_index), float(num_phi_total), flat,
+             flat.shape[0], out), "residuals")
+    return {"F": out[:, 0] + 1j * out[:, 1], "Fp": out[:, 2] + 1j * out[:, 3],
+            "inv_mu": out[:, 4].copy(), "newton": out[:, 5].copy()}
+
+
+def match_root_sets(a, b, rel_tol):
+    """a, b: [S,n,2]. -> (max_err [S], bijective [S])."""
+    a = np.ascontiguousarray(a, _d)
+    b = np.ascontiguousarray(b, _d)
+    assert a.shape == b.shape and a.ndim == 3 and a.shape[2] == 2
+    S, n, _ = a.shape
+    err = np.empty(S, _d)
+    bij = np.empty(S, np.int32)
+    _check(lib().orc_match_root_sets(a, b, S, n, float(rel_tol), err, bij), "match_root_sets")
+    return err, bij

@@ -1,0 +1,392 @@
+"""Pins for the CPU oracle: every check here is against something other than the oracle itself —
+closed forms, numpy's companion-matrix eigenvalues of the expanded polynomial, algebraic
+invariants of the root set (Vieta), long-double residuals, scipy's assignment solver, analytic
+CDFs, published known-answer vectors.  None of this needs a GPU.
+
+Passages: PAPER.md:114 (Eq. 12), :128 (Eq. 15), :136 (Eq. 16), :159 (Eq. 17), :170 (Eq. 19),
+:176-182 (seeds, flags, continuation), :463-471 (App. C).
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2506_02121_b200.configs import CONFIGS
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def cplx(a):
+    return a[..., 0] + 1j * a[..., 1]
+
+
+def c_phi(kappa_s, gamma, phi):
+    return (1.0 - kappa_s) * np.exp(-1j * phi) - gamma
+
+
+def match_sets(a, b):
+    """Greedy-free check: sort-free nearest neighbour, returns (max distance, bijective)."""
+    d = np.abs(a[:, None] - b[None, :])
+    j = d.argmin(axis=1)
+    return d[np.arange(len(a)), j].max(), len(set(j.tolist())) == len(b)
+
+
+# ---------------------------------------------------------------------------------------------
+# P1  Einstein ring: one unit star, kappa_s = gamma = 0  ->  z^2 = e^{i phi}, caustic = 0
+# ---------------------------------------------------------------------------------------------
+def test_p1_einstein_ring(orc):
+    z0 = 0.37 - 0.21j  # translation invariance; also keeps seeds off the symmetric real axis
+    xy = np.array([[z0.real, z0.imag]])
+    m = np.array([1.0])
+    num_phi = 64
+    roots, iters, unconv = orc.critical_curves(xy, m, 0.0, 0.0, num_phi)
+    assert unconv.sum() == 0
+    z = cplx(roots) - z0
+    phi = 2 * np.pi * np.arange(num_phi) / num_phi
+    assert np.abs(np.abs(z) - 1.0).max() < 1e-15 * 4
+    for j in range(num_phi):
+        want = np.array([np.exp(0.5j * phi[j]), -np.exp(0.5j * phi[j])])
+        err, bij = match_sets(z[j], want)
+        assert bij and err < 4e-15
+    w = cplx(orc.caustics(xy, m, 0.0, 0.0, roots))
+    assert np.abs(w - z0).max() < 4e-15  # point caustic at the star (lens map of the ring)
+
+
+# ---------------------------------------------------------------------------------------------
+# P2  Chang–Refsdal: one star of mass m with shear and smooth matter -> z^2 = m / c(phi)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kappa_s,gamma,mass", [(0.2, 0.35, 1.0), (0.0, 0.3, 2.5), (0.1, 0.1, 0.3)])
+def test_p2_chang_refsdal_roots(orc, kappa_s, gamma, mass):
+    z0 = -1.3 + 0.8j
+    xy = np.array([[z0.real, z0.imag]])
+    m = np.array([mass])
+    num_phi = 200
+    roots, iters, unconv = orc.critical_curves(xy, m, kappa_s, gamma, num_phi)
+    assert unconv.sum() == 0
+    z = cplx(roots) - z0
+    phi = 2 * np.pi * np.arange(num_phi) / num_phi
+    for j in range(num_phi):
+        r = np.sqrt(mass / c_phi(kappa_s, gamma, phi[j]))
+        err, bij = match_sets(z[j], np.array([r, -r]))
+        assert bij and err < 1e-14, (j, err)
+    # caustic of the closed-form critical point through Eq. 12 written out for one star
+    w = cplx(orc.caustics(xy, m, kappa_s, gamma, roots))
+    zz = cplx(roots)
+    want = (1 - kappa_s) * zz + gamma * np.conj(zz) - mass / (np.conj(zz) - np.conj(z0))
+    assert np.abs(w - want).max() < 1e-14
+
+
+def test_p2_chang_refsdal_cusps_golden(orc):
+    rows = [l.split() for l in open(os.path.join(HERE, "golden", "chang_refsdal_cusps.txt"))
+            if not l.startswith("#")]
+    for ks, g, re_cusp, im_cusp in rows:
+        ks, g, re_cusp, im_cusp = float(ks), float(g), float(re_cusp), float(im_cusp)
+        xy = np.array([[0.0, 0.0]])
+        m = np.array([1.0])
+        num_phi = 400  # even: row 0 is phi = 0, row 200 is phi = pi
+        roots, _, unconv = orc.critical_curves(xy, m, ks, g, num_phi)
+        assert unconv.sum() == 0
+        w = cplx(orc.caustics(xy, m, ks, g, roots))
+        w0 = np.sort_complex(w[0])
+        assert abs(w0[0] + re_cusp) < 1e-14 and abs(w0[1] - re_cusp) < 1e-14
+        wpi = w[num_phi // 2]
+        assert np.abs(wpi.real).max() < 1e-14
+        assert np.abs(np.sort(wpi.imag) - np.array([-im_cusp, im_cusp])).max() < 1e-14
+
+
+# ---------------------------------------------------------------------------------------------
+# P3  Equal-mass binary without shear: u = z^2 solves a quadratic
+#     e^{-i phi} u^2 - (2 b^2 e^{-i phi} + 2 m) u + (b^4 e^{-i phi} - 2 m b^2) = 0, stars at +-b
+# ---------------------------------------------------------------------------------------------
+def test_p3_equal_mass_binary(orc):
+    b = 0.8 * np.exp(0.3j)
+    mass = 0.7
+    xy = np.array([[b.real, b.imag], [-b.real, -b.imag]])
+    m = np.array([mass, mass])
+    num_phi = 90
+    roots, _, unconv = orc.critical_curves(xy, m, 0.0, 0.0, num_phi)
+    assert unconv.sum() == 0
+    z = cplx(roots)
+    for j in range(num_phi):
+        e = np.exp(-2j * np.pi * j / num_phi)
+        u = np.roots([e, -(2 * b * b * e + 2 * mass), b ** 4 * e - 2 * mass * b * b])
+        want = np.concatenate([np.sqrt(u), -np.sqrt(u)])
+        err, bij = match_sets(z[j], want)
+        assert bij and err < 1e-13, (j, err)
+
+
+# ---------------------------------------------------------------------------------------------
+# P4  Companion matrix: expand P(z) = F(z) prod (z - z_i)^2 (Eq. 16) and take np.roots
+# ---------------------------------------------------------------------------------------------
+def expanded_polynomial(zs, ms, kappa_s, gamma, phi):
+    """-c(phi) prod_i (z-z_i)^2 + sum_i m_i prod_{j != i} (z-z_j)^2, highest power first."""
+    N = len(zs)
+    full = np.array([1.0 + 0j])
+    for zi in zs:
+        full = np.polymul(full, np.polymul([1, -zi], [1, -zi]))
+    p = -c_phi(kappa_s, gamma, phi) * full
+    for i in range(N):
+        part = np.array([1.0 + 0j])
+        for jj in range(N):
+            if jj != i:
+                part = np.polymul(part, np.polymul([1, -zs[jj]], [1, -zs[jj]]))
+        p = np.polyadd(p, ms[i] * part)
+    return p
+
+
+@pytest.mark.parametrize("N", [1, 2, 3, 4, 5, 6])
+def test_p4_companion_matrix(orc, N):
+    rng = np.random.default_rng(100 + N)
+    zs = (rng.uniform(-2, 2, N) + 1j * rng.uniform(-2, 2, N))
+    ms = rng.uniform(0.3, 2.0, N)
+    kappa_s, gamma = 0.15, 0.3
+    xy = np.stack([zs.real, zs.imag], axis=1)
+    num_phi = 24
+    roots, _, unconv = orc.critical_curves(xy, ms, kappa_s, gamma, num_phi)
+    assert unconv.sum() == 0
+    z = cplx(roots)
+    assert z.shape == (num_phi, 2 * N)
+    for j in range(num_phi):
+        p = expanded_polynomial(zs, ms, kappa_s, gamma, 2 * np.pi * j / num_phi)
+        assert len(p) == 2 * N + 1  # degree exactly 2N
+        err, bij = match_sets(z[j], np.roots(p))
+        assert bij and err < 1e-8, (N, j, err)
+
+
+# ---------------------------------------------------------------------------------------------
+# P5-P7  invariants on the synthetic workloads: Vieta sums, det J, long-double Newton residual
+# ---------------------------------------------------------------------------------------------
+def _field(orc, cfg):
+    return orc.star_field(cfg.seed, cfg.N, cfg.kappa_star, cfg.mass_model, cfg.mass_params)
+
+
+def check_row_invariants(orc, xy, m, kappa_s, gamma, row_index, num_phi, z, min_sep=1e-6):
+    """All pins that hold for ANY claimed root set of one phase (also used by the GPU tests)."""
+    zs = xy[:, 0] + 1j * xy[:, 1]
+    N = len(m)
+    assert z.shape == (2 * N,)
+    phi = 2 * np.pi * row_index / num_phi
+    c = c_phi(kappa_s, gamma, phi)
+    # Vieta: sum z_k = 2 sum z_i ; sum z_k^2 = 2 sum z_i^2 + 2 (sum m_i)/c(phi)
+    s1, s2 = z.sum(), (z * z).sum()
+    assert abs(s1 - 2 * zs.sum()) <= 1e-12 * np.abs(z).sum()
+    assert abs(s2 - (2 * (zs * zs).sum() + 2 * m.sum() / c)) <= 1e-12 * (np.abs(z) ** 2).sum()
+    res = orc.residuals(xy, m, kappa_s, gamma, row_index, num_phi,
+                        np.stack([z.real, z.imag], axis=1), long_double=True)
+    ulp = np.spacing(np.abs(z))
+    # residual certificate: the long-double Newton step from the fp64 root is at rounding level
+    assert np.all(res["newton"] <= 4 * ulp + 1e-13), res["newton"].max()
+    # scaled det J bound (App. C linearised)
+    bound = 1e-10 + 4 * (1 - kappa_s) * np.abs(res["Fp"]) * 2.0 ** -52 * (1 + np.abs(z))
+    assert np.all(np.abs(res["inv_mu"]) <= bound), (np.abs(res["inv_mu"]) / bound).max()
+    # distinct roots
+    order = np.argsort(z.real)
+    zr = z[order]
+    sep = np.inf
+    for sh in range(1, 8):
+        sep = min(sep, np.abs(zr[sh:] - zr[:-sh]).min()) if len(zr) > sh else sep
+    assert sep > min_sep
+    return res
+
+
+@pytest.mark.parametrize("name,nrows", [("cfg1", 1000), ("cfg2", 40)])
+def test_p5_p6_p7_invariants_full_chain(orc, name, nrows):
+    cfg = CONFIGS[name]
+    xy, m, R = _field(orc, cfg)
+    roots, iters, unconv = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, cfg.num_phi,
+                                                   np.arange(nrows), cfg.tol, cfg.max_iter)
+    assert unconv.sum() == 0 and iters.max() < cfg.max_iter
+    z = cplx(roots)
+    for j in range(0, nrows, max(1, nrows // 25)):
+        res = check_row_invariants(orc, xy, m, cfg.kappa_s, cfg.gamma, j, cfg.num_phi, z[j])
+        if name in ("cfg1", "cfg2"):
+            assert np.abs(res["inv_mu"]).max() <= 1e-10  # the plain BASELINE.json invariant
+
+
+def test_p5_p6_p7_invariants_cfg3_row(orc):
+    cfg = CONFIGS["cfg3"]
+    xy, m, R = _field(orc, cfg)
+    rows = [0, 1, 2]
+    roots, iters, unconv = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, cfg.num_phi,
+                                                   rows, cfg.tol, cfg.max_iter)
+    assert unconv.sum() == 0
+    for q, j in enumerate(rows):
+        check_row_invariants(orc, xy, m, cfg.kappa_s, cfg.gamma, j, cfg.num_phi, cplx(roots)[q])
+
+
+def test_double_vs_long_double_rows(orc):
+    cfg = CONFIGS["cfg2"]
+    xy, m, R = _field(orc, cfg)
+    rows = [0, 1, 2000, 3999]
+    rd, _, _ = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, cfg.num_phi, rows)
+    rl, _, _ = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, cfg.num_phi, rows, long_double=True)
+    for q in range(len(rows)):
+        err, bij = match_sets(cplx(rd)[q], cplx(rl)[q])
+        assert bij and err < 1e-12
+
+
+def test_seed_independence(orc):
+    """The result is the root SET: a different seeding path reaches the same set."""
+    cfg = CONFIGS["cfg1"]
+    xy, m, R = _field(orc, cfg)
+    a, _, _ = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, cfg.num_phi, [500])
+    b, _, _ = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, cfg.num_phi, np.arange(501))
+    err, bij = match_sets(cplx(a)[0], cplx(b)[500])
+    assert bij and err < 1e-13
+
+
+# ---------------------------------------------------------------------------------------------
+# P8  continuity in phi: z_k(phi + dphi) - z_k(phi) = z'_k dphi + O(dphi^2),
+#     z' = -i (1-kappa_s) e^{-i phi} / F'(z)   (from dF = 0)
+# ---------------------------------------------------------------------------------------------
+def test_p8_continuity(orc):
+    cfg = CONFIGS["cfg2"]
+    xy, m, R = _field(orc, cfg)
+    nrows = 12
+    roots, _, unconv = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, cfg.num_phi,
+                                               np.arange(nrows))
+    z = cplx(roots)
+    dphi = 2 * np.pi / cfg.num_phi
+    zp = []
+    for j in range(nrows):
+        res = orc.residuals(xy, m, cfg.kappa_s, cfg.gamma, j, cfg.num_phi, roots[j])
+        zp.append(-1j * (1 - cfg.kappa_s) * np.exp(-1j * j * dphi) / res["Fp"])
+    for j in range(nrows - 1):
+        # column k of row j+1 continues column k of row j:
+        # trapezoid rule on z' leaves O(dphi^3); the Euler step leaves O(dphi^2)
+        step = z[j + 1] - z[j]
+        trap = 0.5 * (zp[j] + zp[j + 1]) * dphi
+        assert np.abs(step - trap).max() < 1e-3 * np.abs(step).max()
+        assert np.abs(step - zp[j] * dphi).max() < 0.02 * np.abs(step).max()
+        assert np.abs(step).max() < 0.05
+
+
+# ---------------------------------------------------------------------------------------------
+# P9  outer pair: far from the field the lens is Chang–Refsdal with the total mass
+#     (PAPER.md:422 fn. 7): if kappa_star > |c(phi)| two roots sit near |z| = R sqrt(kappa_star/|c|)
+# ---------------------------------------------------------------------------------------------
+def test_p9_outer_pair(orc):
+    cfg = CONFIGS["cfg4"]
+    N = 600
+    xy, m, R = orc.star_field(3, N, cfg.kappa_star, cfg.mass_model, cfg.mass_params)
+    rows = [0]
+    roots, _, unconv = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, 1000, rows)
+    assert unconv.sum() == 0
+    z = cplx(roots)[0]
+    c = abs(c_phi(cfg.kappa_s, cfg.gamma, 0.0))
+    assert cfg.kappa_star > c
+    want = R * np.sqrt(cfg.kappa_star / c)
+    outer = np.sort(np.abs(z))[-2:]
+    assert np.all(np.abs(outer / want - 1) < 0.03), (outer, want)
+    assert np.sort(np.abs(z))[-3] < 1.2 * R
+
+
+# ---------------------------------------------------------------------------------------------
+# orientation: stars lie in negative-parity regions
+# ---------------------------------------------------------------------------------------------
+def test_parity_sign_near_stars(orc):
+    cfg = CONFIGS["cfg1"]
+    xy, m, R = _field(orc, cfg)
+    pts = xy + np.array([1e-3, 0.0])
+    res = orc.residuals(xy, m, cfg.kappa_s, cfg.gamma, 0, 1, pts)
+    assert np.all(res["inv_mu"] < 0)
+
+
+# ---------------------------------------------------------------------------------------------
+# root-set matching against scipy's assignment solver
+# ---------------------------------------------------------------------------------------------
+def test_match_root_sets_vs_assignment(orc):
+    from scipy.optimize import linear_sum_assignment
+    rng = np.random.default_rng(7)
+    S, n = 6, 40
+    b = rng.normal(size=(S, n, 2)) * 10
+    a = np.empty_like(b)
+    for s in range(S):
+        a[s] = b[s][rng.permutation(n)] + rng.normal(size=(n, 2)) * 1e-12
+    a[4, 3] = a[4, 5]          # duplicate: not a bijection
+    a[5, 0, 0] += 1e-3         # one root off by more than the tolerance
+    err, bij = orc.match_root_sets(a, b, 1e-10)
+    assert bij.tolist() == [1, 1, 1, 1, 0, 0]
+    for s in range(4):
+        d = np.linalg.norm(a[s][:, None, :] - b[s][None, :, :], axis=2)
+        r, c = linear_sum_assignment(d)
+        assert abs(d[r, c].max() - err[s]) < 1e-18 + 1e-6 * err[s]
+    assert abs(err[5] - 1e-3) < 1e-9
+
+
+# ---------------------------------------------------------------------------------------------
+# star-field generator: Philox known answers, geometry, statistics, analytic mass CDFs
+# ---------------------------------------------------------------------------------------------
+def test_philox_known_answers(orc):
+    for line in open(os.path.join(HERE, "golden", "philox4x32_10_kat.txt")):
+        if line.startswith("#"):
+            continue
+        w = [int(x, 16) for x in line.split()]
+        assert orc.philox4x32_10(w[0:4], w[4:6]) == w[6:10]
+
+
+def test_star_field_geometry_and_stats(orc):
+    from scipy import stats
+    N = 20000
+    xy, m, R = orc.star_field(0, N, 0.2, 0)
+    assert R == np.sqrt(N / 0.2)
+    r2 = (xy ** 2).sum(axis=1) / R ** 2
+    assert r2.max() < 1.0
+    assert np.all(m == 1.0)
+    assert stats.kstest(r2, "uniform").pvalue > 1e-3          # uniform in area
+    ang = (np.arctan2(xy[:, 1], xy[:, 0]) + np.pi) / (2 * np.pi)
+    assert stats.kstest(ang, "uniform").pvalue > 1e-3
+    assert abs(r2.mean() - 0.5) < 0.01                         # <|z|^2> = R^2/2
+    # different seeds, same seed
+    xy2, _, _ = orc.star_field(1, N, 0.2, 0)
+    xy3, _, _ = orc.star_field(0, N, 0.2, 0)
+    assert np.array_equal(xy, xy3) and not np.array_equal(xy, xy2)
+    # prefix property of a counter-based generator: star i does not depend on N (up to the R scale)
+    xy4, _, R4 = orc.star_field(0, 100, 0.2, 0)
+    assert np.allclose(xy4 / R4, xy[:100] / R, rtol=0, atol=1e-15)
+
+
+def _broken_power_law_cdf(mgrid, p):
+    """Forward CDF by direct numerical integration of the continuous broken power law."""
+    m0, m1, m2, m3, a1, a2, a3 = p
+    A2 = m1 ** (a2 - a1)
+    A3 = A2 * m2 ** (a3 - a2)
+
+    def pdf(x):
+        return np.where(x < m1, x ** -a1, np.where(x < m2, A2 * x ** -a2, A3 * x ** -a3))
+    xs = np.exp(np.linspace(np.log(m0), np.log(m3), 400001))
+    f = pdf(xs)
+    cum = np.concatenate([[0], np.cumsum(0.5 * (f[1:] + f[:-1]) * np.diff(xs))])
+    cum /= cum[-1]
+    return np.interp(mgrid, xs, cum)
+
+
+def test_star_field_mass_functions(orc):
+    from scipy import stats
+    N = 40000
+    # Salpeter
+    xy, m, R = orc.star_field(0, N, 0.45, 1)
+    assert abs(m.mean() - 1) < 1e-12 and abs(m.sum() - N) < 1e-8
+    assert abs(m.max() / m.min()) <= 1.0 / 0.08 + 1e-9
+    raw = m / m.min() * 0.08 if False else None  # (scale unknown after normalisation; use ratios)
+    lo, hi, al = 0.08, 1.0, 2.35
+    scale = None
+    # recover the scale: unnormalised mean of the power law
+    e1, e2 = 1 - al, 2 - al
+    mean_raw = ((hi ** e2 - lo ** e2) / e2) / ((hi ** e1 - lo ** e1) / e1)
+    raw = m * mean_raw  # approximately the unnormalised masses (sample mean ~ population mean)
+    cdf = lambda x: np.clip((x ** e1 - lo ** e1) / (hi ** e1 - lo ** e1), 0, 1)
+    assert stats.kstest(raw, cdf).pvalue > 1e-4
+    # Kroupa-like broken power law
+    p = (0.01, 0.08, 0.5, 1.5, 0.3, 1.3, 2.3)
+    xy, m, R = orc.star_field(0, N, 0.2, 2)
+    assert abs(m.mean() - 1) < 1e-12
+    assert m.max() / m.min() <= 150.0 + 1e-6
+    xs = np.exp(np.linspace(np.log(p[0]), np.log(p[3]), 200001))
+    cdfx = _broken_power_law_cdf(xs, p)
+    pdf_mean = np.trapezoid(xs * np.gradient(cdfx, xs), xs)
+    raw = m * pdf_mean
+    assert stats.kstest(raw, lambda x: np.interp(x, xs, cdfx)).pvalue > 1e-4
+    # explicit parameters == defaults
+    xy2, m2, _ = orc.star_field(0, N, 0.2, 2, p)
+    assert np.array_equal(m, m2) and np.array_equal(xy, xy2)
