@@ -1,0 +1,190 @@
+/* mlcc.h — C-ABI of the B200-native critical-curve / caustic library (libmlcc.so).
+ *
+ * Hot path of arXiv 2506.02121 ("A GPU Code for Finding Microlensing Critical Curves and
+ * Caustics"), cited below as PAPER.md:<line>.  Lengths are in Einstein radii of the unit mass
+ * (theta_star = 1).  The lens equation is Eq. 12 with the infinite
+ * compensating sheet alpha_s(z) = -kappa_star z of Appendix A:
+ *
+ *     w = (1 - kappa_s) z + gamma conj(z) - sum_i m_i / (conj(z) - conj(z_i)),
+ *     kappa_s = kappa - kappa_star   (smooth convergence),
+ *
+ * and the critical curves are the roots z of Eq. 15 for each phase phi:
+ *
+ *     F(z, phi) = gamma + sum_i m_i / (z - z_i)^2 - (1 - kappa_s) e^{-i phi} = 0,
+ *
+ * i.e. the 2N roots of P(z) = F(z) prod_i (z - z_i)^2 (Eq. 16).
+ *
+ * Conventions for every entry point
+ *  - Complex numbers are interleaved (re, im) doubles; arrays of them must be 16-byte aligned.
+ *  - Unless the name ends in _host, array pointers are DEVICE pointers to caller-owned,
+ *    caller-allocated buffers (e.g. PyTorch tensors).  The library never frees or keeps them.
+ *    Pointers documented "host" are host pointers.  _host entry points take HOST pointers for
+ *    everything and do their own device allocation and host<->device copies.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Work is
+ *    enqueued on it; calls that return a status computed on the device (convergence counts)
+ *    synchronise that stream before returning.  Entry points without a stream argument use the
+ *    default stream and synchronise it.
+ *  - Workspace is allocated per call with the stream-ordered allocator and released before return.
+ *  - Return value: mlcc_status.  Errors never throw or exit; mlcc_last_error() gives the text
+ *    of the last failure on the calling thread.
+ *  - Thread-safety: re-entrant; concurrent calls must use distinct streams.
+ */
+#ifndef MLCC_H_
+#define MLCC_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum mlcc_status {
+    MLCC_OK = 0,
+    MLCC_ERR_INVALID_ARG = 1,   /* null pointer, N < 1, num_phi < 1, tol <= 0, max_iter < 1, non-finite
+                                   kappa_s / gamma, or c(phi_j) = (1-kappa_s) e^{-i phi_j} - gamma = 0 on
+                                   a grid row (the degree of P drops there)            */
+    MLCC_ERR_CUDA = 2,          /* a CUDA call failed; text in mlcc_last_error()                       */
+    MLCC_ERR_NOMEM = 3,         /* workspace allocation failed                                         */
+    MLCC_ERR_NOT_CONVERGED = 4, /* some root hit max_iter; outputs are fully written, the counts are in
+                                   out_unconverged                                                     */
+    MLCC_ERR_DEGENERATE = 5     /* a NaN/Inf step: a root landed on a star or on another root, or two
+                                   stars coincide; the offending roots are frozen where they were       */
+} mlcc_status;
+
+/* Mass models of the star-field generator (BASELINE.json configs; the paper names none). */
+enum { MLCC_MASS_EQUAL = 0, MLCC_MASS_POWER_LAW = 1, MLCC_MASS_BROKEN_POWER_LAW = 2 };
+
+/* Options of mlcc_critical_curves_ex.  Zero-initialise, or call mlcc_options_default(). */
+typedef struct mlcc_options {
+    int32_t struct_size;      /* = sizeof(mlcc_options)                                             */
+    int32_t num_subchains;    /* sub-chains grown concurrently from their centre rows outwards
+                                 (PAPER.md:211-213); 0 = chosen from N and num_phi                  */
+    int32_t predictor_order;  /* seeds of a new row: 0 = the previous row's roots;
+                                 p >= 1 = polynomial extrapolation through the last p+1 rows of the
+                                 chain (result-preserving: only the starting guess changes); max 5;
+                                 -1 = library default                                               */
+    int32_t max_iter_cold;    /* iteration cap of the cold-started centre rows; 0 = max_iter        */
+    int64_t phi_index_offset; /* row j has phase phi = 2 pi (j + phi_index_offset) / phi_index_total */
+    int64_t phi_index_total;  /* 0 = num_phi (the half-open grid over [0, 2 pi))                     */
+    int32_t min_lanes_per_root; /* lower bound on the threads that split one root's sums
+                                   (power of two <= 256); 0 = library default                        */
+    int32_t reserved;
+} mlcc_options;
+
+/* Counters of one mlcc_critical_curves_ex call (host struct, filled on return). */
+typedef struct mlcc_stats {
+    int64_t root_iterations;   /* sum over all Aberth iterations of the number of unfrozen roots updated */
+    int64_t star_pairs;        /* (root, star) pair evaluations  = root_iterations * N                  */
+    int64_t root_pairs;        /* (root, root) pair evaluations  = root_iterations * (2N - 1)           */
+    int64_t kernel_launches;   /* kernels launched by the call                                          */
+    int32_t total_iterations;  /* Aberth iterations summed over steps (one step = all chains advance 1 row) */
+    int32_t steps;             /* steps taken (cold step included)                                      */
+    int32_t subchains;         /* sub-chains used                                                       */
+    int32_t predictor_order;   /* predictor order used                                                  */
+    int32_t unconverged_rows;  /* rows with out_unconverged > 0                                         */
+    int32_t degenerate_roots;  /* NaN/Inf steps seen                                                    */
+    float   solve_ms;          /* device time of the call's kernels, CUDA events on `stream`            */
+    float   reserved;
+} mlcc_stats;
+
+int         mlcc_version(void);                 /* major*10000 + minor*100 + patch                       */
+const char *mlcc_status_string(int status);     /* static string                                         */
+const char *mlcc_last_error(void);              /* text of the calling thread's last failure ("" if none) */
+void        mlcc_options_default(mlcc_options *opt /*host*/);
+
+/* a0  Star field (Eq. 9, with A_star = pi R^2).
+ * N stars uniform in the disk of radius R = sqrt(N / kappa_star) around the origin, masses from
+ * `mass_model`, divided by their sample mean so that sum m_i = N (theta_star is the Einstein
+ * radius of the mean mass).  Counter-based Philox4x32-10 keyed by `seed`; the recipe is in
+ * DESIGN.md "Input recipe" and the same seed gives the same field on every call.
+ *   mass_params (host, may be NULL = defaults):
+ *     MLCC_MASS_EQUAL: ignored.
+ *     MLCC_MASS_POWER_LAW: {m_lo, m_hi, alpha}, dN/dm ~ m^-alpha (default 0.08, 1, 2.35).
+ *     MLCC_MASS_BROKEN_POWER_LAW: {m0, m1, m2, m3, alpha1, alpha2, alpha3}, continuous at m1, m2
+ *       (default 0.01, 0.08, 0.5, 1.5, 0.3, 1.3, 2.3).
+ *   star_xy [N][2], masses [N]: device, written.  out_radius: host, may be NULL.
+ * Synchronises `stream`.  Errors: INVALID_ARG (N < 1, kappa_star <= 0, bad model/params), CUDA.  */
+int mlcc_star_field(uint64_t seed, int64_t N, double kappa_star, int mass_model,
+                    const double *mass_params, double *star_xy, double *masses,
+                    double *out_radius, void *stream);
+
+/* a1-a6  Critical curves (PAPER.md:128 Eq. 15, :159 Eq. 17, :170 Eq. 19, :176-182, :211-213).
+ * For each row j of the grid phi_j = 2 pi j / num_phi finds all 2N roots of F(z, phi_j) by the
+ * Aberth–Ehrlich iteration evaluated from the rational form (O(N) star sums and an O(N) sum over
+ * the other roots per root and iteration), every root frozen once its step |dz| < tol, roots of
+ * one row seeding the next along each chain.
+ *   star_xy [N][2], masses [N]: device, read.
+ *   out_roots [num_phi][2N][2]: device, written.  Row j is the root SET of phi_j; the column
+ *     order is continuous along a sub-chain but otherwise unspecified.
+ * Default options and the default stream; returns after the work has finished.
+ * Errors: INVALID_ARG, CUDA, NOMEM, NOT_CONVERGED, DEGENERATE (outputs are written in the last two). */
+int mlcc_critical_curves(const double *star_xy, const double *masses, int64_t N,
+                         double kappa_s, double gamma, int64_t num_phi, double tol,
+                         int32_t max_iter, double *out_roots);
+
+/* As above with options, an initial guess, per-row diagnostics and a stream.
+ *   opt: host, NULL = defaults.
+ *   init_roots [2N][2]: device or NULL.  Starting approximations of every cold-started centre row
+ *     instead of the paper's z_i +/- 1.
+ *   out_iters [num_phi], out_unconverged [num_phi]: device int32 or NULL.  Iterations spent on the
+ *     row; roots of the row still unfrozen at max_iter.
+ *   out_stats: host or NULL.                                                                     */
+int mlcc_critical_curves_ex(const double *star_xy, const double *masses, int64_t N,
+                            double kappa_s, double gamma, int64_t num_phi, double tol,
+                            int32_t max_iter, double *out_roots,
+                            const mlcc_options *opt, const double *init_roots,
+                            int32_t *out_iters, int32_t *out_unconverged,
+                            mlcc_stats *out_stats, void *stream);
+
+/* a7  Caustic mapping (Eq. 12 at :114): w_p = lens equation at points[p].
+ *   points [P][2]: device, read.  out_caustics [P][2]: device, written (may not alias points).
+ * Asynchronous on `stream` (no device status to read back).  P = 0 is a no-op.
+ * Errors: INVALID_ARG, CUDA.                                                                     */
+int mlcc_caustics(const double *star_xy, const double *masses, int64_t N, double kappa_s,
+                  double gamma, const double *points, int64_t P, double *out_caustics,
+                  void *stream);
+
+/* a8  Root-set matching validator (BASELINE.json north_star: "root sets per phase are compared
+ * after optimal nearest-neighbour matching").  For each of S sets, every a_i is paired with its
+ * nearest b_j (uniform-grid search).  If that map is a bijection it is the matching that
+ * minimises every pair's distance, hence also the maximum distance.
+ *   a, b [S][n][2]: device, read.
+ *   out_max_err [S]: device, max_i |a_i - b_j(i)| (inf if a set holds a non-finite value).
+ *   out_bijective [S]: device int32, 1 iff j(.) is a bijection and every pair satisfies
+ *     |a_i - b_j(i)| <= rel_tol (1 + |b_j(i)|).
+ * Asynchronous on `stream`.  Errors: INVALID_ARG, CUDA, NOMEM.                                   */
+int mlcc_match_root_sets(const double *a, const double *b, int64_t S, int64_t n, double rel_tol,
+                         double *out_max_err, int32_t *out_bijective, void *stream);
+
+/* Host-only planning helper of the phase-continuation driver: splits rows
+ * [0, num_phi) into `num_subchains` contiguous sub-chains and returns, per sub-chain c, its
+ * first row, its centre row (cold-started) and one past its last row.  num_subchains = 0 asks
+ * for the library's choice for this N.  Returns the number of sub-chains written (<= capacity),
+ * or a negative mlcc_status on bad arguments.  All pointers host.  No CUDA call is made.        */
+int mlcc_plan_subchains(int64_t N, int64_t num_phi, int32_t num_subchains, int32_t capacity,
+                        int64_t *first_row, int64_t *centre_row, int64_t *end_row);
+
+/* Host-buffer variants (every pointer is a HOST pointer; the library allocates device memory,
+ * copies in, runs the device path above on the default stream, copies out and frees).
+ * mlcc_curves_and_caustics_host runs a0..a7 without bringing the roots back to the host in
+ * between; out_caustics may be NULL (critical curves only).                                      */
+int mlcc_critical_curves_host(const double *star_xy, const double *masses, int64_t N,
+                              double kappa_s, double gamma, int64_t num_phi, double tol,
+                              int32_t max_iter, double *out_roots);
+int mlcc_caustics_host(const double *star_xy, const double *masses, int64_t N, double kappa_s,
+                       double gamma, const double *points, int64_t P, double *out_caustics);
+int mlcc_curves_and_caustics_host(const double *star_xy, const double *masses, int64_t N,
+                                  double kappa_s, double gamma, int64_t num_phi, double tol,
+                                  int32_t max_iter, const mlcc_options *opt,
+                                  double *out_roots, double *out_caustics, mlcc_stats *out_stats);
+
+/* Measurement helper: runs a dependent-free DFMA loop on every SM for about `ms_target`
+ * milliseconds and returns the FP64 FMA rate reached, in TFLOP/s (2 flop per FMA) through
+ * *out_tflops (host).  This is the measured denominator of the "alu" roofline in bench.py
+ * (MEASURED_PEAKS.json has no FP64 entry).  Synchronises `stream`.                               */
+int mlcc_fp64_peak(double ms_target, double *out_tflops, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MLCC_H_ */

@@ -1,0 +1,293 @@
+"""Thin Python binding of libmlcc.so (include/mlcc.h): same names, argument marshalling only.
+
+PyTorch supplies device memory (float64 CUDA tensors) and the current stream; every step of the
+path runs in the library's own kernels.  There is no CPU fallback: if the library has not been
+built, or a tensor is not a contiguous float64 CUDA tensor, the call raises.
+"""
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmlcc.so")
+
+MLCC_OK = 0
+MLCC_ERR_INVALID_ARG = 1
+MLCC_ERR_CUDA = 2
+MLCC_ERR_NOMEM = 3
+MLCC_ERR_NOT_CONVERGED = 4
+MLCC_ERR_DEGENERATE = 5
+
+
+class MlccError(RuntimeError):
+    def __init__(self, status: int, text: str):
+        super().__init__(f"{_status_string(status)}: {text}")
+        self.status = status
+
+
+class mlcc_options(C.Structure):
+    _fields_ = [("struct_size", C.c_int32), ("num_subchains", C.c_int32),
+                ("predictor_order", C.c_int32), ("max_iter_cold", C.c_int32),
+                ("phi_index_offset", C.c_int64), ("phi_index_total", C.c_int64),
+                ("min_lanes_per_root", C.c_int32), ("reserved", C.c_int32)]
+
+
+class mlcc_stats(C.Structure):
+    _fields_ = [("root_iterations", C.c_int64), ("star_pairs", C.c_int64), ("root_pairs", C.c_int64),
+                ("kernel_launches", C.c_int64), ("total_iterations", C.c_int32), ("steps", C.c_int32),
+                ("subchains", C.c_int32), ("predictor_order", C.c_int32),
+                ("unconverged_rows", C.c_int32), ("degenerate_roots", C.c_int32),
+                ("solve_ms", C.c_float), ("reserved", C.c_float)]
+
+
+@dataclass
+class Stats:
+    root_iterations: int
+    star_pairs: int
+    root_pairs: int
+    kernel_launches: int
+    total_iterations: int
+    steps: int
+    subchains: int
+    predictor_order: int
+    unconverged_rows: int
+    degenerate_roots: int
+    solve_ms: float
+    status: int = 0
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Loads libmlcc.so (built in-tree by paper_2506_02121_b200.build); raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2506_02121_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, i64, i32, dbl = C.c_void_p, C.c_int64, C.c_int32, C.c_double
+        L.mlcc_version.restype = C.c_int
+        L.mlcc_status_string.restype = C.c_char_p
+        L.mlcc_status_string.argtypes = [C.c_int]
+        L.mlcc_last_error.restype = C.c_char_p
+        L.mlcc_options_default.argtypes = [C.POINTER(mlcc_options)]
+        L.mlcc_options_default.restype = None
+        L.mlcc_star_field.argtypes = [C.c_uint64, i64, dbl, C.c_int, vp, vp, vp, C.POINTER(dbl), vp]
+        L.mlcc_critical_curves.argtypes = [vp, vp, i64, dbl, dbl, i64, dbl, i32, vp]
+        L.mlcc_critical_curves_ex.argtypes = [vp, vp, i64, dbl, dbl, i64, dbl, i32, vp,
+                                              C.POINTER(mlcc_options), vp, vp, vp,
+                                              C.POINTER(mlcc_stats), vp]
+        L.mlcc_caustics.argtypes = [vp, vp, i64, dbl, dbl, vp, i64, vp, vp]
+        L.mlcc_match_root_sets.argtypes = [vp, vp, i64, i64, dbl, vp, vp, vp]
+        L.mlcc_plan_subchains.argtypes = [i64, i64, i32, i32, vp, vp, vp]
+        L.mlcc_critical_curves_host.argtypes = [vp, vp, i64, dbl, dbl, i64, dbl, i32, vp]
+        L.mlcc_caustics_host.argtypes = [vp, vp, i64, dbl, dbl, vp, i64, vp]
+        L.mlcc_curves_and_caustics_host.argtypes = [vp, vp, i64, dbl, dbl, i64, dbl, i32,
+                                                    C.POINTER(mlcc_options), vp, vp, C.POINTER(mlcc_stats)]
+        L.mlcc_fp64_peak.argtypes = [dbl, C.POINTER(dbl), vp]
+        _lib = L
+    return _lib
+
+
+def _status_string(status: int) -> str:
+    return lib().mlcc_status_string(int(status)).decode()
+
+
+def _raise(status: int):
+    raise MlccError(status, lib().mlcc_last_error().decode())
+
+
+def _dev(t: Optional[torch.Tensor], dtype=torch.float64, name="tensor") -> Optional[int]:
+    if t is None:
+        return None
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+        raise TypeError(f"{name} must be a contiguous {dtype} CUDA tensor")
+    return t.data_ptr()
+
+
+def _stream() -> int:
+    return torch.cuda.current_stream().cuda_stream
+
+
+def version() -> int:
+    return int(lib().mlcc_version())
+
+
+def last_error() -> str:
+    return lib().mlcc_last_error().decode()
+
+
+def options(num_subchains=0, predictor_order=-1, max_iter_cold=0, phi_index_offset=0,
+            phi_index_total=0, min_lanes_per_root=0) -> mlcc_options:
+    o = mlcc_options()
+    lib().mlcc_options_default(C.byref(o))
+    o.num_subchains = num_subchains
+    o.predictor_order = predictor_order
+    o.max_iter_cold = max_iter_cold
+    o.phi_index_offset = phi_index_offset
+    o.phi_index_total = phi_index_total
+    o.min_lanes_per_root = min_lanes_per_root
+    return o
+
+
+def star_field(seed: int, N: int, kappa_star: float, mass_model: int = 0, mass_params=None,
+               device="cuda"):
+    """mlcc_star_field -> (star_xy [N,2], masses [N], R)."""
+    xy = torch.empty((N, 2), dtype=torch.float64, device=device)
+    m = torch.empty((N,), dtype=torch.float64, device=device)
+    R = C.c_double(0.0)
+    pp = None
+    if mass_params is not None:
+        arr = np.ascontiguousarray(mass_params, np.float64)
+        pp = arr.ctypes.data_as(C.c_void_p)
+    rc = lib().mlcc_star_field(int(seed), int(N), float(kappa_star), int(mass_model), pp,
+                               xy.data_ptr(), m.data_ptr(), C.byref(R), _stream())
+    if rc != MLCC_OK:
+        _raise(rc)
+    return xy, m, R.value
+
+
+def critical_curves(star_xy, masses, kappa_s, gamma, num_phi, tol=1e-12, max_iter=50):
+    """mlcc_critical_curves (default options, default stream) -> roots [num_phi, 2N, 2]."""
+    N = masses.shape[0]
+    out = torch.empty((num_phi, 2 * N, 2), dtype=torch.float64, device=masses.device)
+    torch.cuda.current_stream().synchronize()  # the call runs on the legacy default stream
+    rc = lib().mlcc_critical_curves(_dev(star_xy, name="star_xy"), _dev(masses, name="masses"), N,
+                                    float(kappa_s), float(gamma), int(num_phi), float(tol),
+                                    int(max_iter), out.data_ptr())
+    if rc != MLCC_OK:
+        _raise(rc)
+    return out
+
+
+def critical_curves_ex(star_xy, masses, kappa_s, gamma, num_phi, tol=1e-12, max_iter=50, opt=None,
+                       init_roots=None, out_roots=None, want_diagnostics=True, strict=True):
+    """mlcc_critical_curves_ex -> (roots [num_phi,2N,2], iters [num_phi] i32, unconverged [num_phi] i32, Stats).
+
+    strict=False returns the outputs also for MLCC_ERR_NOT_CONVERGED / MLCC_ERR_DEGENERATE
+    (Stats.status carries the code)."""
+    N = masses.shape[0]
+    dev = masses.device
+    if out_roots is None:
+        out_roots = torch.empty((num_phi, 2 * N, 2), dtype=torch.float64, device=dev)
+    iters = unconv = None
+    if want_diagnostics:
+        iters = torch.zeros((num_phi,), dtype=torch.int32, device=dev)
+        unconv = torch.zeros((num_phi,), dtype=torch.int32, device=dev)
+    st = mlcc_stats()
+    rc = lib().mlcc_critical_curves_ex(
+        _dev(star_xy, name="star_xy"), _dev(masses, name="masses"), N, float(kappa_s), float(gamma),
+        int(num_phi), float(tol), int(max_iter), _dev(out_roots, name="out_roots"),
+        C.byref(opt) if opt is not None else None, _dev(init_roots, name="init_roots"),
+        _dev(iters, torch.int32, "iters"), _dev(unconv, torch.int32, "unconverged"), C.byref(st), _stream())
+    if rc != MLCC_OK and (strict or rc not in (MLCC_ERR_NOT_CONVERGED, MLCC_ERR_DEGENERATE)):
+        _raise(rc)
+    stats = Stats(st.root_iterations, st.star_pairs, st.root_pairs, st.kernel_launches,
+                  st.total_iterations, st.steps, st.subchains, st.predictor_order,
+                  st.unconverged_rows, st.degenerate_roots, st.solve_ms, rc)
+    return out_roots, iters, unconv, stats
+
+
+def caustics(star_xy, masses, kappa_s, gamma, points, out=None):
+    """mlcc_caustics: points [..., 2] -> caustic points of the same shape (asynchronous on the current stream)."""
+    N = masses.shape[0]
+    P = points.numel() // 2
+    if out is None:
+        out = torch.empty_like(points)
+    rc = lib().mlcc_caustics(_dev(star_xy, name="star_xy"), _dev(masses, name="masses"), N,
+                             float(kappa_s), float(gamma), _dev(points, name="points"), P,
+                             _dev(out, name="out"), _stream())
+    if rc != MLCC_OK:
+        _raise(rc)
+    return out
+
+
+def match_root_sets(a, b, rel_tol):
+    """mlcc_match_root_sets: a, b [S,n,2] -> (max_err [S] f64, bijective [S] i32)."""
+    if a.shape != b.shape or a.dim() != 3 or a.shape[2] != 2:
+        raise ValueError("a and b must both be [S, n, 2]")
+    S, n, _ = a.shape
+    err = torch.empty((S,), dtype=torch.float64, device=a.device)
+    bij = torch.empty((S,), dtype=torch.int32, device=a.device)
+    rc = lib().mlcc_match_root_sets(_dev(a, name="a"), _dev(b, name="b"), S, n, float(rel_tol),
+                                    err.data_ptr(), bij.data_ptr(), _stream())
+    if rc != MLCC_OK:
+        _raise(rc)
+    return err, bij
+
+
+def plan_subchains(N: int, num_phi: int, num_subchains: int = 0):
+    """mlcc_plan_subchains (host only, no CUDA) -> (first_row, centre_row, end_row) int64 arrays."""
+    cap = 1024
+    f = np.zeros(cap, np.int64)
+    c = np.zeros(cap, np.int64)
+    e = np.zeros(cap, np.int64)
+    n = lib().mlcc_plan_subchains(int(N), int(num_phi), int(num_subchains), cap,
+                                  f.ctypes.data, c.ctypes.data, e.ctypes.data)
+    if n < 0:
+        raise MlccError(-n, "mlcc_plan_subchains")
+    return f[:n].copy(), c[:n].copy(), e[:n].copy()
+
+
+def curves_and_caustics_host(star_xy: np.ndarray, masses: np.ndarray, kappa_s, gamma, num_phi,
+                             tol=1e-12, max_iter=50, opt=None, out_roots=None, out_caustics=None,
+                             want_caustics=True):
+    """mlcc_curves_and_caustics_host: HOST arrays in, HOST arrays out (numpy or pinned torch CPU tensors)."""
+    def hptr(x):
+        if isinstance(x, torch.Tensor):
+            assert not x.is_cuda and x.dtype == torch.float64 and x.is_contiguous()
+            return x.data_ptr()
+        assert x.dtype == np.float64 and x.flags["C_CONTIGUOUS"]
+        return x.ctypes.data
+    N = int(masses.shape[0])
+    if out_roots is None:
+        out_roots = np.empty((num_phi, 2 * N, 2), np.float64)
+    if want_caustics and out_caustics is None:
+        out_caustics = np.empty((num_phi, 2 * N, 2), np.float64)
+    st = mlcc_stats()
+    rc = lib().mlcc_curves_and_caustics_host(hptr(star_xy), hptr(masses), N, float(kappa_s), float(gamma),
+                                             int(num_phi), float(tol), int(max_iter),
+                                             C.byref(opt) if opt is not None else None, hptr(out_roots),
+                                             hptr(out_caustics) if want_caustics else None, C.byref(st))
+    if rc != MLCC_OK:
+        _raise(rc)
+    stats = Stats(st.root_iterations, st.star_pairs, st.root_pairs, st.kernel_launches,
+                  st.total_iterations, st.steps, st.subchains, st.predictor_order,
+                  st.unconverged_rows, st.degenerate_roots, st.solve_ms, rc)
+    return out_roots, out_caustics, stats
+
+
+def critical_curves_host(star_xy: np.ndarray, masses: np.ndarray, kappa_s, gamma, num_phi, tol=1e-12, max_iter=50):
+    N = int(masses.shape[0])
+    out = np.empty((num_phi, 2 * N, 2), np.float64)
+    rc = lib().mlcc_critical_curves_host(star_xy.ctypes.data, masses.ctypes.data, N, float(kappa_s),
+                                         float(gamma), int(num_phi), float(tol), int(max_iter), out.ctypes.data)
+    if rc != MLCC_OK:
+        _raise(rc)
+    return out
+
+
+def caustics_host(star_xy: np.ndarray, masses: np.ndarray, kappa_s, gamma, points: np.ndarray):
+    N = int(masses.shape[0])
+    pts = np.ascontiguousarray(points, np.float64)
+    out = np.empty_like(pts)
+    rc = lib().mlcc_caustics_host(star_xy.ctypes.data, masses.ctypes.data, N, float(kappa_s), float(gamma),
+                                  pts.ctypes.data, pts.size // 2, out.ctypes.data)
+    if rc != MLCC_OK:
+        _raise(rc)
+    return out
+
+
+def fp64_peak(ms_target: float = 50.0) -> float:
+    """mlcc_fp64_peak: measured DFMA rate in TFLOP/s."""
+    v = C.c_double(0.0)
+    rc = lib().mlcc_fp64_peak(float(ms_target), C.byref(v), _stream())
+    if rc != MLCC_OK:
+        _raise(rc)
+    return v.value

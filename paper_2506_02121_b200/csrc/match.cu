@@ -1,0 +1,207 @@
+// match.cu — root-set matching validator (BASELINE.json north_star).
+//
+// For each of S sets: every a_i is paired with its nearest b_j.  If i -> j(i) is a bijection,
+// it is the perfect matching in which every pair has its least possible distance, so its
+// largest distance is the optimum of the bottleneck assignment.
+//
+// One CTA per set (grid-stride over sets).  b is binned into a uniform G x G grid over its
+// bounding box (G^2 ~ n cells) by a counting sort in global scratch; each a_i searches the
+// (2r+1)^2 cells around its own, r = 1, 2, ... until the best distance found is <= r * cell size
+// (every unsearched point is then farther away), falling back to all of b after r = 4.
+#include "mlcc_common.cuh"
+
+namespace mlcc {
+namespace {
+
+constexpr int BLOCK = 256;
+
+__device__ __forceinline__ double block_reduce(double v, bool take_max, double *s_buf)
+{
+    const int tid = threadIdx.x;
+    s_buf[tid] = v;
+    __syncthreads();
+    for (int o = BLOCK / 2; o > 0; o >>= 1) {
+        if (tid < o) s_buf[tid] = take_max ? fmax(s_buf[tid], s_buf[tid + o]) : fmin(s_buf[tid], s_buf[tid + o]);
+        __syncthreads();
+    }
+    const double r = s_buf[0];
+    __syncthreads();
+    return r;
+}
+
+__device__ __forceinline__ int cell_coord(double v, double lo, double inv_h, int G)
+{
+    double c = floor((v - lo) * inv_h);
+    if (!(c > 0.0)) c = 0.0;           // also catches NaN
+    if (c > (double)(G - 1)) c = (double)(G - 1);
+    return (int)c;
+}
+
+__global__ void __launch_bounds__(BLOCK) k_match(const double2 *__restrict__ a, const double2 *__restrict__ b,
+                                                 long long S, int n, double rel_tol, int G,
+                                                 int *scratch, long long scratch_stride,
+                                                 double *out_max_err, int *out_bijective)
+{
+    __shared__ double s_buf[BLOCK];
+    __shared__ int s_scan[BLOCK];
+    __shared__ int s_flag;
+    const int tid = threadIdx.x;
+    const int ncell = G * G;
+    int *cell_start = scratch + (long long)blockIdx.x * scratch_stride;  // [ncell + 1]
+    int *cursor = cell_start + ncell + 1;                                // [ncell]
+    int *sorted = cursor + ncell;                                        // [n]
+    int *hits = sorted + n;                                              // [n]
+
+    for (long long s = blockIdx.x; s < S; s += gridDim.x) {
+        const double2 *as = a + s * n, *bs = b + s * n;
+        // ---- bounding box of b, finiteness of a and b ----
+        double xmin = 1e308, xmax = -1e308, ymin = 1e308, ymax = -1e308, bad = 0.0;
+        for (int j = tid; j < n; j += BLOCK) {
+            const double2 q = bs[j], q2 = as[j];
+            xmin = fmin(xmin, q.x); xmax = fmax(xmax, q.x);
+            ymin = fmin(ymin, q.y); ymax = fmax(ymax, q.y);
+            if (!(fabs(q.x) <= 1e300) || !(fabs(q.y) <= 1e300) || !(fabs(q2.x) <= 1e300) || !(fabs(q2.y) <= 1e300)) bad = 1.0;
+        }
+        xmin = block_reduce(xmin, false, s_buf); xmax = block_reduce(xmax, true, s_buf);
+        ymin = block_reduce(ymin, false, s_buf); ymax = block_reduce(ymax, true, s_buf);
+        bad = block_reduce(bad, true, s_buf);
+        if (bad > 0.0) {
+            if (tid == 0) { out_max_err[s] = INFINITY; out_bijective[s] = 0; }
+            continue;
+        }
+        const double wx = xmax - xmin, wy = ymax - ymin;
+        const double hx = wx > 0.0 ? wx / G : 1.0, hy = wy > 0.0 ? wy / G : 1.0;
+        const double inv_hx = 1.0 / hx, inv_hy = 1.0 / hy;
+        const double hmin = fmin(hx, hy);
+        // ---- counting sort of b into cells ----
+        for (int c = tid; c <= ncell; c += BLOCK) cell_start[c] = 0;
+        for (int j = tid; j < n; j += BLOCK) hits[j] = 0;
+        __syncthreads();
+        for (int j = tid; j < n; j += BLOCK) {
+            const double2 q = bs[j];
+            const int c = cell_coord(q.y, ymin, inv_hy, G) * G + cell_coord(q.x, xmin, inv_hx, G);
+            atomicAdd(&cell_start[c + 1], 1);
+        }
+        __syncthreads();
+        {   // inclusive scan of cell_start[1..ncell] (block-wide, contiguous chunks)
+            const int chunk = (ncell + BLOCK - 1) / BLOCK;
+            const int lo = 1 + tid * chunk, hi = min(ncell + 1, lo + chunk);
+            int sum = 0;
+            for (int c = lo; c < hi; ++c) sum += cell_start[c];
+            s_scan[tid] = sum;
+            __syncthreads();
+            if (tid == 0) {
+                int run = 0;
+                for (int t = 0; t < BLOCK; ++t) { const int v = s_scan[t]; s_scan[t] = run; run += v; }
+            }
+            __syncthreads();
+            int run = s_scan[tid];
+            for (int c = lo; c < hi; ++c) { run += cell_start[c]; cell_start[c] = run; }
+            __syncthreads();
+        }
+        for (int c = tid; c < ncell; c += BLOCK) cursor[c] = cell_start[c];
+        __syncthreads();
+        for (int j = tid; j < n; j += BLOCK) {
+            const double2 q = bs[j];
+            const int c = cell_coord(q.y, ymin, inv_hy, G) * G + cell_coord(q.x, xmin, inv_hx, G);
+            sorted[atomicAdd(&cursor[c], 1)] = j;
+        }
+        __syncthreads();
+        // ---- nearest b for every a ----
+        double max_d2 = 0.0;
+        int ok = 1;
+        for (int i = tid; i < n; i += BLOCK) {
+            const double2 p = as[i];
+            const int cx = cell_coord(p.x, xmin, inv_hx, G), cy = cell_coord(p.y, ymin, inv_hy, G);
+            double best = INFINITY;
+            int bj = -1;
+            int r_done = 0;
+            for (int r = 1; r <= 4; ++r) {
+                // ring r-1 .. r: search cells of the (2r+1)^2 block not in the (2r-1)^2 block (r = 1: all 9)
+                for (int yy = cy - r; yy <= cy + r; ++yy) {
+                    if (yy < 0 || yy >= G) continue;
+                    for (int xx = cx - r; xx <= cx + r; ++xx) {
+                        if (xx < 0 || xx >= G) continue;
+                        if (r > 1 && abs(yy - cy) < r && abs(xx - cx) < r) continue;
+                        const int c = yy * G + xx;
+                        for (int t = cell_start[c]; t < cell_start[c + 1]; ++t) {
+                            const int j = sorted[t];
+                            const double2 q = bs[j];
+                            const double dx = p.x - q.x, dy = p.y - q.y;
+                            const double d2 = dx * dx + dy * dy;
+                            if (d2 < best || (d2 == best && j < bj)) { best = d2; bj = j; }
+                        }
+                    }
+                }
+                r_done = r;
+                const double reach = r * hmin;
+                if (best <= reach * reach) break;
+                if (cx - r <= 0 && cy - r <= 0 && cx + r >= G - 1 && cy + r >= G - 1) break;  // whole grid seen
+            }
+            const double reach = r_done * hmin;
+            const bool whole = (cx - r_done <= 0 && cy - r_done <= 0 && cx + r_done >= G - 1 && cy + r_done >= G - 1);
+            if (!(best <= reach * reach) && !whole) {   // rare: nothing close, look at everything
+                for (int j = 0; j < n; ++j) {
+                    const double2 q = bs[j];
+                    const double dx = p.x - q.x, dy = p.y - q.y;
+                    const double d2 = dx * dx + dy * dy;
+                    if (d2 < best || (d2 == best && j < bj)) { best = d2; bj = j; }
+                }
+            }
+            max_d2 = fmax(max_d2, best);
+            if (bj >= 0) {
+                atomicAdd(&hits[bj], 1);
+                const double2 q = bs[bj];
+                const double lim = rel_tol * (1.0 + sqrt(q.x * q.x + q.y * q.y));
+                if (!(sqrt(best) <= lim)) ok = 0;
+            } else {
+                ok = 0;
+            }
+        }
+        max_d2 = block_reduce(max_d2, true, s_buf);
+        if (tid == 0) s_flag = 1;
+        __syncthreads();
+        if (!ok) s_flag = 0;
+        __syncthreads();
+        for (int j = tid; j < n; j += BLOCK) if (hits[j] != 1) s_flag = 0;
+        __syncthreads();
+        if (tid == 0) { out_max_err[s] = sqrt(max_d2); out_bijective[s] = s_flag; }
+        __syncthreads();
+    }
+}
+
+}  // namespace
+
+int match_root_sets_impl(const double *a, const double *b, int64_t S, int64_t n, double rel_tol,
+                         double *out_max_err, int32_t *out_bijective, cudaStream_t stream)
+{
+    if (S < 0) return invalid("S < 0");
+    if (n < 1 || n > (1 << 30)) return invalid("n out of range");
+    if (!(rel_tol >= 0.0)) return invalid("rel_tol must be >= 0");
+    if (S == 0) return MLCC_OK;
+    if (!a || !b || !out_max_err || !out_bijective) return invalid("null pointer");
+    int G = (int)ceil(sqrt((double)n));
+    if (G < 1) G = 1;
+    if (G > 2048) G = 2048;
+    const long long ncell = (long long)G * G;
+    const long long stride = (ncell + 1) + ncell + 2 * n;
+    const int sms = device_sm_count();
+    long long grid = 2ll * sms;
+    if (grid > S) grid = S;
+    Workspace ws(stream);
+    int *scratch = nullptr;
+    cudaError_t e = ws.alloc(&scratch, (size_t)(stride * grid));
+    if (e == cudaErrorMemoryAllocation) {
+        cudaGetLastError();
+        set_last_error("workspace allocation failed");
+        return MLCC_ERR_NOMEM;
+    }
+    MLCC_CUDA(e);
+    k_match<<<(int)grid, BLOCK, 0, stream>>>(reinterpret_cast<const double2 *>(a),
+                                            reinterpret_cast<const double2 *>(b), (long long)S, (int)n,
+                                            rel_tol, G, scratch, stride, out_max_err, out_bijective);
+    MLCC_CUDA(cudaGetLastError());
+    return MLCC_OK;
+}
+
+}  // namespace mlcc

@@ -1,0 +1,84 @@
+// mlcc_common.cuh — shared host/device helpers of libmlcc (product path; not used by oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string>
+
+#include "../../include/mlcc.h"
+
+namespace mlcc {
+
+// ---- error plumbing -------------------------------------------------------------------------
+void set_last_error(const std::string &msg);
+int cuda_fail(cudaError_t e, const char *what, const char *file, int line);
+
+#define MLCC_CUDA(call)                                                              \
+    do {                                                                             \
+        cudaError_t e__ = (call);                                                    \
+        if (e__ != cudaSuccess) return ::mlcc::cuda_fail(e__, #call, __FILE__, __LINE__); \
+    } while (0)
+
+inline int invalid(const char *msg)
+{
+    set_last_error(std::string("invalid argument: ") + msg);
+    return MLCC_ERR_INVALID_ARG;
+}
+
+// Stream-ordered workspace that frees itself (cudaFreeAsync) when it goes out of scope.
+struct Workspace {
+    cudaStream_t stream;
+    void *ptrs[32];
+    int n = 0;
+    explicit Workspace(cudaStream_t s) : stream(s) {}
+    ~Workspace()
+    {
+        for (int i = n - 1; i >= 0; --i) cudaFreeAsync(ptrs[i], stream);
+    }
+    template <typename T>
+    cudaError_t alloc(T **out, size_t count)
+    {
+        void *p = nullptr;
+        cudaError_t e = cudaMallocAsync(&p, count * sizeof(T) > 0 ? count * sizeof(T) : 16, stream);
+        if (e != cudaSuccess) return e;
+        if (n < 32) ptrs[n++] = p;
+        *out = static_cast<T *>(p);
+        return cudaSuccess;
+    }
+};
+
+int device_sm_count();
+
+// ---- device arithmetic ------------------------------------------------------------------------
+#ifdef __CUDACC__
+
+// MUFU.RCP64H seed: ~20 correct bits of 1/x from the high word of x (low word of the result is 0).
+__device__ __forceinline__ double rcp_seed(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    return y;
+}
+
+// Seed with the exponent clamped so that x = 0 (a root paired with itself) gives a finite
+// number: the pair's contribution conj(d) * inv is then exactly 0 instead of NaN.
+__device__ __forceinline__ double rcp_seed_finite(double x)
+{
+    double y = rcp_seed(x);
+    int hi = min(__double2hiint(y), 0x5FE00000);
+    return __hiloint2double(hi, 0);
+}
+
+// 1/x to ~1 ulp for normal positive x: one cubically convergent step from the 20-bit seed,
+// y1 = y0 (1 + e + e^2), e = 1 - x y0  (error e^3 ~ 2^-60 before rounding).  No slow path.
+__device__ __forceinline__ double rcp_full(double x)
+{
+    double y = rcp_seed_finite(x);
+    double e = fma(-x, y, 1.0);
+    double t = fma(e, e, e);
+    return fma(y, t, y);
+}
+
+#endif  // __CUDACC__
+
+}  // namespace mlcc

@@ -1,0 +1,124 @@
+"""CPU-only checks of the product's host side: the C-ABI library loads and exports every symbol
+include/mlcc.h declares; status strings; the sub-chain planner (host logic, no CUDA call);
+argument validation that is decided before any CUDA call."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2506_02121_b200 import build
+    build.build()
+    from paper_2506_02121_b200 import api
+    return api.lib()
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "mlcc.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(mlcc_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_every_declared_symbol_is_exported(lib):
+    names = declared_symbols()
+    assert len(names) >= 12 and "mlcc_critical_curves" in names and "mlcc_caustics" in names
+    for n in names:
+        assert hasattr(lib, n), n
+
+
+def test_version_and_status_strings(lib):
+    assert lib.mlcc_version() >= 100
+    lib.mlcc_status_string.restype = C.c_char_p
+    seen = {lib.mlcc_status_string(i).decode() for i in range(6)}
+    assert seen == {"MLCC_OK", "MLCC_ERR_INVALID_ARG", "MLCC_ERR_CUDA", "MLCC_ERR_NOMEM",
+                    "MLCC_ERR_NOT_CONVERGED", "MLCC_ERR_DEGENERATE"}
+    assert lib.mlcc_status_string(99).decode() == "MLCC_ERR_UNKNOWN"
+
+
+def test_options_default_and_struct_layout(lib):
+    from paper_2506_02121_b200 import api
+    o = api.options()
+    assert o.struct_size == C.sizeof(api.mlcc_options) == 40
+    assert o.predictor_order == -1 and o.num_subchains == 0 and o.phi_index_total == 0
+    assert C.sizeof(api.mlcc_stats) == 64
+
+
+@pytest.mark.parametrize("N,num_phi,req", [(10, 1000, 0), (200, 4000, 0), (2000, 5000, 0), (10000, 10000, 0),
+                                           (50000, 2000, 0), (3, 1, 0), (3, 7, 5), (5, 100, 7), (1, 2, 64)])
+def test_plan_subchains_covers_every_row_once(lib, N, num_phi, req):
+    from paper_2506_02121_b200 import api
+    first, centre, end = api.plan_subchains(N, num_phi, req)
+    n = len(first)
+    assert 1 <= n <= min(num_phi, 512)
+    if req:
+        assert n == min(req, num_phi)
+    assert first[0] == 0 and end[-1] == num_phi
+    assert np.all(first[1:] == end[:-1])          # contiguous, disjoint
+    assert np.all(end > first)                     # non-empty
+    assert np.all((centre >= first) & (centre < end))
+    # growing outwards from the centres reaches every row exactly once
+    seen = np.zeros(num_phi, int)
+    for c in range(n):
+        seen[centre[c]] += 1
+        s = 1
+        while centre[c] - s >= first[c] or centre[c] + s < end[c]:
+            if centre[c] - s >= first[c]:
+                seen[centre[c] - s] += 1
+            if centre[c] + s < end[c]:
+                seen[centre[c] + s] += 1
+            s += 1
+    assert np.all(seen == 1)
+
+
+def test_plan_subchains_rejects_bad_arguments(lib):
+    from paper_2506_02121_b200 import api
+    with pytest.raises(api.MlccError):
+        api.plan_subchains(0, 10)
+    with pytest.raises(api.MlccError):
+        api.plan_subchains(5, 0)
+
+
+def test_invalid_arguments_fail_before_any_cuda_call(lib):
+    """Null pointers and out-of-range scalars return MLCC_ERR_INVALID_ARG on a box with no GPU."""
+    from paper_2506_02121_b200 import api
+    L = lib
+    one = 16  # any non-null fake pointer: validation happens before it would be dereferenced
+    assert L.mlcc_critical_curves(None, one, 3, 0.0, 0.1, 10, 1e-12, 50, one) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_critical_curves(one, one, 0, 0.0, 0.1, 10, 1e-12, 50, one) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_critical_curves(one, one, 3, 0.0, 0.1, 0, 1e-12, 50, one) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_critical_curves(one, one, 3, 0.0, 0.1, 10, 0.0, 50, one) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_critical_curves(one, one, 3, 0.0, 0.1, 10, 1e-12, 0, one) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_critical_curves(one, one, 3, float("nan"), 0.1, 10, 1e-12, 50, one) == api.MLCC_ERR_INVALID_ARG
+    # c(phi_0) = (1 - kappa_s) - gamma = 0: the polynomial's degree drops on row 0
+    assert L.mlcc_critical_curves(one, one, 3, 0.5, 0.5, 10, 1e-12, 50, one) == api.MLCC_ERR_INVALID_ARG
+    assert b"c(phi_j)" in L.mlcc_last_error()
+    assert L.mlcc_caustics(None, one, 3, 0.0, 0.1, one, 5, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_caustics(one, one, 3, 0.0, 0.1, one, -1, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_caustics(one, one, 3, 0.0, 0.1, one, 5, one, None) == api.MLCC_ERR_INVALID_ARG  # aliasing
+    assert L.mlcc_caustics(one, one, 3, 0.0, 0.1, None, 0, None, None) == api.MLCC_OK              # P = 0
+    assert L.mlcc_match_root_sets(None, one, 2, 5, 1e-10, one, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_match_root_sets(one, one, 2, 0, 1e-10, one, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_match_root_sets(None, None, 0, 5, 1e-10, None, None, None) == api.MLCC_OK       # S = 0
+    assert L.mlcc_star_field(0, 0, 0.4, 0, None, one, one, None, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_star_field(0, 5, -1.0, 0, None, one, one, None, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_star_field(0, 5, 0.4, 7, None, one, one, None, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_fp64_peak(50.0, None, None) == api.MLCC_ERR_INVALID_ARG
+
+
+def test_product_does_not_import_the_oracle():
+    """The product path may not route through oracle/ (no CPU fallback)."""
+    pkg = os.path.join(ROOT, "paper_2506_02121_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle\b", text, flags=re.M), f
+                assert "liboracle" not in text and "mlcc_oracle" not in text, f
+    text = open(os.path.join(ROOT, "include", "mlcc.h")).read()
+    assert "oracle" not in text.lower()

@@ -1,0 +1,332 @@
+"""GPU parity tests: the CUDA path (through the C-ABI binding) against the CPU oracle on the same
+seeded inputs.  All inputs are generated on the CPU by the oracle's generator and uploaded; no oracle
+input or expected value comes from the CUDA path.
+
+Tolerances (BASELINE.json north_star): root sets per phase after nearest-neighbour matching
+max |dz| <= 1e-10 (1 + |z|); caustic points within 1e-9; integer outputs exact.
+"""
+import numpy as np
+import pytest
+
+from paper_2506_02121_b200.configs import CONFIGS
+from test_oracle_pins import check_row_invariants, c_phi, cplx
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+ROOT_TOL = 1e-10
+CAUSTIC_TOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def api():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2506_02121_b200 import api as a
+    a.lib()  # raises if libmlcc.so is missing: no fallback
+    return a
+
+
+def dev(x, dtype=torch.float64):
+    return torch.as_tensor(np.ascontiguousarray(x), dtype=dtype).cuda()
+
+
+def field(orc, cfg, N=None):
+    return orc.star_field(cfg.seed, N or cfg.N, cfg.kappa_star, cfg.mass_model, cfg.mass_params)
+
+
+def assert_rows_match(orc, gpu_rows, ref_rows, tol=ROOT_TOL):
+    """gpu_rows, ref_rows: [S, n, 2] numpy.  Oracle brute-force matching, b = reference."""
+    err, bij = orc.match_root_sets(gpu_rows, ref_rows, tol)
+    assert bij.all(), (np.where(bij == 0)[0][:10], err.max())
+    return err.max()
+
+
+def assert_caustics_match(g_roots, g_caus, ref_roots, ref_caus, tol=CAUSTIC_TOL):
+    """One row each: pair GPU roots with oracle roots (KD-tree), compare their caustic points."""
+    from scipy.spatial import cKDTree
+    dist, perm = cKDTree(ref_roots).query(g_roots)
+    assert len(set(perm.tolist())) == len(perm)
+    assert np.abs(cplx(g_caus) - cplx(ref_caus)[perm]).max() <= tol
+
+
+# ---------------------------------------------------------------------------------------------
+# a0 star field
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["cfg1", "cfg3", "cfg4", "cfg5"])
+def test_star_field_matches_oracle_generator(api, orc, name):
+    cfg = CONFIGS[name]
+    xy, m, R = api.star_field(cfg.seed, cfg.N, cfg.kappa_star, cfg.mass_model, cfg.mass_params)
+    oxy, om, oR = field(orc, cfg)
+    assert R == oR
+    assert np.array_equal(xy.cpu().numpy(), oxy)            # positions: bit-exact
+    assert np.abs(m.cpu().numpy() / om - 1).max() < 1e-14   # masses: pow() may differ by a few ulp
+    assert abs(float(m.sum()) - cfg.N) < 1e-9 * cfg.N
+
+
+def test_star_field_seed_and_defaults(api, orc):
+    a = api.star_field(5, 1000, 0.3, 2)
+    b = api.star_field(5, 1000, 0.3, 2, (0.01, 0.08, 0.5, 1.5, 0.3, 1.3, 2.3))
+    c = api.star_field(6, 1000, 0.3, 2)
+    assert torch.equal(a[0], b[0]) and torch.equal(a[1], b[1])
+    assert not torch.equal(a[0], c[0])
+    oxy, om, _ = orc.star_field(5, 1000, 0.3, 1, (0.1, 2.0, 1.0))   # alpha = 1 branch
+    gxy, gm, _ = api.star_field(5, 1000, 0.3, 1, (0.1, 2.0, 1.0))
+    assert np.array_equal(gxy.cpu().numpy(), oxy) and np.abs(gm.cpu().numpy() / om - 1).max() < 1e-14
+
+
+# ---------------------------------------------------------------------------------------------
+# a1-a6 critical curves, a7 caustics: full grids where the oracle finishes in seconds
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["cfg1", "cfg2"])
+def test_curves_and_caustics_full_grid(api, orc, name):
+    cfg = CONFIGS[name]
+    xy, m, R = field(orc, cfg)
+    ref, it_ref, un_ref = orc.critical_curves(xy, m, cfg.kappa_s, cfg.gamma, cfg.num_phi, cfg.tol, cfg.max_iter)
+    assert un_ref.sum() == 0
+    roots, iters, unconv, stats = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, cfg.num_phi,
+                                                         cfg.tol, cfg.max_iter)
+    assert int(unconv.sum()) == 0 and stats.unconverged_rows == 0 and stats.degenerate_roots == 0
+    assert int(iters.min()) >= 1 and int(iters.max()) <= cfg.max_iter
+    assert stats.root_iterations >= cfg.num_phi * 2 * cfg.N
+    g = roots.cpu().numpy()
+    assert_rows_match(orc, g, ref)
+    # caustics: GPU roots -> GPU caustics, oracle roots -> oracle caustics, compared through the matching
+    w_gpu = api.caustics(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, roots).cpu().numpy()
+    w_ref = orc.caustics(xy, m, cfg.kappa_s, cfg.gamma, ref)
+    for j in range(0, cfg.num_phi, max(1, cfg.num_phi // 200)):
+        assert_caustics_match(g[j], w_gpu[j], ref[j], w_ref[j])
+    # the same points through both caustic maps, element by element
+    w_same = api.caustics(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, dev(ref)).cpu().numpy()
+    assert np.abs(w_same - w_ref).max() <= 1e-12 * (1 + np.abs(w_ref).max())
+    # default-options entry point on the default stream
+    r2 = api.critical_curves(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, cfg.num_phi, cfg.tol, cfg.max_iter)
+    assert torch.equal(r2, roots)
+
+
+# ---------------------------------------------------------------------------------------------
+# full-size runs of the larger configs in the launch configuration bench.py times (default options):
+# oracle on sampled rows; invariants that hold at any size on all / many rows
+# ---------------------------------------------------------------------------------------------
+def vieta_all_rows(roots, xy, m, kappa_s, gamma, num_phi):
+    """sum z_k = 2 sum z_i and sum z_k^2 = 2 sum z_i^2 + 2 sum m / c(phi) on every row (torch on the device)."""
+    z = torch.view_as_complex(roots)
+    zs = torch.view_as_complex(dev(xy))
+    phi = 2 * np.pi * torch.arange(num_phi, device="cuda", dtype=torch.float64) / num_phi
+    c = (1 - kappa_s) * torch.exp(-1j * phi) - gamma
+    s1 = z.sum(dim=1)
+    s2 = (z * z).sum(dim=1)
+    scale1 = z.abs().sum(dim=1)
+    scale2 = (z.abs() ** 2).sum(dim=1)
+    e1 = (s1 - 2 * zs.sum()).abs() / scale1
+    e2 = (s2 - (2 * (zs * zs).sum() + 2 * float(m.sum()) / c)).abs() / scale2
+    return float(e1.max()), float(e2.max())
+
+
+@pytest.mark.parametrize("name,sample_rows", [("cfg3", [0, 1, 1250, 2499, 2500, 4999]),
+                                              ("cfg4", [0, 4999, 9999]),
+                                              ("cfg5", [1000])])
+def test_full_size_sampled_rows_and_invariants(api, orc, name, sample_rows):
+    cfg = CONFIGS[name]
+    xy, m, R = field(orc, cfg)
+    roots, iters, unconv, stats = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, cfg.num_phi,
+                                                         cfg.tol, cfg.max_iter)
+    torch.cuda.synchronize()
+    assert int(unconv.sum()) == 0 and stats.degenerate_roots == 0
+    assert int(iters.min()) >= 1
+    # properties that hold at any size, every row: Vieta sums (complete, no duplicated root)
+    e1, e2 = vieta_all_rows(roots, xy, m, cfg.kappa_s, cfg.gamma, cfg.num_phi)
+    assert e1 < 1e-12 and e2 < 1e-12, (e1, e2)
+    # sampled rows against the oracle (each row cold-started by the oracle on its own)
+    for j in sample_rows:
+        ref, _, un = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, cfg.num_phi, [j], cfg.tol, cfg.max_iter)
+        assert un.sum() == 0
+        g = roots[j:j + 1].cpu().numpy()
+        assert_rows_match(orc, g, ref)
+        # caustic points of that row
+        w_gpu = api.caustics(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, roots[j:j + 1].contiguous()).cpu().numpy()
+        w_ref = orc.caustics(xy, m, cfg.kappa_s, cfg.gamma, ref)
+        assert_caustics_match(g[0], w_gpu[0], ref[0], w_ref[0])
+    # certificates on more rows than the oracle can solve: long-double residuals, det J, distinctness
+    rng = np.random.default_rng(1)
+    for j in rng.choice(cfg.num_phi, size=4, replace=False):
+        check_row_invariants(orc, xy, m, cfg.kappa_s, cfg.gamma, int(j), cfg.num_phi,
+                             cplx(roots[int(j)].cpu().numpy()))
+
+
+# ---------------------------------------------------------------------------------------------
+# options do not change the answer (the iteration path is not part of the contract)
+# ---------------------------------------------------------------------------------------------
+def test_options_do_not_change_the_root_sets(api, orc):
+    cfg = CONFIGS["cfg2"]
+    xy, m, R = field(orc, cfg)
+    num_phi = 240
+    ref, _, _ = orc.critical_curves(xy, m, cfg.kappa_s, cfg.gamma, num_phi)
+    dxy, dm = dev(xy), dev(m)
+    seen_iters = {}
+    for order in range(0, 6):
+        for nsub in (1, 3, 16):
+            r, it, un, st = api.critical_curves_ex(dxy, dm, cfg.kappa_s, cfg.gamma, num_phi,
+                                                   opt=api.options(num_subchains=nsub, predictor_order=order))
+            assert st.subchains == nsub and st.predictor_order == order and int(un.sum()) == 0
+            assert_rows_match(orc, r.cpu().numpy(), ref)
+            seen_iters[(order, nsub)] = st.root_iterations
+    # the predictor only removes work
+    assert seen_iters[(3, 1)] < seen_iters[(0, 1)]
+    for T in (1, 2, 4, 8, 16, 32, 64, 128, 256):
+        r, it, un, st = api.critical_curves_ex(dxy, dm, cfg.kappa_s, cfg.gamma, num_phi,
+                                               opt=api.options(num_subchains=4, min_lanes_per_root=T))
+        assert_rows_match(orc, r.cpu().numpy(), ref)
+
+
+def test_phase_offset_selects_rows_of_a_larger_grid(api, orc):
+    """Rows [off, off+n) of a num_phi_total grid: the multi-GPU sharding contract."""
+    cfg = CONFIGS["cfg1"]
+    xy, m, R = field(orc, cfg)
+    total, off, n = 1000, 300, 120
+    ref, _, _ = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, total, np.arange(off, off + n))
+    r, it, un, st = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, n,
+                                           opt=api.options(phi_index_offset=off, phi_index_total=total))
+    assert_rows_match(orc, r.cpu().numpy(), ref)
+
+
+def test_init_roots_replace_the_cold_seeds(api, orc):
+    # one star with gamma > 1 - kappa_s at phi = 0: z_i +/- 1 stay on the real axis for ever
+    # (reading R6); rotated seeds converge to +/- i sqrt(m / (gamma - (1 - kappa_s)))
+    xy = np.array([[0.0, 0.0]])
+    m = np.array([1.0])
+    ks, g = 0.5, 0.8
+    init = np.array([[np.cos(0.3), np.sin(0.3)], [-np.cos(0.3), -np.sin(0.3)]])
+    r, it, un, st = api.critical_curves_ex(dev(xy), dev(m), ks, g, 1, init_roots=dev(init),
+                                           opt=api.options(num_subchains=1))
+    z = cplx(r.cpu().numpy())[0]
+    want = np.sqrt(1.0 / c_phi(ks, g, 0.0) + 0j)
+    assert min(abs(z[0] - want), abs(z[0] + want)) < 1e-14 and abs(z[0] + z[1]) < 1e-14
+    oref, _, _ = orc.critical_curve_rows(xy, m, ks, g, 1, [0], init_roots=init)
+    assert_rows_match(orc, r.cpu().numpy(), oref)
+
+
+# ---------------------------------------------------------------------------------------------
+# degenerate and edge cases
+# ---------------------------------------------------------------------------------------------
+def test_smallest_problem_single_star_single_phase(api, orc):
+    xy = np.array([[0.3, -0.2]])
+    m = np.array([1.7])
+    r, it, un, st = api.critical_curves_ex(dev(xy), dev(m), 0.1, 0.2, 1)
+    ref, _, _ = orc.critical_curves(xy, m, 0.1, 0.2, 1)
+    assert r.shape == (1, 2, 2)
+    assert_rows_match(orc, r.cpu().numpy(), ref)
+    w = api.caustics(dev(xy), dev(m), 0.1, 0.2, r).cpu().numpy()
+    assert np.abs(np.sort_complex(cplx(w)[0]) - np.sort_complex(cplx(orc.caustics(xy, m, 0.1, 0.2, ref))[0])).max() < 1e-12
+
+
+def test_ragged_sizes_span_tiles(api, orc):
+    """N chosen so that stars and roots straddle the 1024-wide shared-memory tiles with a ragged tail."""
+    for N, num_phi in ((513, 7), (1025, 5), (37, 33)):
+        xy, m, R = orc.star_field(11, N, 0.35, 1)
+        ref, _, un = orc.critical_curves(xy, m, 0.05, 0.3, num_phi)
+        assert un.sum() == 0
+        r, it, unc, st = api.critical_curves_ex(dev(xy), dev(m), 0.05, 0.3, num_phi)
+        assert_rows_match(orc, r.cpu().numpy(), ref)
+        pts = np.random.default_rng(N).normal(size=(777, 2)) * R
+        w = api.caustics(dev(xy), dev(m), 0.05, 0.3, dev(pts)).cpu().numpy()
+        wr = orc.caustics(xy, m, 0.05, 0.3, pts)
+        assert np.abs(w - wr).max() <= 1e-12 * (1 + np.abs(wr).max())
+
+
+def test_max_iter_reports_unconverged_but_writes_everything(api, orc):
+    cfg = CONFIGS["cfg2"]
+    xy, m, R = field(orc, cfg)
+    r, it, un, st = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, 8, max_iter=2,
+                                           opt=api.options(num_subchains=1), strict=False)
+    assert st.status == api.MLCC_ERR_NOT_CONVERGED and st.unconverged_rows >= 1
+    assert int(un.max()) > 0 and int(it.max()) == 2
+    assert torch.isfinite(r).all()
+    with pytest.raises(api.MlccError) as e:
+        api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, 8, max_iter=2)
+    assert e.value.status == api.MLCC_ERR_NOT_CONVERGED
+    # the oracle agrees on which rows are unfinished after 2 sweeps of the cold row
+    _, it_o, un_o = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, 8, [4], max_iter=2)
+    assert un_o[0] > 0 and it_o[0] == 2 and int(un[4]) == int(un_o[0])
+
+
+def test_coincident_stars_are_reported_degenerate(api):
+    xy = np.array([[0.5, 0.5], [0.5, 0.5], [-1.0, 0.2]])
+    m = np.ones(3)
+    # two stars at one point: P(z) has only 2N - 2 roots, the degree claim fails
+    with pytest.raises(api.MlccError) as e:
+        api.critical_curves_ex(dev(xy), dev(m), 0.0, 0.1, 4)
+    assert e.value.status == api.MLCC_ERR_DEGENERATE
+    xy[1, 0] = np.nan
+    with pytest.raises(api.MlccError) as e:
+        api.critical_curves_ex(dev(xy), dev(m), 0.0, 0.1, 4)
+    assert e.value.status == api.MLCC_ERR_INVALID_ARG
+
+
+def test_empty_inputs(api):
+    xy, m = dev(np.zeros((2, 2))), dev(np.ones(2))
+    empty = torch.empty((0, 2), dtype=torch.float64, device="cuda")
+    assert api.caustics(xy, m, 0.0, 0.1, empty).shape == (0, 2)
+    e, b = api.match_root_sets(torch.empty((0, 5, 2), dtype=torch.float64, device="cuda"),
+                               torch.empty((0, 5, 2), dtype=torch.float64, device="cuda"), 1e-10)
+    assert e.shape == (0,) and b.shape == (0,)
+
+
+def test_binding_rejects_cpu_tensors(api):
+    with pytest.raises(TypeError):
+        api.caustics(torch.zeros(2, 2, dtype=torch.float64), torch.ones(2, dtype=torch.float64).cuda(), 0, 0.1,
+                     torch.zeros(3, 2, dtype=torch.float64).cuda())
+
+
+# ---------------------------------------------------------------------------------------------
+# a8 validator against the oracle's brute force
+# ---------------------------------------------------------------------------------------------
+def test_match_root_sets_against_brute_force(api, orc):
+    rng = np.random.default_rng(3)
+    for S, n in ((5, 1), (7, 2), (6, 40), (3, 1000), (2, 20011)):
+        b = rng.normal(size=(S, n, 2)) * 50
+        a = np.empty_like(b)
+        for s in range(S):
+            a[s] = b[s][rng.permutation(n)] + rng.normal(size=(n, 2)) * 1e-12
+        if n >= 40:
+            a[0, 3] = a[0, 5]            # duplicated root, one missing
+            a[1, 0, 0] += 1e-3           # beyond tolerance
+            a[2, 7] += 30.0              # far from everything: exercises the ring expansion / fallback
+        e_o, b_o = orc.match_root_sets(a, b, 1e-10)
+        e_g, b_g = api.match_root_sets(dev(a), dev(b), 1e-10)
+        assert b_g.cpu().numpy().tolist() == b_o.tolist()
+        assert np.abs(e_g.cpu().numpy() - e_o).max() <= 1e-15 * (1 + e_o.max())
+    # clustered sets with an outlier pair (the shape of a critical-curve row) and a non-finite value
+    cfg = CONFIGS["cfg2"]
+    xy, m, R = field(orc, cfg)
+    ref, _, _ = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, 16, np.arange(4))
+    a = ref[:, rng.permutation(ref.shape[1])] + 1e-13
+    e_o, b_o = orc.match_root_sets(a, ref, 1e-10)
+    e_g, b_g = api.match_root_sets(dev(a), dev(ref), 1e-10)
+    assert b_o.all() and b_g.cpu().numpy().all() and np.abs(e_g.cpu().numpy() - e_o).max() < 1e-18
+    a[1, 2, 0] = np.nan
+    e_g, b_g = api.match_root_sets(dev(a), dev(ref), 1e-10)
+    assert b_g.cpu().numpy().tolist() == [1, 0, 1, 1] and np.isinf(e_g.cpu().numpy()[1])
+
+
+# ---------------------------------------------------------------------------------------------
+# host-buffer entry points
+# ---------------------------------------------------------------------------------------------
+def test_host_buffer_entry_points(api, orc):
+    cfg = CONFIGS["cfg1"]
+    xy, m, R = field(orc, cfg)
+    roots_h, caus_h, st = api.curves_and_caustics_host(xy, m, cfg.kappa_s, cfg.gamma, 200)
+    ref, _, _ = orc.critical_curves(xy, m, cfg.kappa_s, cfg.gamma, 200)
+    assert_rows_match(orc, roots_h, ref)
+    ref_caus = orc.caustics(xy, m, cfg.kappa_s, cfg.gamma, ref)
+    for j in range(0, 200, 7):
+        assert_caustics_match(roots_h[j], caus_h[j], ref[j], ref_caus[j])
+    r2 = api.critical_curves_host(xy, m, cfg.kappa_s, cfg.gamma, 200)
+    assert np.array_equal(r2, roots_h)
+    c2 = api.caustics_host(xy, m, cfg.kappa_s, cfg.gamma, ref)
+    assert np.abs(c2 - orc.caustics(xy, m, cfg.kappa_s, cfg.gamma, ref)).max() < 1e-12
+
+
+def test_fp64_peak_probe_is_plausible(api):
+    tf = api.fp64_peak(20.0)
+    assert 5.0 < tf < 80.0, tf
