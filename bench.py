@@ -1,0 +1,293 @@
+#!/usr/bin/env python
+"""bench.py — converged critical-curve roots/s on the headline workload (BASELINE.json: N = 10^4 stars, fp64).
+
+One "step" is one pass of the whole hot path over the cfg4 workload, through the C-ABI:
+  a0 mlcc_star_field -> a1..a6 mlcc_critical_curves_ex -> a7 mlcc_caustics -> a8 mlcc_match_root_sets
+(the validator compares the step's root sets with those of the previous step: the run-to-run check).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg4] [--num-phi M]
+N > 1: launched by torch.distributed.run, one rank per GPU; the phase grid is N times as long and rank r owns
+rows [r*num_phi, (r+1)*num_phi) (weak scaling, no data-path collective).
+
+Prints ONE JSON line (rank 0).  `--impl reference` times the CPU oracle on the host cores instead.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_2506_02121_b200.configs import CONFIGS, HEADLINE  # noqa: E402
+
+METRIC = "converged critical-curve roots/s"
+UNIT = "roots/s"
+FLOP_PER_STAR_PAIR = 27.0   # algorithmic flop per (root, star) pair, 1 reciprocal = 1 flop
+FLOP_PER_ROOT_PAIR = 10.0   # per (root, root) pair
+NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # SMs x FP64 lanes x 2 flop x max SM clock
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default=HEADLINE, choices=sorted(CONFIGS))
+    ap.add_argument("--num-phi", type=int, default=0, help="override the number of phases (profiling runs)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--subchains", type=int, default=0)
+    ap.add_argument("--order", type=int, default=-1)
+    ap.add_argument("--min-lanes", type=int, default=0)
+    return ap.parse_args()
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region (B200_PROFILING.md)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index=0):
+        self.rows, self.proc, self.thread, self.gpu = [], None, None, gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "200", "-i", str(self.gpu)], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 9:
+                continue
+            try:
+                sm.append(float(r[1])); smax.append(float(r[2])); power.append(float(r[3]))
+            except ValueError:
+                continue
+            for n, v in zip(names, r[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(cfg, rows, num_phi_total, j_offset=0):
+    """Times the oracle as it stands on `rows` (first row cold-started, the rest continued). -> (seconds, roots)."""
+    import oracle
+    xy, m, R = oracle.star_field(cfg.seed, cfg.N, cfg.kappa_star, cfg.mass_model, cfg.mass_params)
+    t0 = time.perf_counter()
+    roots, iters, unconv = oracle.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, num_phi_total, rows, cfg.tol,
+                                                      cfg.max_iter, j_offset=j_offset)
+    oracle.caustics(xy, m, cfg.kappa_s, cfg.gamma, roots)
+    dt = time.perf_counter() - t0
+    return dt, len(rows) * 2 * cfg.N, oracle.num_threads()
+
+
+def run_reference(args, cfg, num_phi):
+    """--impl reference: the CPU oracle on a bounded sample of the workload per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    # cold row + a few continued rows, sized to ~10 s per step at N = 10^4 on 16 cores
+    n_rows = 3 if cfg.N >= 5000 else (8 if cfg.N >= 1000 else min(num_phi, 200))
+    rows = list(range(num_phi // 2, num_phi // 2 + n_rows))
+    for _ in range(args.warmup):
+        oracle_sample(cfg, rows[:1] if cfg.N >= 5000 else rows, num_phi)
+    t_all, roots_all, cores = 0.0, 0, 1
+    for _ in range(args.steps):
+        dt, nroots, cores = oracle_sample(cfg, rows, num_phi)
+        t_all += dt
+        roots_all += nroots
+    value = roots_all / t_all
+    sample = (f"per step: rows {rows[0]}..{rows[-1]} of {num_phi} (first cold-started from z_i+/-1, the rest continued) "
+              f"+ their caustic points")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_all / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{cfg.name}: N={cfg.N}, num_phi={num_phi} (bounded sample)", "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    args = parse()
+    cfg = CONFIGS[args.workload]
+    num_phi = args.num_phi or cfg.num_phi
+    if args.impl == "reference":
+        run_reference(args, cfg, num_phi)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2506_02121_b200 import api
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    api.lib()
+    n_r = 2 * cfg.N
+    opt = api.options(num_subchains=args.subchains, predictor_order=args.order, min_lanes_per_root=args.min_lanes,
+                      phi_index_offset=rank * num_phi, phi_index_total=world * num_phi)
+
+    roots = torch.empty((num_phi, n_r, 2), dtype=torch.float64, device="cuda")
+    prev = torch.empty_like(roots)
+    caus = torch.empty_like(roots)
+    last = {}
+
+    def step():
+        xy, m, R = api.star_field(cfg.seed, cfg.N, cfg.kappa_star, cfg.mass_model, cfg.mass_params)
+        _, _, _, st = api.critical_curves_ex(xy, m, cfg.kappa_s, cfg.gamma, num_phi, cfg.tol, cfg.max_iter, opt=opt,
+                                             out_roots=roots, want_diagnostics=False)
+        api.caustics(xy, m, cfg.kappa_s, cfg.gamma, roots, out=caus)
+        err, bij = api.match_root_sets(roots, prev, 1e-10)
+        last.update(stats=st, err=err, bij=bij)
+        return st
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # warm-up (also fills `prev` for the validator)
+    for w in range(max(args.warmup, 1)):
+        step()
+        prev.copy_(roots)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    solve_ms = 0.0
+    launches = 0
+    alg_flop = 0.0
+    compute_launches = 0
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        st = step()
+        solve_ms += st.solve_ms
+        launches += st.kernel_launches + 3 + 1 + 1      # star field (3 kernels), caustics, matcher
+        alg_flop += FLOP_PER_STAR_PAIR * st.star_pairs + FLOP_PER_ROOT_PAIR * st.root_pairs
+        compute_launches += st.total_iterations
+    ev1.record()
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    clocks = sampler.stop() if rank == 0 else None
+    st = last["stats"]
+    assert bool(last["bij"].all()), "validator: this step's root sets differ from the previous step's"
+    assert st.unconverged_rows == 0 and st.degenerate_roots == 0
+    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    ms_per_step = ms_max / args.steps
+    value = world * num_phi * n_r / (ms_per_step * 1e-3)
+
+    # ---- roofline of the dominant kernel (the Aberth compute kernel): FP64 ALU bound ----
+    peak_measured = api.fp64_peak(50.0) if rank == 0 else 0.0
+    achieved = alg_flop / (solve_ms * 1e-3) / 1e12 if solve_ms > 0 else 0.0
+    roofline = {"bound": "alu", "kernel": "mlcc::k_compute (Aberth iteration)", "achieved": achieved,
+                "peak": peak_measured, "unit": "TFLOP/s", "frac": achieved / peak_measured if peak_measured else None,
+                "peak_source": "measured on this GPU by mlcc_fp64_peak (dependent-free DFMA loop); "
+                               f"nominal {NOMINAL_FP64_TFLOPS:.1f} TFLOP/s = 148 SMs x 64 lanes x 2 x 1.965 GHz",
+                "frac_of_nominal": achieved / NOMINAL_FP64_TFLOPS,
+                "algorithmic_flop_per_launch": alg_flop / max(compute_launches, 1),
+                "avg_launch_ms": solve_ms / max(compute_launches, 1),
+                "note": "achieved = (27 flop x star pairs + 10 flop x root pairs of unfrozen roots) / device time of the "
+                        "whole solve (seed/apply/finalize launches included), CUDA events on the launch stream",
+                "traffic": None}
+
+    # ---- end to end through the host-buffer C-ABI call (pinned host memory both ways) ----
+    e2e = None
+    if not args.no_e2e:
+        gxy, gm, _ = api.star_field(cfg.seed, cfg.N, cfg.kappa_star, cfg.mass_model, cfg.mass_params)
+        p_xy = gxy.cpu().pin_memory()     # the user's host arrays (outside the timed region)
+        p_m = gm.cpu().pin_memory()
+        h_roots = torch.empty((num_phi, n_r, 2), dtype=torch.float64, pin_memory=True)
+        h_caus = torch.empty((num_phi, n_r, 2), dtype=torch.float64, pin_memory=True)
+        del prev
+        torch.cuda.empty_cache()
+        api.curves_and_caustics_host(p_xy, p_m, cfg.kappa_s, cfg.gamma, num_phi, cfg.tol, cfg.max_iter, opt=opt,
+                                     out_roots=h_roots, out_caustics=h_caus)       # warm-up
+        barrier()
+        t0 = time.perf_counter()
+        n_e2e = max(1, min(args.steps, 2))
+        for _ in range(n_e2e):
+            api.curves_and_caustics_host(p_xy, p_m, cfg.kappa_s, cfg.gamma, num_phi, cfg.tol, cfg.max_iter, opt=opt,
+                                         out_roots=h_roots, out_caustics=h_caus)
+        torch.cuda.synchronize()
+        dt = (time.perf_counter() - t0) / n_e2e
+        te = torch.tensor([dt], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * num_phi * n_r / float(te.item()), "unit": UNIT,
+               "h2d_bytes_per_step": int(p_xy.numel() * 8 + p_m.numel() * 8),
+               "d2h_bytes_per_step": int(h_roots.numel() * 8 + h_caus.numel() * 8),
+               "seconds_per_step": float(te.item()),
+               "call": "mlcc_curves_and_caustics_host (host pointers; device alloc + H2D + solve + caustics + D2H inside)"}
+
+    # ---- CPU baseline: the oracle as it stands on a bounded sample (rank 0, N = 1 only) ----
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        n_rows = 3 if cfg.N >= 5000 else (8 if cfg.N >= 1000 else min(num_phi, 200))
+        rows = list(range(num_phi // 2, num_phi // 2 + n_rows))
+        dt, nroots, cores = oracle_sample(cfg, rows, num_phi)
+        cpu = {"value": nroots / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
+               "sample": f"rows {rows[0]}..{rows[-1]} of {num_phi} ({n_rows} phases: first cold-started from z_i+/-1, "
+                         f"the rest continued) + their caustic points"}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": f"{cfg.name}: N={cfg.N} stars, {num_phi} phases per GPU, kappa_star={cfg.kappa_star}, "
+                                       f"kappa_s={cfg.kappa_s}, gamma={cfg.gamma}, tol={cfg.tol}, max_iter={cfg.max_iter}, seed={cfg.seed}",
+                           "step": "star_field + critical_curves_ex + caustics + match_root_sets",
+                           "subchains": st.subchains, "predictor_order": st.predictor_order,
+                           "l2": f"inputs larger than L2: each step writes {2 * num_phi * n_r * 16 / 1e9:.2f} GB of roots and caustics "
+                                 f"and reads a {num_phi * n_r * 16 / 1e9:.2f} GB comparison set (L2 is 126 MB)",
+                           "seconds_per_curve_set": st.solve_ms * 1e-3,
+                           "aberth_iterations_per_step": st.total_iterations,
+                           "root_iterations_per_root": st.root_iterations / float(num_phi * n_r)},
+                "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -37,7 +37,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     for u in UNITS:
         obj = os.path.join(objdir, u.replace(".cu", ".o"))
         objs.append(obj)
-        cmd = [nvcc, *NVCC_FLAGS, "-I", INCLUDE, "-c", os.path.join(CSRC, u), "-o", obj]
+        extra = os.environ.get("MLCC_EXTRA_NVCC_FLAGS", "").split()   # tuning experiments only
+        cmd = [nvcc, *NVCC_FLAGS, *extra, "-I", INCLUDE, "-c", os.path.join(CSRC, u), "-o", obj]
         procs.append((u, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     log = []
     for u, pr in procs:

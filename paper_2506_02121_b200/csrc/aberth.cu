@@ -33,6 +33,18 @@ constexpr int BLOCK = 256;        // threads per CTA of the compute kernel
 constexpr int TILE = 1024;        // sources staged in shared memory per tile
 constexpr int MAX_ORDER = 5;      // highest predictor order
 constexpr int MAX_SLOTS = 1024;   // most slots in one step (2 per sub-chain)
+constexpr double TINY = 1e-300;   // added to |d|^2: makes the self pair finite, invisible otherwise
+#ifndef MLCC_U_STAR
+#define MLCC_U_STAR 4
+#endif
+#ifndef MLCC_U_ROOT
+#define MLCC_U_ROOT 8
+#endif
+#ifndef MLCC_MIN_BLOCKS
+#define MLCC_MIN_BLOCKS 2
+#endif
+constexpr int U_STAR = MLCC_U_STAR;   // pairs in flight per thread in the star loop
+constexpr int U_ROOT = MLCC_U_ROOT;   // ... in the root loop (even)
 
 struct DevState {
     int step;             // current step: 0 = cold centre rows, s >= 1 = rows centre +/- s
@@ -100,7 +112,7 @@ __device__ __forceinline__ void pair_star(double zx, double zy, double2 s, doubl
 {
     double dx = zx - s.x;
     double dy = s.y - zy;
-    double r2 = fma(dy, dy, dx * dx);
+    double r2 = fma(dy, dy, fma(dx, dx, TINY));
     double inv = rcp_full(r2);
     double wx = dx * inv;
     double wy = dy * inv;
@@ -119,14 +131,15 @@ __device__ __forceinline__ void pair_star(double zx, double zy, double2 s, doubl
 }
 
 // (root, root): A += 1/(z_k - z_r).  Only the convergence RATE depends on A (the fixed point of
-// the update is F = 0 whatever A is), so the 20-bit reciprocal seed is used as it is; a root paired
-// with itself has d = 0 exactly and contributes 0 because the seed is clamped to a finite value.
+// the update is F = 0 whatever A is), so the 20-bit reciprocal seed is used as it is.  A root
+// paired with itself has d = 0 exactly: |d|^2 + TINY = 1e-300, the seed is finite, and the pair
+// contributes conj(d) * inv = 0.  For every other pair TINY is lost in the rounding of |d|^2.
 __device__ __forceinline__ void pair_root(double zx, double zy, double2 r, double &ax, double &ay)
 {
     double dx = zx - r.x;
     double dy = r.y - zy;
-    double r2 = fma(dy, dy, dx * dx);
-    double inv = rcp_seed_finite(r2);
+    double r2 = fma(dy, dy, fma(dx, dx, TINY));
+    double inv = rcp_seed(r2);
     ax = fma(dx, inv, ax);
     ay = fma(dy, inv, ay);
 }
@@ -181,7 +194,7 @@ __global__ void k_seed(Params p)
 // ------------------------------------------------------------------------------------------------
 // compute kernel
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(BLOCK, 2) k_compute(Params p)
+__global__ void __launch_bounds__(BLOCK, MLCC_MIN_BLOCKS) k_compute(Params p)
 {
     __shared__ double2 s_xy[TILE];
     __shared__ double s_m[TILE];
@@ -222,7 +235,7 @@ __global__ void __launch_bounds__(BLOCK, 2) k_compute(Params p)
             zx = z.x;
             zy = z.y;
         }
-        double s1x = 0, s1y = 0, s2x = 0, s2y = 0, s3x = 0, s3y = 0, ax = 0, ay = 0;
+        double s1x = 0, s1y = 0, s2x = 0, s2y = 0, s3x = 0, s3y = 0, ax = 0, ay = 0, bx = 0, by = 0;
 
         // ---- stars ----
         for (int base = 0; base < p.N; base += TILE) {
@@ -234,8 +247,19 @@ __global__ void __launch_bounds__(BLOCK, 2) k_compute(Params p)
             }
             __syncthreads();
             if (valid) {
-#pragma unroll 4
-                for (int j = sub; j < cnt; j += T)
+                // blocks of U_STAR independent pairs with no exit in between, so that their
+                // dependent chains (|d|^2 -> reciprocal -> powers) interleave; then the ragged tail
+                int j = sub;
+                for (; j + (U_STAR - 1) * T < cnt; j += U_STAR * T) {
+                    double2 s[U_STAR];
+                    double m[U_STAR];
+#pragma unroll
+                    for (int u = 0; u < U_STAR; ++u) { s[u] = s_xy[j + u * T]; m[u] = s_m[j + u * T]; }
+#pragma unroll
+                    for (int u = 0; u < U_STAR; ++u)
+                        pair_star(zx, zy, s[u], m[u], s1x, s1y, s2x, s2y, s3x, s3y);
+                }
+                for (; j < cnt; j += T)
                     pair_star(zx, zy, s_xy[j], s_m[j], s1x, s1y, s2x, s2y, s3x, s3y);
             }
         }
@@ -246,13 +270,23 @@ __global__ void __launch_bounds__(BLOCK, 2) k_compute(Params p)
             for (int i = tid; i < cnt; i += BLOCK) s_xy[i] = zrow[base + i];
             __syncthreads();
             if (valid) {
-#pragma unroll 4
-                for (int j = sub; j < cnt; j += T) pair_root(zx, zy, s_xy[j], ax, ay);
+                int j = sub;
+                for (; j + (U_ROOT - 1) * T < cnt; j += U_ROOT * T) {
+                    double2 r[U_ROOT];
+#pragma unroll
+                    for (int u = 0; u < U_ROOT; ++u) r[u] = s_xy[j + u * T];
+#pragma unroll
+                    for (int u = 0; u < U_ROOT; u += 2) {   // two accumulator chains
+                        pair_root(zx, zy, r[u], ax, ay);
+                        pair_root(zx, zy, r[u + 1], bx, by);
+                    }
+                }
+                for (; j < cnt; j += T) pair_root(zx, zy, s_xy[j], ax, ay);
             }
         }
         // ---- reduce the T partial sums ----
-        double tx = 2.0 * s1x - ax;   // 2 S1 - A
-        double ty = 2.0 * s1y - ay;
+        double tx = 2.0 * s1x - (ax + bx);   // 2 S1 - A
+        double ty = 2.0 * s1y - (ay + by);
         for (int o = TL >> 1; o > 0; o >>= 1) {
             s2x += __shfl_xor_sync(0xffffffffu, s2x, o);
             s2y += __shfl_xor_sync(0xffffffffu, s2y, o);

@@ -51,7 +51,7 @@ __global__ void __launch_bounds__(BLOCK) k_caustics(const double2 *__restrict__ 
                     const double2 s = s_xy[j];
                     const double dx = zx - s.x;
                     const double dy = zy - s.y;
-                    const double r2 = fma(dy, dy, dx * dx);
+                    const double r2 = fma(dy, dy, fma(dx, dx, 1e-300));   // a point on a star contributes 0
                     const double minv = s_m[j] * rcp_full(r2);
                     ax = fma(dx, minv, ax);
                     ay = fma(dy, minv, ay);

@@ -283,7 +283,7 @@ def test_binding_rejects_cpu_tensors(api):
 # ---------------------------------------------------------------------------------------------
 def test_match_root_sets_against_brute_force(api, orc):
     rng = np.random.default_rng(3)
-    for S, n in ((5, 1), (7, 2), (6, 40), (3, 1000), (2, 20011)):
+    for S, n in ((5, 1), (7, 2), (6, 40), (3, 1000), (3, 20011)):
         b = rng.normal(size=(S, n, 2)) * 50
         a = np.empty_like(b)
         for s in range(S):
