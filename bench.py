@@ -2,7 +2,7 @@
 """bench.py — converged critical-curve roots/s on the headline workload (BASELINE.json: N = 10^4 stars, fp64).
 
 One "step" is one pass of the whole hot path over the cfg4 workload, through the C-ABI:
-  a0 mlcc_star_field -> a1..a6 mlcc_critical_curves_ex -> a7 mlcc_caustics -> a8 mlcc_match_root_sets
+  a0 mlcc_star_field -> a1..a7 mlcc_curves_and_caustics (caustic map fused into the Aberth kernel) -> a8 mlcc_match_root_sets
 (the validator compares the step's root sets with those of the previous step: the run-to-run check).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg4] [--num-phi M]
@@ -47,6 +47,10 @@ def parse():
     ap.add_argument("--subchains", type=int, default=0)
     ap.add_argument("--order", type=int, default=-1)
     ap.add_argument("--min-lanes", type=int, default=0)
+    ap.add_argument("--aberth-sum", type=int, default=0, choices=[0, 32, 64],
+                    help="arithmetic of the Aberth sum: 32 = double-single FP32 (default), 64 = FP64 seed form")
+    ap.add_argument("--separate-caustics", action="store_true",
+                    help="run mlcc_critical_curves_ex + mlcc_caustics instead of the fused call")
     return ap.parse_args()
 
 
@@ -161,7 +165,8 @@ def main():
     api.lib()
     n_r = 2 * cfg.N
     opt = api.options(num_subchains=args.subchains, predictor_order=args.order, min_lanes_per_root=args.min_lanes,
-                      phi_index_offset=rank * num_phi, phi_index_total=world * num_phi)
+                      phi_index_offset=rank * num_phi, phi_index_total=world * num_phi,
+                      aberth_sum_precision=args.aberth_sum)
 
     roots = torch.empty((num_phi, n_r, 2), dtype=torch.float64, device="cuda")
     prev = torch.empty_like(roots)
@@ -170,9 +175,14 @@ def main():
 
     def step():
         xy, m, R = api.star_field(cfg.seed, cfg.N, cfg.kappa_star, cfg.mass_model, cfg.mass_params)
-        _, _, _, st = api.critical_curves_ex(xy, m, cfg.kappa_s, cfg.gamma, num_phi, cfg.tol, cfg.max_iter, opt=opt,
-                                             out_roots=roots, want_diagnostics=False)
-        api.caustics(xy, m, cfg.kappa_s, cfg.gamma, roots, out=caus)
+        if args.separate_caustics:
+            _, _, _, st = api.critical_curves_ex(xy, m, cfg.kappa_s, cfg.gamma, num_phi, cfg.tol, cfg.max_iter,
+                                                 opt=opt, out_roots=roots, want_diagnostics=False)
+            api.caustics(xy, m, cfg.kappa_s, cfg.gamma, roots, out=caus)
+        else:
+            _, _, _, _, st = api.curves_and_caustics(xy, m, cfg.kappa_s, cfg.gamma, num_phi, cfg.tol, cfg.max_iter,
+                                                     opt=opt, out_roots=roots, out_caustics=caus,
+                                                     want_diagnostics=False)
         err, bij = api.match_root_sets(roots, prev, 1e-10)
         last.update(stats=st, err=err, bij=bij)
         return st
@@ -200,7 +210,7 @@ def main():
     for _ in range(args.steps):
         st = step()
         solve_ms += st.solve_ms
-        launches += st.kernel_launches + 3 + 1 + 1      # star field (3 kernels), caustics, matcher
+        launches += st.kernel_launches + 3 + 1 + (1 if args.separate_caustics else 0)   # star field (3), matcher, caustics
         alg_flop += FLOP_PER_STAR_PAIR * st.star_pairs + FLOP_PER_ROOT_PAIR * st.root_pairs
         compute_launches += st.total_iterations
     ev1.record()
@@ -276,7 +286,9 @@ def main():
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                 "config": {"workload": f"{cfg.name}: N={cfg.N} stars, {num_phi} phases per GPU, kappa_star={cfg.kappa_star}, "
                                        f"kappa_s={cfg.kappa_s}, gamma={cfg.gamma}, tol={cfg.tol}, max_iter={cfg.max_iter}, seed={cfg.seed}",
-                           "step": "star_field + critical_curves_ex + caustics + match_root_sets",
+                           "step": ("star_field + critical_curves_ex + caustics + match_root_sets" if args.separate_caustics
+                                    else "star_field + curves_and_caustics (fused) + match_root_sets"),
+                           "aberth_sum_precision": st.aberth_sum_precision,
                            "subchains": st.subchains, "predictor_order": st.predictor_order,
                            "l2": f"inputs larger than L2: each step writes {2 * num_phi * n_r * 16 / 1e9:.2f} GB of roots and caustics "
                                  f"and reads a {num_phi * n_r * 16 / 1e9:.2f} GB comparison set (L2 is 126 MB)",

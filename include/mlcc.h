@@ -67,8 +67,14 @@ typedef struct mlcc_options {
     int64_t phi_index_offset; /* row j has phase phi = 2 pi (j + phi_index_offset) / phi_index_total */
     int64_t phi_index_total;  /* 0 = num_phi (the half-open grid over [0, 2 pi))                     */
     int32_t min_lanes_per_root; /* lower bound on the threads that split one root's sums
-                                   (power of two <= 256); 0 = library default                        */
-    int32_t reserved;
+                                   (power of two <= 128); 0 = library default                        */
+    int32_t aberth_sum_precision; /* arithmetic of the Aberth sum A = sum_{r != k} 1/(z_k - z_r)
+                                   (Eq. 17).  A multiplies F in the denominator of the
+                                   update, so it steers the convergence rate only: the fixed point
+                                   F = 0 and the freeze test do not depend on it (R19).
+                                   0 or 32 = double-single FP32 (z = hi + lo, differences exact to
+                                   ~2^-23 |z_k - z_r|); 64 = FP64 differences with the 20-bit
+                                   reciprocal seed.  Star sums (F, F') are FP64 in both.            */
 } mlcc_options;
 
 /* Counters of one mlcc_critical_curves_ex call (host struct, filled on return). */
@@ -84,7 +90,7 @@ typedef struct mlcc_stats {
     int32_t unconverged_rows;  /* rows with out_unconverged > 0                                         */
     int32_t degenerate_roots;  /* NaN/Inf steps seen                                                    */
     float   solve_ms;          /* device time of the call's kernels, CUDA events on `stream`            */
-    float   reserved;
+    int32_t aberth_sum_precision; /* 32 or 64: the Aberth-sum arithmetic used                           */
 } mlcc_stats;
 
 int         mlcc_version(void);                 /* major*10000 + minor*100 + patch                       */
@@ -136,6 +142,20 @@ int mlcc_critical_curves_ex(const double *star_xy, const double *masses, int64_t
                             int32_t *out_iters, int32_t *out_unconverged,
                             mlcc_stats *out_stats, void *stream);
 
+/* a1-a7 fused: critical curves and their caustic points in one pass.  Same as
+ * mlcc_critical_curves_ex, and out_caustics [num_phi][2N][2] (device, written, may not alias
+ * out_roots) receives w(z) of Eq. 12 for every root.  The Aberth kernel carries
+ * Sm = sum_i m_i/(z - z_i) beside the star sums it needs anyway, and writes
+ * w(z - dz) from Sm(z - dz) = Sm + dz S2 + dz^2 S3 + O(dz^3 S4): exact to rounding for a frozen
+ * root (|dz| < tol).  A root still unfrozen at max_iter gets the caustic point of its last
+ * iterate to that order.  Errors: as mlcc_critical_curves_ex.                                   */
+int mlcc_curves_and_caustics(const double *star_xy, const double *masses, int64_t N,
+                             double kappa_s, double gamma, int64_t num_phi, double tol,
+                             int32_t max_iter, double *out_roots, double *out_caustics,
+                             const mlcc_options *opt, const double *init_roots,
+                             int32_t *out_iters, int32_t *out_unconverged,
+                             mlcc_stats *out_stats, void *stream);
+
 /* a7  Caustic mapping (Eq. 12 at :114): w_p = lens equation at points[p].
  *   points [P][2]: device, read.  out_caustics [P][2]: device, written (may not alias points).
  * Asynchronous on `stream` (no device status to read back).  P = 0 is a no-op.
@@ -166,8 +186,8 @@ int mlcc_plan_subchains(int64_t N, int64_t num_phi, int32_t num_subchains, int32
 
 /* Host-buffer variants (every pointer is a HOST pointer; the library allocates device memory,
  * copies in, runs the device path above on the default stream, copies out and frees).
- * mlcc_curves_and_caustics_host runs a0..a7 without bringing the roots back to the host in
- * between; out_caustics may be NULL (critical curves only).                                      */
+ * mlcc_curves_and_caustics_host runs the fused a1..a7 pass (mlcc_curves_and_caustics);
+ * out_caustics may be NULL (critical curves only).                                               */
 int mlcc_critical_curves_host(const double *star_xy, const double *masses, int64_t N,
                               double kappa_s, double gamma, int64_t num_phi, double tol,
                               int32_t max_iter, double *out_roots);

@@ -33,7 +33,7 @@ class mlcc_options(C.Structure):
     _fields_ = [("struct_size", C.c_int32), ("num_subchains", C.c_int32),
                 ("predictor_order", C.c_int32), ("max_iter_cold", C.c_int32),
                 ("phi_index_offset", C.c_int64), ("phi_index_total", C.c_int64),
-                ("min_lanes_per_root", C.c_int32), ("reserved", C.c_int32)]
+                ("min_lanes_per_root", C.c_int32), ("aberth_sum_precision", C.c_int32)]
 
 
 class mlcc_stats(C.Structure):
@@ -41,7 +41,7 @@ class mlcc_stats(C.Structure):
                 ("kernel_launches", C.c_int64), ("total_iterations", C.c_int32), ("steps", C.c_int32),
                 ("subchains", C.c_int32), ("predictor_order", C.c_int32),
                 ("unconverged_rows", C.c_int32), ("degenerate_roots", C.c_int32),
-                ("solve_ms", C.c_float), ("reserved", C.c_float)]
+                ("solve_ms", C.c_float), ("aberth_sum_precision", C.c_int32)]
 
 
 @dataclass
@@ -58,6 +58,7 @@ class Stats:
     degenerate_roots: int
     solve_ms: float
     status: int = 0
+    aberth_sum_precision: int = 0
 
 
 _lib = None
@@ -83,6 +84,9 @@ def lib() -> C.CDLL:
         L.mlcc_critical_curves_ex.argtypes = [vp, vp, i64, dbl, dbl, i64, dbl, i32, vp,
                                               C.POINTER(mlcc_options), vp, vp, vp,
                                               C.POINTER(mlcc_stats), vp]
+        L.mlcc_curves_and_caustics.argtypes = [vp, vp, i64, dbl, dbl, i64, dbl, i32, vp, vp,
+                                               C.POINTER(mlcc_options), vp, vp, vp,
+                                               C.POINTER(mlcc_stats), vp]
         L.mlcc_caustics.argtypes = [vp, vp, i64, dbl, dbl, vp, i64, vp, vp]
         L.mlcc_match_root_sets.argtypes = [vp, vp, i64, i64, dbl, vp, vp, vp]
         L.mlcc_plan_subchains.argtypes = [i64, i64, i32, i32, vp, vp, vp]
@@ -124,7 +128,7 @@ def last_error() -> str:
 
 
 def options(num_subchains=0, predictor_order=-1, max_iter_cold=0, phi_index_offset=0,
-            phi_index_total=0, min_lanes_per_root=0) -> mlcc_options:
+            phi_index_total=0, min_lanes_per_root=0, aberth_sum_precision=0) -> mlcc_options:
     o = mlcc_options()
     lib().mlcc_options_default(C.byref(o))
     o.num_subchains = num_subchains
@@ -133,6 +137,7 @@ def options(num_subchains=0, predictor_order=-1, max_iter_cold=0, phi_index_offs
     o.phi_index_offset = phi_index_offset
     o.phi_index_total = phi_index_total
     o.min_lanes_per_root = min_lanes_per_root
+    o.aberth_sum_precision = aberth_sum_precision
     return o
 
 
@@ -166,6 +171,12 @@ def critical_curves(star_xy, masses, kappa_s, gamma, num_phi, tol=1e-12, max_ite
     return out
 
 
+def _stats(st: mlcc_stats, rc: int) -> Stats:
+    return Stats(st.root_iterations, st.star_pairs, st.root_pairs, st.kernel_launches,
+                 st.total_iterations, st.steps, st.subchains, st.predictor_order,
+                 st.unconverged_rows, st.degenerate_roots, st.solve_ms, rc, st.aberth_sum_precision)
+
+
 def critical_curves_ex(star_xy, masses, kappa_s, gamma, num_phi, tol=1e-12, max_iter=50, opt=None,
                        init_roots=None, out_roots=None, want_diagnostics=True, strict=True):
     """mlcc_critical_curves_ex -> (roots [num_phi,2N,2], iters [num_phi] i32, unconverged [num_phi] i32, Stats).
@@ -188,10 +199,32 @@ def critical_curves_ex(star_xy, masses, kappa_s, gamma, num_phi, tol=1e-12, max_
         _dev(iters, torch.int32, "iters"), _dev(unconv, torch.int32, "unconverged"), C.byref(st), _stream())
     if rc != MLCC_OK and (strict or rc not in (MLCC_ERR_NOT_CONVERGED, MLCC_ERR_DEGENERATE)):
         _raise(rc)
-    stats = Stats(st.root_iterations, st.star_pairs, st.root_pairs, st.kernel_launches,
-                  st.total_iterations, st.steps, st.subchains, st.predictor_order,
-                  st.unconverged_rows, st.degenerate_roots, st.solve_ms, rc)
-    return out_roots, iters, unconv, stats
+    return out_roots, iters, unconv, _stats(st, rc)
+
+
+def curves_and_caustics(star_xy, masses, kappa_s, gamma, num_phi, tol=1e-12, max_iter=50, opt=None,
+                        init_roots=None, out_roots=None, out_caustics=None, want_diagnostics=True, strict=True):
+    """mlcc_curves_and_caustics (fused a1-a7) -> (roots, caustics [num_phi,2N,2], iters, unconverged, Stats)."""
+    N = masses.shape[0]
+    dev = masses.device
+    if out_roots is None:
+        out_roots = torch.empty((num_phi, 2 * N, 2), dtype=torch.float64, device=dev)
+    if out_caustics is None:
+        out_caustics = torch.empty((num_phi, 2 * N, 2), dtype=torch.float64, device=dev)
+    iters = unconv = None
+    if want_diagnostics:
+        iters = torch.zeros((num_phi,), dtype=torch.int32, device=dev)
+        unconv = torch.zeros((num_phi,), dtype=torch.int32, device=dev)
+    st = mlcc_stats()
+    rc = lib().mlcc_curves_and_caustics(
+        _dev(star_xy, name="star_xy"), _dev(masses, name="masses"), N, float(kappa_s), float(gamma),
+        int(num_phi), float(tol), int(max_iter), _dev(out_roots, name="out_roots"),
+        _dev(out_caustics, name="out_caustics"),
+        C.byref(opt) if opt is not None else None, _dev(init_roots, name="init_roots"),
+        _dev(iters, torch.int32, "iters"), _dev(unconv, torch.int32, "unconverged"), C.byref(st), _stream())
+    if rc != MLCC_OK and (strict or rc not in (MLCC_ERR_NOT_CONVERGED, MLCC_ERR_DEGENERATE)):
+        _raise(rc)
+    return out_roots, out_caustics, iters, unconv, _stats(st, rc)
 
 
 def caustics(star_xy, masses, kappa_s, gamma, points, out=None):
@@ -257,10 +290,7 @@ def curves_and_caustics_host(star_xy: np.ndarray, masses: np.ndarray, kappa_s, g
                                              hptr(out_caustics) if want_caustics else None, C.byref(st))
     if rc != MLCC_OK:
         _raise(rc)
-    stats = Stats(st.root_iterations, st.star_pairs, st.root_pairs, st.kernel_launches,
-                  st.total_iterations, st.steps, st.subchains, st.predictor_order,
-                  st.unconverged_rows, st.degenerate_roots, st.solve_ms, rc)
-    return out_roots, out_caustics, stats
+    return out_roots, out_caustics, _stats(st, rc)
 
 
 def critical_curves_host(star_xy: np.ndarray, masses: np.ndarray, kappa_s, gamma, num_phi, tol=1e-12, max_iter=50):

@@ -8,7 +8,7 @@
 //   Delta_k  = F / (F' + F (2 S1 - A)),  A = sum_{r != k} 1/(z_k - z_r),  z_k <- z_k - Delta_k,
 //   root k frozen once |Delta_k| < tol.
 //
-// Organisation:
+// Organisation (DESIGN.md "Driver" and "Kernels"):
 //   * The rows [0, num_phi) are cut into sub-chains; each sub-chain cold-starts its centre row from
 //     z_i +/- 1 and then grows towards both ends.  One "step"
 //     advances every growing direction ("slot") by one row; all slots of a step are iterated
@@ -16,11 +16,18 @@
 //   * A device-side state machine (DevState) decides what each launch does; the host only enqueues
 //     [seed, compute, apply, finalize] groups and polls one flag per chunk.  No host round trip
 //     sits inside the iteration loop.
-//   * compute: one CTA per tile of unfrozen roots of one slot.  Each root's sums are split over
-//     T threads (T = 1..256, chosen on the device from the number of unfrozen roots so that the
-//     machine stays full when few roots are left); stars and the slot's current roots stream
-//     through shared memory.  Jacobi: updates go to a separate buffer and are applied by `apply`,
-//     which also compacts the list of unfrozen roots.
+//   * compute: persistent CTAs of 128 threads pull tiles of unfrozen roots from an atomic counter.
+//     A root's sums are split over T lanes (T = 1..128, chosen on the device so that there are
+//     many more tiles than SMs).  Sources stream through shared memory in double-buffered stages
+//     of 256 stars + 512 roots, each stage filled by three TMA bulk copies (cp.async.bulk) that
+//     complete on an mbarrier, so no thread spends issue slots on loads.  One loop iteration
+//     evaluates one (root, star) pair in FP64 and two (root, root) pairs: the star sums carry F and
+//     must be FP64; the Aberth sum A only steers the convergence RATE (it multiplies F in the
+//     denominator) and is evaluated in double-single FP32 with packed f32x2 instructions, which
+//     read half the register-file bytes of the FP64 form (the register-file read ports, not the
+//     FP64 pipe, bound this kernel: DESIGN.md "Measured issue model").
+//   * Jacobi: updates go to a side buffer and are applied by `apply`, which also refreshes the
+//     per-slot source copy of the row and compacts the list of unfrozen roots.
 #include "mlcc_common.cuh"
 
 #include <math.h>
@@ -29,22 +36,18 @@
 namespace mlcc {
 namespace {
 
-constexpr int BLOCK = 256;        // threads per CTA of the compute kernel
-constexpr int TILE = 1024;        // sources staged in shared memory per tile
+constexpr int CTA = 128;          // threads per CTA of the compute kernel
+constexpr int S_TILE = 256;       // stars per stage; a stage also holds the 2*S_TILE roots paired with them
+constexpr int STAGE_BYTES = S_TILE * 16 + S_TILE * 8 + 2 * S_TILE * 16;
+constexpr int BLOCK = 256;        // threads per CTA of the small kernels
 constexpr int MAX_ORDER = 5;      // highest predictor order
 constexpr int MAX_SLOTS = 1024;   // most slots in one step (2 per sub-chain)
-constexpr double TINY = 1e-300;   // added to |d|^2: makes the self pair finite, invisible otherwise
-#ifndef MLCC_U_STAR
-#define MLCC_U_STAR 4
-#endif
-#ifndef MLCC_U_ROOT
-#define MLCC_U_ROOT 8
-#endif
-#ifndef MLCC_MIN_BLOCKS
-#define MLCC_MIN_BLOCKS 2
-#endif
-constexpr int U_STAR = MLCC_U_STAR;   // pairs in flight per thread in the star loop
-constexpr int U_ROOT = MLCC_U_ROOT;   // ... in the root loop (even)
+constexpr double TINY = 1e-300;   // added to |d|^2 (FP64 root pairs): makes the self pair finite
+constexpr float TINYF = 1e-30f;   // same for the FP32 root pairs
+constexpr double PAD_STAR = 1e150;  // padding star: mass 0 at (1e150, 1e150); its 1/d ~ 1e-151 is lost in S1
+constexpr float PAD_ROOT_F = 1e18f; // padding root of the FP32 source copy: its 1/d ~ 1e-18
+constexpr int MODE_F32 = 0;       // Aberth sum in double-single FP32 (default)
+constexpr int MODE_F64 = 1;       // Aberth sum in FP64 with the 20-bit reciprocal seed
 
 struct DevState {
     int step;             // current step: 0 = cold centre rows, s >= 1 = rows centre +/- s
@@ -53,12 +56,14 @@ struct DevState {
     int done;             // all steps finished
     int need_seed;        // the seed kernel must write starting values for this step
     int cur;              // which of the two active lists is current
-    int T;                // threads per root of the next compute launch
+    int T;                // lanes per root of the next compute launch
     int n_tiles;          // CTA tiles of the next compute launch
+    int next_tile;        // tile counter of the running compute launch (atomic)
     int total_active;     // unfrozen roots over all slots
     int total_iterations;
     int unconverged_rows;
     int degenerate;
+    int pad_;
     long long root_iterations;
     long long launches_used;  // compute launches that did work
 };
@@ -69,16 +74,19 @@ struct Params {
     const double *masses;     // [N]
     int N;
     int n_r;                  // 2N
+    int N_pad;                // N rounded up to a multiple of S_TILE
     double gamma;
+    double omk;               // 1 - kappa_s
     double tol2;              // tol^2
     int max_iter;
     int max_iter_cold;
     int order;                // predictor order
     int min_T;
-    int target_threads;       // threads the compute grid can keep resident
+    int tiles_target;         // the compute launch wants at least this many tiles
     const double2 *rot;       // [num_phi]  (1-kappa_s) e^{-i phi_j}
     const double2 *init_roots;  // [n_r] or null
     double2 *roots;           // [num_phi][n_r]
+    double2 *caustics;        // [num_phi][n_r] or null
     int *out_iters;           // [num_phi] or null
     int *out_unconverged;     // [num_phi] or null
     // plan
@@ -89,6 +97,12 @@ struct Params {
     int max_steps;            // largest distance from a centre to an end of its sub-chain
     // workspace
     DevState *state;
+    double2 *stars_pad;       // [N_pad]  stars, then padding stars
+    double *mass_pad;         // [N_pad]
+    float4 *src;              // [max_slots][2 N_pad] 16-byte source entries of the row each slot is solving:
+                              //   MODE_F32: entries 2q, 2q+1 = (xh_a, xh_b, yh_a, yh_b), (xl_a, xl_b, yl_a, yl_b)
+                              //             of roots a = 2q, b = 2q+1 (z = h + l, h = float(z), l = float(z - h))
+                              //   MODE_F64: entry r = root r as double2
     long long *slot_row;      // [MAX_SLOTS] row solved by the slot in this step
     int *slot_sub;            // [MAX_SLOTS] sub-chain of the slot
     int *slot_dir;            // [MAX_SLOTS] -1, +1 (0 = centre)
@@ -101,47 +115,180 @@ struct Params {
 };
 
 // ------------------------------------------------------------------------------------------------
-// pair bodies
+// small device helpers: packed FP32 arithmetic (FADD2 / FFMA2), mbarrier, TMA bulk copy
 // ------------------------------------------------------------------------------------------------
-
-// (root, star): accumulates S1 += 1/d, S2 += m/d^2, S3 += m/d^3 with d = z - z_i.
-// w = 1/d = conj(d)/|d|^2; dy is taken as (y_i - y) so that w = (dx, dy) * inv.
-__device__ __forceinline__ void pair_star(double zx, double zy, double2 s, double m,
-                                          double &s1x, double &s1y, double &s2x, double &s2y,
-                                          double &s3x, double &s3y)
+__device__ __forceinline__ float2 add2(float2 a, float2 b)
 {
-    double dx = zx - s.x;
-    double dy = s.y - zy;
-    double r2 = fma(dy, dy, fma(dx, dx, TINY));
-    double inv = rcp_full(r2);
-    double wx = dx * inv;
-    double wy = dy * inv;
-    s1x += wx;
-    s1y += wy;
-    double ux = m * wx;
-    double uy = m * wy;
-    double qx = fma(-uy, wy, ux * wx);   // q = m w^2
-    double qy = fma(ux, wy, uy * wx);
-    s2x += qx;
-    s2y += qy;
-    s3x = fma(qx, wx, s3x);               // S3 += q w
-    s3x = fma(-qy, wy, s3x);
-    s3y = fma(qx, wy, s3y);
-    s3y = fma(qy, wx, s3y);
+    float2 r;
+    asm("{.reg .b64 ra, rb, rr; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; add.rn.ftz.f32x2 rr, ra, rb; "
+        "mov.b64 {%0,%1}, rr;}" : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return r;
+}
+__device__ __forceinline__ float2 sub2(float2 a, float2 b)
+{
+    float2 r;
+    asm("{.reg .b64 ra, rb, rr; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; sub.rn.ftz.f32x2 rr, ra, rb; "
+        "mov.b64 {%0,%1}, rr;}" : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return r;
+}
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c)
+{
+    float2 r;
+    asm("{.reg .b64 ra, rb, rc, rr; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; mov.b64 rc, {%6,%7}; "
+        "fma.rn.ftz.f32x2 rr, ra, rb, rc; mov.b64 {%0,%1}, rr;}"
+        : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y), "f"(c.x), "f"(c.y));
+    return r;
+}
+__device__ __forceinline__ float rcp_f32(float x)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
 }
 
-// (root, root): A += 1/(z_k - z_r).  Only the convergence RATE depends on A (the fixed point of
-// the update is F = 0 whatever A is), so the 20-bit reciprocal seed is used as it is.  A root
-// paired with itself has d = 0 exactly: |d|^2 + TINY = 1e-300, the seed is finite, and the pair
-// contributes conj(d) * inv = 0.  For every other pair TINY is lost in the rounding of |d|^2.
-__device__ __forceinline__ void pair_root(double zx, double zy, double2 r, double &ax, double &ay)
+__device__ __forceinline__ unsigned smem_u32(const void *p)
 {
-    double dx = zx - r.x;
-    double dy = r.y - zy;
-    double r2 = fma(dy, dy, fma(dx, dx, TINY));
-    double inv = rcp_seed(r2);
+    return (unsigned)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity)
+{
+    unsigned ok;
+    do {
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!ok);
+}
+// TMA bulk copy global -> shared (bytes a multiple of 16, both addresses 16-byte aligned)
+__device__ __forceinline__ void tma_load(void *dst, const void *src, unsigned bytes, unsigned long long *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// double -> (h, l) with h = float(z), l = float(z - h): z = h + l to ~2^-48 relative
+__device__ __forceinline__ void split_ds(double v, float &h, float &l)
+{
+    h = __double2float_rn(v);
+    l = __double2float_rn(v - (double)h);
+}
+
+// writes root k of a slot's row into the slot's source copy
+template <int MODE>
+__device__ __forceinline__ void store_src(float4 *slot_src, int k, double2 z)
+{
+    if (MODE == MODE_F64) {
+        reinterpret_cast<double2 *>(slot_src)[k] = z;
+    } else {
+        float xh, xl, yh, yl;
+        split_ds(z.x, xh, xl);
+        split_ds(z.y, yh, yl);
+        float *f = reinterpret_cast<float *>(slot_src) + (size_t)(k >> 1) * 8 + (k & 1);
+        f[0] = xh; f[2] = yh; f[4] = xl; f[6] = yl;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// pair bodies
+// ------------------------------------------------------------------------------------------------
+struct StarAcc {
+    double s1x, s1y;   // S1
+    double s2x, s2h;   // Re S2, (Im S2)/2
+    double s3x, s3y;   // S3
+    double smx, smy;   // sum m/(z-z_i) (caustic map; only with CAUS)
+};
+
+// (root, star): with d = z - z_i, w = 1/d = conj(d)/|d|^2 = (wx, wy)  [dy is taken as y_i - y],
+//   S1 += w,  S2 += m w^2 = m (wx^2 - wy^2, 2 wx wy),  S3 += m w^3 = m (wx (wx^2 - 3 wy^2), wy (3 wx^2 - wy^2)).
+// 22 FP64 instructions + 1 MUFU; 18 of them name at most two distinct register sources.
+template <bool CAUS>
+__device__ __forceinline__ void pair_star(double zx, double zy, double2 s, double m, StarAcc &a)
+{
+    const double dx = zx - s.x;
+    const double dy = s.y - zy;
+    const double r2 = fma(dy, dy, dx * dx);
+    const double inv = rcp_full(r2);
+    const double wx = dx * inv;
+    const double wy = dy * inv;
+    a.s1x += wx;
+    a.s1y += wy;
+    const double ux = m * wx;
+    const double uy = m * wy;
+    if (CAUS) {
+        a.smx += ux;
+        a.smy += uy;
+    }
+    const double A = wx * wx;
+    const double B = wy * wy;
+    const double g = fma(-3.0, B, A);
+    const double h = fma(3.0, A, -B);
+    const double c = A - B;
+    a.s2x = fma(m, c, a.s2x);
+    a.s2h = fma(ux, wy, a.s2h);
+    a.s3x = fma(ux, g, a.s3x);
+    a.s3y = fma(uy, h, a.s3y);
+}
+
+// (root, root) in FP64: A += 1/(z_k - z_r) with the 20-bit reciprocal seed.  Only the convergence
+// RATE depends on A (the fixed point of the update is F = 0 whatever A is).  A root paired with
+// itself has d = 0 exactly: |d|^2 + TINY = 1e-300, the seed is finite, the pair contributes 0.
+__device__ __forceinline__ void pair_root_f64(double zx, double zy, double2 r, double &ax, double &ay)
+{
+    const double dx = zx - r.x;
+    const double dy = r.y - zy;
+    const double r2 = fma(dy, dy, fma(dx, dx, TINY));
+    const double inv = rcp_seed(r2);
     ax = fma(dx, inv, ax);
     ay = fma(dy, inv, ay);
+}
+
+// two (root, root) pairs in double-single FP32, packed: lanes .x / .y of every float2 are the two
+// source roots.  d = (zh - rh) + (zl - rl) is accurate to ~2^-23 |d| (the high parts cancel
+// exactly when the roots are close), so 1/d carries ~6 digits like the FP64 seed form.
+__device__ __forceinline__ void pair_root2_f32(float2 zxh, float2 zyh, float2 zxl, float2 zyl, float4 h, float4 l,
+                                               float2 &ax, float2 &ay)
+{
+    const float2 dx = add2(sub2(zxh, make_float2(h.x, h.y)), sub2(zxl, make_float2(l.x, l.y)));
+    const float2 dy = add2(sub2(make_float2(h.z, h.w), zyh), sub2(make_float2(l.z, l.w), zyl));
+    const float2 r2 = fma2(dy, dy, fma2(dx, dx, make_float2(TINYF, TINYF)));
+    const float2 inv = make_float2(rcp_f32(r2.x), rcp_f32(r2.y));
+    ax = fma2(dx, inv, ax);
+    ay = fma2(dy, inv, ay);
+}
+
+// ------------------------------------------------------------------------------------------------
+// prepare kernel: padded star arrays, padding entries of every slot's source copy
+// ------------------------------------------------------------------------------------------------
+template <int MODE>
+__global__ void k_prepare(Params p)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const long long t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    for (long long i = t0; i < p.N_pad; i += stride) {
+        const bool real = i < p.N;
+        p.stars_pad[i] = real ? p.stars[i] : make_double2(PAD_STAR, PAD_STAR);
+        p.mass_pad[i] = real ? p.masses[i] : 0.0;
+    }
+    const int n_src = 2 * p.N_pad;
+    const int n_padroots = n_src - p.n_r;
+    for (long long idx = t0; idx < (long long)p.max_slots * n_padroots; idx += stride) {
+        const int slot = (int)(idx / n_padroots);
+        const int k = p.n_r + (int)(idx - (long long)slot * n_padroots);
+        float4 *slot_src = p.src + (size_t)slot * n_src;
+        if (MODE == MODE_F64) {
+            reinterpret_cast<double2 *>(slot_src)[k] = make_double2(PAD_STAR, PAD_STAR);
+        } else {
+            float *f = reinterpret_cast<float *>(slot_src) + (size_t)(k >> 1) * 8 + (k & 1);
+            f[0] = PAD_ROOT_F; f[2] = PAD_ROOT_F; f[4] = 0.f; f[6] = 0.f;
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -151,6 +298,7 @@ __constant__ double c_coef[MAX_ORDER + 1][MAX_ORDER + 1] = {
     {1, 0, 0, 0, 0, 0},          {2, -1, 0, 0, 0, 0},          {3, -3, 1, 0, 0, 0},
     {4, -6, 4, -1, 0, 0},        {5, -10, 10, -5, 1, 0},       {6, -15, 20, -15, 6, -1}};
 
+template <int MODE>
 __global__ void k_seed(Params p)
 {
     const DevState st = *p.state;
@@ -187,6 +335,7 @@ __global__ void k_seed(Params p)
             z = make_double2(zx, zy);
         }
         p.roots[row * p.n_r + k] = z;
+        store_src<MODE>(p.src + (size_t)slot * 2 * p.N_pad, k, z);
         p.list[((long long)st.cur * p.max_slots + slot) * p.n_r + k] = k;
     }
 }
@@ -194,36 +343,65 @@ __global__ void k_seed(Params p)
 // ------------------------------------------------------------------------------------------------
 // compute kernel
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(BLOCK, MLCC_MIN_BLOCKS) k_compute(Params p)
+struct __align__(128) Stage {
+    double2 sxy[S_TILE];     // star positions
+    double sm[S_TILE];       // star masses
+    float4 rp[2 * S_TILE];   // the slot's source entries 2 j0 .. 2 j0 + 2 S_TILE
+};
+
+template <int MODE, bool CAUS>
+__global__ void __launch_bounds__(CTA, 4) k_compute(Params p)
 {
-    __shared__ double2 s_xy[TILE];
-    __shared__ double s_m[TILE];
-    __shared__ double s_red[BLOCK / 32][6];
+    __shared__ Stage s_stage[2];
+    __shared__ __align__(8) unsigned long long s_full[2];
+    __shared__ double s_red[CTA / 32][8];
+    __shared__ int s_tile;
 
     const DevState st = *p.state;
     if (st.done) return;
-    const int T = st.T;                 // threads per root (power of two, 1..256)
+    const int T = st.T;                 // lanes per root (power of two, 1..CTA)
     const int TL = T < 32 ? T : 32;     // of which inside one warp
     const int W = T / TL;               // warps per root
-    const int roots_per_tile = BLOCK / T;
+    const int roots_per_tile = CTA / T;
     const int tid = threadIdx.x;
     const int lane = tid & 31;
     const int warp = tid >> 5;
-    // position of this thread's root inside the tile, and which share of the sources it sums
-    const int local_root = (warp / W) * (32 / TL) + lane / TL;
-    const int sub = (warp % W) * TL + (lane % TL);
-    const int* n_active = p.n_active + st.cur * MAX_SLOTS;
+    const int local_root = tid / T;     // position of this thread's root inside the tile
+    const int sub = tid % T;            // which share of the sources it sums
+    const int n_it = S_TILE / T;        // loop iterations per stage (>= 2)
+    const int n_stage = p.N_pad / S_TILE;
+    const int n_src = 2 * p.N_pad;
+    const int *n_active = p.n_active + st.cur * MAX_SLOTS;
 
-    for (int tile = blockIdx.x; tile < st.n_tiles; tile += gridDim.x) {
+    if (tid == 0) {
+        mbar_init(&s_full[0], 1);
+        mbar_init(&s_full[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    unsigned g = 0;   // stages consumed by this CTA so far: buffer g & 1, parity (g >> 1) & 1
+
+    for (;;) {
+        if (tid == 0) s_tile = atomicAdd(&p.state->next_tile, 1);
+        __syncthreads();
+        const int tile = s_tile;
+        if (tile >= st.n_tiles) break;
         // slot of this tile: last slot with tile_start <= tile
         int lo = 0, hi = st.n_slots;
         while (hi - lo > 1) {
-            int mid = (lo + hi) >> 1;
+            const int mid = (lo + hi) >> 1;
             if (p.tile_start[mid] <= tile) lo = mid; else hi = mid;
         }
         const int slot = lo;
         const long long row = p.slot_row[slot];
-        const double2 *zrow = p.roots + row * p.n_r;
+        const float4 *slot_src = p.src + (size_t)slot * n_src;
+        if (tid == 0) {   // first stage of this tile
+            const unsigned b = g & 1u;
+            mbar_expect_tx(&s_full[b], STAGE_BYTES);
+            tma_load(s_stage[b].sxy, p.stars_pad, S_TILE * 16, &s_full[b]);
+            tma_load(s_stage[b].sm, p.mass_pad, S_TILE * 8, &s_full[b]);
+            tma_load(s_stage[b].rp, slot_src, 2 * S_TILE * 16, &s_full[b]);
+        }
         const int *list = p.list + ((long long)st.cur * p.max_slots + slot) * p.n_r;
         const int pos = (tile - p.tile_start[slot]) * roots_per_tile + local_root;
         const bool valid = pos < n_active[slot];
@@ -231,100 +409,126 @@ __global__ void __launch_bounds__(BLOCK, MLCC_MIN_BLOCKS) k_compute(Params p)
         double zx = 0.0, zy = 0.0;
         if (valid) {
             k = list[pos];
-            const double2 z = zrow[k];
+            const double2 z = p.roots[row * p.n_r + k];
             zx = z.x;
             zy = z.y;
         }
-        double s1x = 0, s1y = 0, s2x = 0, s2y = 0, s3x = 0, s3y = 0, ax = 0, ay = 0, bx = 0, by = 0;
+        float zxh, zxl, zyh, zyl;
+        split_ds(zx, zxh, zxl);
+        split_ds(zy, zyh, zyl);
+        const float2 zxh2 = make_float2(zxh, zxh), zyh2 = make_float2(zyh, zyh);
+        const float2 zxl2 = make_float2(zxl, zxl), zyl2 = make_float2(zyl, zyl);
+        StarAcc acc = {0, 0, 0, 0, 0, 0, 0, 0};
+        double ax = 0, ay = 0, bx = 0, by = 0;                     // MODE_F64: two chains
+        float2 fx = make_float2(0.f, 0.f), fy = make_float2(0.f, 0.f);   // MODE_F32: packed lanes
 
-        // ---- stars ----
-        for (int base = 0; base < p.N; base += TILE) {
-            const int cnt = min(TILE, p.N - base);
-            __syncthreads();
-            for (int i = tid; i < cnt; i += BLOCK) {
-                s_xy[i] = p.stars[base + i];
-                s_m[i] = p.masses[base + i];
+        for (int t = 0; t < n_stage; ++t, ++g) {
+            const unsigned b = g & 1u;
+            if (tid == 0 && t + 1 < n_stage) {   // prefetch: buffer b^1 was last read in stage g-1, closed by a barrier
+                const unsigned nb = b ^ 1u;
+                mbar_expect_tx(&s_full[nb], STAGE_BYTES);
+                tma_load(s_stage[nb].sxy, p.stars_pad + (size_t)(t + 1) * S_TILE, S_TILE * 16, &s_full[nb]);
+                tma_load(s_stage[nb].sm, p.mass_pad + (size_t)(t + 1) * S_TILE, S_TILE * 8, &s_full[nb]);
+                tma_load(s_stage[nb].rp, slot_src + (size_t)(t + 1) * 2 * S_TILE, 2 * S_TILE * 16, &s_full[nb]);
             }
-            __syncthreads();
+            mbar_wait(&s_full[b], (g >> 1) & 1u);
             if (valid) {
-                // blocks of U_STAR independent pairs with no exit in between, so that their
-                // dependent chains (|d|^2 -> reciprocal -> powers) interleave; then the ragged tail
-                int j = sub;
-                for (; j + (U_STAR - 1) * T < cnt; j += U_STAR * T) {
-                    double2 s[U_STAR];
-                    double m[U_STAR];
+                const Stage &sg = s_stage[b];
+                // blocks of independent (1 star + 2 roots) bodies with no exit in between, so that
+                // their dependent chains (|d|^2 -> reciprocal -> powers) interleave
+                if (n_it >= 4) {
+                    for (int i = 0; i < n_it; i += 4) {
 #pragma unroll
-                    for (int u = 0; u < U_STAR; ++u) { s[u] = s_xy[j + u * T]; m[u] = s_m[j + u * T]; }
+                        for (int u = 0; u < 4; ++u) {
+                            const int j = sub + (i + u) * T;
+                            pair_star<CAUS>(zx, zy, sg.sxy[j], sg.sm[j], acc);
+                            if (MODE == MODE_F64) {
+                                const double2 *r = reinterpret_cast<const double2 *>(sg.rp);
+                                pair_root_f64(zx, zy, r[2 * j], ax, ay);
+                                pair_root_f64(zx, zy, r[2 * j + 1], bx, by);
+                            } else {
+                                pair_root2_f32(zxh2, zyh2, zxl2, zyl2, sg.rp[2 * j], sg.rp[2 * j + 1], fx, fy);
+                            }
+                        }
+                    }
+                } else {
 #pragma unroll
-                    for (int u = 0; u < U_STAR; ++u)
-                        pair_star(zx, zy, s[u], m[u], s1x, s1y, s2x, s2y, s3x, s3y);
-                }
-                for (; j < cnt; j += T)
-                    pair_star(zx, zy, s_xy[j], s_m[j], s1x, s1y, s2x, s2y, s3x, s3y);
-            }
-        }
-        // ---- the other roots of this row (frozen ones included) ----
-        for (int base = 0; base < p.n_r; base += TILE) {
-            const int cnt = min(TILE, p.n_r - base);
-            __syncthreads();
-            for (int i = tid; i < cnt; i += BLOCK) s_xy[i] = zrow[base + i];
-            __syncthreads();
-            if (valid) {
-                int j = sub;
-                for (; j + (U_ROOT - 1) * T < cnt; j += U_ROOT * T) {
-                    double2 r[U_ROOT];
-#pragma unroll
-                    for (int u = 0; u < U_ROOT; ++u) r[u] = s_xy[j + u * T];
-#pragma unroll
-                    for (int u = 0; u < U_ROOT; u += 2) {   // two accumulator chains
-                        pair_root(zx, zy, r[u], ax, ay);
-                        pair_root(zx, zy, r[u + 1], bx, by);
+                    for (int u = 0; u < 2; ++u) {
+                        const int j = sub + u * T;
+                        pair_star<CAUS>(zx, zy, sg.sxy[j], sg.sm[j], acc);
+                        if (MODE == MODE_F64) {
+                            const double2 *r = reinterpret_cast<const double2 *>(sg.rp);
+                            pair_root_f64(zx, zy, r[2 * j], ax, ay);
+                            pair_root_f64(zx, zy, r[2 * j + 1], bx, by);
+                        } else {
+                            pair_root2_f32(zxh2, zyh2, zxl2, zyl2, sg.rp[2 * j], sg.rp[2 * j + 1], fx, fy);
+                        }
                     }
                 }
-                for (; j < cnt; j += T) pair_root(zx, zy, s_xy[j], ax, ay);
             }
+            __syncthreads();   // everyone is done with buffer b before it is refilled
         }
         // ---- reduce the T partial sums ----
-        double tx = 2.0 * s1x - (ax + bx);   // 2 S1 - A
-        double ty = 2.0 * s1y - (ay + by);
+        if (MODE == MODE_F32) {
+            ax = (double)fx.x + (double)fx.y;
+            ay = (double)fy.x + (double)fy.y;
+        } else {
+            ax += bx;
+            ay += by;
+        }
+        double v[8];
+        v[0] = acc.s2x; v[1] = acc.s2h; v[2] = acc.s3x; v[3] = acc.s3y;
+        v[4] = 2.0 * acc.s1x - ax;   // 2 S1 - A
+        v[5] = 2.0 * acc.s1y - ay;
+        v[6] = acc.smx; v[7] = acc.smy;
+        constexpr int NV = CAUS ? 8 : 6;
         for (int o = TL >> 1; o > 0; o >>= 1) {
-            s2x += __shfl_xor_sync(0xffffffffu, s2x, o);
-            s2y += __shfl_xor_sync(0xffffffffu, s2y, o);
-            s3x += __shfl_xor_sync(0xffffffffu, s3x, o);
-            s3y += __shfl_xor_sync(0xffffffffu, s3y, o);
-            tx += __shfl_xor_sync(0xffffffffu, tx, o);
-            ty += __shfl_xor_sync(0xffffffffu, ty, o);
+#pragma unroll
+            for (int q = 0; q < NV; ++q) v[q] += __shfl_xor_sync(0xffffffffu, v[q], o);
         }
         if (W > 1) {
-            __syncthreads();
             if (lane == 0) {
-                s_red[warp][0] = s2x; s_red[warp][1] = s2y; s_red[warp][2] = s3x;
-                s_red[warp][3] = s3y; s_red[warp][4] = tx;  s_red[warp][5] = ty;
+#pragma unroll
+                for (int q = 0; q < NV; ++q) s_red[warp][q] = v[q];
             }
             __syncthreads();
-            if (warp % W == 0 && lane == 0) {
+            if (sub == 0) {
                 for (int w2 = 1; w2 < W; ++w2) {
-                    s2x += s_red[warp + w2][0]; s2y += s_red[warp + w2][1];
-                    s3x += s_red[warp + w2][2]; s3y += s_red[warp + w2][3];
-                    tx += s_red[warp + w2][4];  ty += s_red[warp + w2][5];
+#pragma unroll
+                    for (int q = 0; q < NV; ++q) v[q] += s_red[warp + w2][q];
                 }
             }
         }
         // ---- Aberth step ----
         if (valid && sub == 0) {
             const double2 rot = p.rot[row];
-            const double fx = p.gamma + s2x - rot.x;   // F
-            const double fy = s2y - rot.y;
+            const double s2x = v[0], s2y = 2.0 * v[1], s3x = v[2], s3y = v[3], tx = v[4], ty = v[5];
+            const double fx_ = p.gamma + s2x - rot.x;   // F
+            const double fy_ = s2y - rot.y;
             const double gx = -2.0 * s3x;               // F'
             const double gy = -2.0 * s3y;
-            const double dnx = gx + (fx * tx - fy * ty);  // F' + F (2 S1 - A)
-            const double dny = gy + (fx * ty + fy * tx);
+            const double dnx = gx + (fx_ * tx - fy_ * ty);  // F' + F (2 S1 - A)
+            const double dny = gy + (fx_ * ty + fy_ * tx);
             const double dn2 = dnx * dnx + dny * dny;
             double2 d;
-            d.x = (fx * dnx + fy * dny) / dn2;          // F / den
-            d.y = (fy * dnx - fx * dny) / dn2;
+            d.x = (fx_ * dnx + fy_ * dny) / dn2;          // F / den
+            d.y = (fy_ * dnx - fx_ * dny) / dn2;
             p.delta[(long long)slot * p.n_r + pos] = d;
+            if (CAUS) {
+                // caustic point of z' = z - Delta (Eq. 12) from the sums at z:
+                // Sm(z') = Sm + Delta S2 + Delta^2 S3 + O(Delta^3 S4), Sm = sum m_i/(z - z_i);
+                // exact to rounding once the root freezes (|Delta| < tol).  Rewritten every iteration.
+                const double d2x = d.x * d.x - d.y * d.y, d2y = 2.0 * d.x * d.y;
+                const double mx = v[6] + (d.x * s2x - d.y * s2y) + (d2x * s3x - d2y * s3y);
+                const double my = v[7] + (d.x * s2y + d.y * s2x) + (d2x * s3y + d2y * s3x);
+                const double nx = zx - d.x, ny = zy - d.y;
+                double2 c;
+                c.x = fma(p.omk + p.gamma, nx, -mx);   // (1-kappa_s) x + gamma x - Re Sm
+                c.y = fma(p.omk - p.gamma, ny, my);    // (1-kappa_s) y - gamma y + Im Sm  (conj)
+                p.caustics[row * p.n_r + k] = c;
+            }
         }
+        __syncthreads();   // s_tile and s_red are rewritten by the next tile
     }
 }
 
@@ -332,6 +536,7 @@ __global__ void __launch_bounds__(BLOCK, MLCC_MIN_BLOCKS) k_compute(Params p)
 // apply kernel: z_k -= Delta_k, freeze converged roots, compact the list of unfrozen roots
 // grid: (ceil(n_r / BLOCK), max_slots)
 // ------------------------------------------------------------------------------------------------
+template <int MODE>
 __global__ void k_apply(Params p)
 {
     const DevState st = *p.state;
@@ -355,6 +560,7 @@ __global__ void k_apply(Params p)
             z.x -= d.x;
             z.y -= d.y;
             *zp = z;
+            store_src<MODE>(p.src + (size_t)slot * 2 * p.N_pad, k, z);
             keep = !(d2 < p.tol2);
         } else {                                // NaN / Inf: freeze where it is, report
             atomicAdd(&p.state->degenerate, 1);
@@ -369,12 +575,15 @@ __global__ void k_apply(Params p)
 }
 
 // ------------------------------------------------------------------------------------------------
-// finalize kernel (one block): advances the state machine
+// finalize kernel (one thread): advances the state machine
 // ------------------------------------------------------------------------------------------------
+// lanes per root: the smallest power of two that cuts the unfrozen roots into at least
+// tiles_target tiles (many more tiles than SMs: the atomic tile counter then balances the SMs to
+// within one tile), so a launch with few unfrozen roots still uses the whole machine
 __device__ int pick_T(const Params &p, int total_active)
 {
     int T = 1;
-    while (T < 256 && (long long)total_active * T * 2 <= p.target_threads) T <<= 1;
+    while (T < CTA && ((long long)total_active * T + CTA - 1) / CTA < p.tiles_target) T <<= 1;
     if (T < p.min_T) T = p.min_T;
     return T;
 }
@@ -387,7 +596,7 @@ __device__ void build_tiles(const Params &p, DevState &st)
     for (int s = 0; s < st.n_slots; ++s) total += n_active[s];
     st.total_active = total;
     st.T = pick_T(p, total);
-    const int rpt = BLOCK / st.T;
+    const int rpt = CTA / st.T;
     int t = 0;
     for (int s = 0; s < st.n_slots; ++s) {
         p.tile_start[s] = t;
@@ -395,6 +604,7 @@ __device__ void build_tiles(const Params &p, DevState &st)
     }
     p.tile_start[st.n_slots] = t;
     st.n_tiles = t;
+    st.next_tile = 0;
 }
 
 // one thread: slots of step st.step
@@ -437,7 +647,7 @@ __global__ void k_check_stars(const double2 *__restrict__ stars, const double *_
     if (i < N) {
         me = stars[i];
         const double m = masses[i];
-        if (!(fabs(me.x) <= 1e300) || !(fabs(me.y) <= 1e300) || !(fabs(m) <= 1e300)) atomicAdd(&flags[0], 1);
+        if (!(fabs(me.x) <= 1e100) || !(fabs(me.y) <= 1e100) || !(fabs(m) <= 1e100)) atomicAdd(&flags[0], 1);
     }
     int same = 0;
     for (int base = 0; base < N; base += BLOCK) {
@@ -457,8 +667,8 @@ __global__ void k_init(Params p)
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     DevState st;
     st.step = 0; st.iter = 0; st.n_slots = 0; st.done = 0; st.need_seed = 1; st.cur = 0;
-    st.T = 1; st.n_tiles = 0; st.total_active = 0; st.total_iterations = 0;
-    st.unconverged_rows = 0; st.degenerate = 0; st.root_iterations = 0; st.launches_used = 0;
+    st.T = 1; st.n_tiles = 0; st.next_tile = 0; st.total_active = 0; st.total_iterations = 0;
+    st.unconverged_rows = 0; st.degenerate = 0; st.pad_ = 0; st.root_iterations = 0; st.launches_used = 0;
     build_slots(p, st);
     build_tiles(p, st);
     *p.state = st;
@@ -502,6 +712,27 @@ __global__ void k_finalize(Params p)
     *p.state = st;
 }
 
+// the kernels of one Aberth-sum mode / caustic fusion choice
+struct KernelSet {
+    void (*prepare)(Params);
+    void (*seed)(Params);
+    void (*compute)(Params);
+    void (*apply)(Params);
+};
+
+KernelSet kernel_set(int mode, bool caus)
+{
+    KernelSet k;
+    if (mode == MODE_F64) {
+        k.prepare = k_prepare<MODE_F64>; k.seed = k_seed<MODE_F64>; k.apply = k_apply<MODE_F64>;
+        k.compute = caus ? k_compute<MODE_F64, true> : k_compute<MODE_F64, false>;
+    } else {
+        k.prepare = k_prepare<MODE_F32>; k.seed = k_seed<MODE_F32>; k.apply = k_apply<MODE_F32>;
+        k.compute = caus ? k_compute<MODE_F32, true> : k_compute<MODE_F32, false>;
+    }
+    return k;
+}
+
 }  // namespace
 
 // ------------------------------------------------------------------------------------------------
@@ -535,16 +766,17 @@ int plan_subchains_host(int64_t N, int64_t num_phi, int32_t num_subchains, int32
 
 int critical_curves_impl(const double *star_xy, const double *masses, int64_t N, double kappa_s,
                          double gamma, int64_t num_phi, double tol, int32_t max_iter,
-                         double *out_roots, const mlcc_options *opt_in, const double *init_roots,
-                         int32_t *out_iters, int32_t *out_unconverged, mlcc_stats *out_stats,
-                         cudaStream_t stream)
+                         double *out_roots, double *out_caustics, const mlcc_options *opt_in,
+                         const double *init_roots, int32_t *out_iters, int32_t *out_unconverged,
+                         mlcc_stats *out_stats, cudaStream_t stream)
 {
     if (!star_xy || !masses || !out_roots) return invalid("null pointer");
-    if (N < 1 || N > (1 << 29)) return invalid("N out of range");
+    if (N < 1 || N > (1 << 28)) return invalid("N out of range");
     if (num_phi < 1) return invalid("num_phi < 1");
     if (!(tol > 0.0) || !isfinite(tol)) return invalid("tol must be positive and finite");
     if (max_iter < 1) return invalid("max_iter < 1");
     if (!isfinite(kappa_s) || !isfinite(gamma)) return invalid("kappa_s / gamma not finite");
+    if (out_caustics == out_roots) return invalid("out_caustics aliases out_roots");
     mlcc_options opt;
     mlcc_options_default(&opt);
     if (opt_in) {
@@ -557,8 +789,11 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     int order = opt.predictor_order < 0 ? 3 : opt.predictor_order;
     if (order > MAX_ORDER) return invalid("predictor_order > 5");
     int min_T = opt.min_lanes_per_root <= 0 ? 1 : opt.min_lanes_per_root;
-    if (min_T > 256 || (min_T & (min_T - 1))) return invalid("min_lanes_per_root must be a power of two <= 256");
+    if (min_T > CTA || (min_T & (min_T - 1))) return invalid("min_lanes_per_root must be a power of two <= 128");
     if (opt.num_subchains < 0 || opt.max_iter_cold < 0) return invalid("negative option");
+    if (opt.aberth_sum_precision != 0 && opt.aberth_sum_precision != 32 && opt.aberth_sum_precision != 64)
+        return invalid("aberth_sum_precision must be 0, 32 or 64");
+    const int mode = opt.aberth_sum_precision == 64 ? MODE_F64 : MODE_F32;
 
     // phase table (1-kappa_s) e^{-i phi_j}; c(phi_j) = 0 on a row is rejected (degree drop)
     std::vector<double2> rot((size_t)num_phi);
@@ -587,6 +822,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     }
     const int max_slots = 2 * n_sub > 1 ? 2 * n_sub : 1;
     const int n_r = (int)(2 * N);
+    const int N_pad = (int)((N + S_TILE - 1) / S_TILE) * S_TILE;
 
     Workspace ws(stream);
     Params p{};
@@ -596,6 +832,9 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     if ((e = ws.alloc(&d_rot, (size_t)num_phi)) != cudaSuccess ||
         (e = ws.alloc(&d_plan, (size_t)3 * n_sub)) != cudaSuccess ||
         (e = ws.alloc(&p.state, 1)) != cudaSuccess ||
+        (e = ws.alloc(&p.stars_pad, (size_t)N_pad)) != cudaSuccess ||
+        (e = ws.alloc(&p.mass_pad, (size_t)N_pad)) != cudaSuccess ||
+        (e = ws.alloc(&p.src, (size_t)max_slots * 2 * N_pad)) != cudaSuccess ||
         (e = ws.alloc(&p.slot_row, MAX_SLOTS)) != cudaSuccess ||
         (e = ws.alloc(&p.slot_sub, MAX_SLOTS)) != cudaSuccess ||
         (e = ws.alloc(&p.slot_dir, MAX_SLOTS)) != cudaSuccess ||
@@ -630,15 +869,16 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
         MLCC_CUDA(cudaMemcpyAsync(h_flags, d_flags, 2 * sizeof(int), cudaMemcpyDeviceToHost, stream));
         MLCC_CUDA(cudaStreamSynchronize(stream));
         MLCC_CUDA(cudaGetLastError());
-        if (h_flags[0]) return invalid("non-finite star position or mass");
+        if (h_flags[0]) return invalid("non-finite (or > 1e100) star position or mass");
         if (h_flags[1]) {
             set_last_error("coincident stars: P(z) loses roots (merge them into one star of the summed mass)");
             return MLCC_ERR_DEGENERATE;
         }
     }
 
+    const KernelSet ks = kernel_set(mode, out_caustics != nullptr);
     int blocks_per_sm = 0;
-    MLCC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, k_compute, BLOCK, 0));
+    MLCC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, ks.compute, CTA, 0));
     if (blocks_per_sm < 1) blocks_per_sm = 1;
     const int sms = device_sm_count();
     const int grid_compute = sms * blocks_per_sm;
@@ -647,16 +887,19 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     p.masses = masses;
     p.N = (int)N;
     p.n_r = n_r;
+    p.N_pad = N_pad;
     p.gamma = gamma;
+    p.omk = 1.0 - kappa_s;
     p.tol2 = tol * tol;
     p.max_iter = max_iter;
     p.max_iter_cold = opt.max_iter_cold > 0 ? opt.max_iter_cold : max_iter;
     p.order = order;
     p.min_T = min_T;
-    p.target_threads = grid_compute * BLOCK;
+    p.tiles_target = 12 * sms;
     p.rot = d_rot;
     p.init_roots = reinterpret_cast<const double2 *>(init_roots);
     p.roots = reinterpret_cast<double2 *>(out_roots);
+    p.caustics = reinterpret_cast<double2 *>(out_caustics);
     p.out_iters = out_iters;
     p.out_unconverged = out_unconverged;
     p.n_sub = n_sub;
@@ -676,10 +919,11 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     h_state[0].done = h_state[1].done = 0;
 
     MLCC_CUDA(cudaEventRecord(ev0, stream));
-    k_init<<<1, 32, 0, stream>>>(p);
     const int grid_seed = sms * 4;
+    ks.prepare<<<grid_seed, BLOCK, 0, stream>>>(p);
+    k_init<<<1, 32, 0, stream>>>(p);
     const dim3 grid_apply((unsigned)((n_r + BLOCK - 1) / BLOCK), (unsigned)max_slots);
-    int64_t launches = 1;
+    int64_t launches = 3;   // check, prepare, init
     // Upper bound on iteration groups, so that a device-side fault cannot spin the host forever.
     const long long max_groups = (long long)(max_steps + 1) * (long long)(p.max_iter > p.max_iter_cold ? p.max_iter : p.max_iter_cold) + 8;
     const int chunk = 16;
@@ -689,9 +933,9 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     int rc = MLCC_OK;
     while (!finished && groups < max_groups + 2 * chunk) {
         for (int g = 0; g < chunk; ++g) {
-            k_seed<<<grid_seed, BLOCK, 0, stream>>>(p);
-            k_compute<<<grid_compute, BLOCK, 0, stream>>>(p);
-            k_apply<<<grid_apply, BLOCK, 0, stream>>>(p);
+            ks.seed<<<grid_seed, BLOCK, 0, stream>>>(p);
+            ks.compute<<<grid_compute, CTA, 0, stream>>>(p);
+            ks.apply<<<grid_apply, BLOCK, 0, stream>>>(p);
             k_finalize<<<1, 32, 0, stream>>>(p);
         }
         launches += 4 * chunk;
@@ -737,7 +981,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
         out_stats->unconverged_rows = fin.unconverged_rows;
         out_stats->degenerate_roots = fin.degenerate;
         out_stats->solve_ms = ms;
-        out_stats->reserved = 0.f;
+        out_stats->aberth_sum_precision = mode == MODE_F64 ? 64 : 32;
     }
     if (fin.degenerate > 0) {
         set_last_error("NaN/Inf Aberth step: a root landed on a star or another root, or stars coincide");

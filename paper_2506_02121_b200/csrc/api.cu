@@ -30,8 +30,8 @@ int device_sm_count()
 // implemented in the other translation units
 int plan_subchains_host(int64_t, int64_t, int32_t, int32_t, int64_t *, int64_t *, int64_t *);
 int critical_curves_impl(const double *, const double *, int64_t, double, double, int64_t, double, int32_t,
-                         double *, const mlcc_options *, const double *, int32_t *, int32_t *, mlcc_stats *,
-                         cudaStream_t);
+                         double *, double *, const mlcc_options *, const double *, int32_t *, int32_t *,
+                         mlcc_stats *, cudaStream_t);
 int caustics_impl(const double *, const double *, int64_t, double, double, const double *, int64_t, double *,
                   cudaStream_t);
 int star_field_impl(uint64_t, int64_t, double, int, const double *, double *, double *, double *, cudaStream_t);
@@ -102,6 +102,7 @@ void mlcc_options_default(mlcc_options *opt)
     opt->phi_index_offset = 0;
     opt->phi_index_total = 0;
     opt->min_lanes_per_root = 0;
+    opt->aberth_sum_precision = 0;
 }
 
 int mlcc_star_field(uint64_t seed, int64_t N, double kappa_star, int mass_model, const double *mass_params,
@@ -115,7 +116,7 @@ int mlcc_critical_curves(const double *star_xy, const double *masses, int64_t N,
                          int64_t num_phi, double tol, int32_t max_iter, double *out_roots)
 {
     return critical_curves_impl(star_xy, masses, N, kappa_s, gamma, num_phi, tol, max_iter, out_roots, nullptr,
-                                nullptr, nullptr, nullptr, nullptr, nullptr);
+                                nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
 }
 
 int mlcc_critical_curves_ex(const double *star_xy, const double *masses, int64_t N, double kappa_s, double gamma,
@@ -123,8 +124,19 @@ int mlcc_critical_curves_ex(const double *star_xy, const double *masses, int64_t
                             const mlcc_options *opt, const double *init_roots, int32_t *out_iters,
                             int32_t *out_unconverged, mlcc_stats *out_stats, void *stream)
 {
-    return critical_curves_impl(star_xy, masses, N, kappa_s, gamma, num_phi, tol, max_iter, out_roots, opt,
-                                init_roots, out_iters, out_unconverged, out_stats,
+    return critical_curves_impl(star_xy, masses, N, kappa_s, gamma, num_phi, tol, max_iter, out_roots, nullptr,
+                                opt, init_roots, out_iters, out_unconverged, out_stats,
+                                static_cast<cudaStream_t>(stream));
+}
+
+int mlcc_curves_and_caustics(const double *star_xy, const double *masses, int64_t N, double kappa_s, double gamma,
+                             int64_t num_phi, double tol, int32_t max_iter, double *out_roots,
+                             double *out_caustics, const mlcc_options *opt, const double *init_roots,
+                             int32_t *out_iters, int32_t *out_unconverged, mlcc_stats *out_stats, void *stream)
+{
+    if (!out_caustics) return invalid("null pointer");
+    return critical_curves_impl(star_xy, masses, N, kappa_s, gamma, num_phi, tol, max_iter, out_roots,
+                                out_caustics, opt, init_roots, out_iters, out_unconverged, out_stats,
                                 static_cast<cudaStream_t>(stream));
 }
 
@@ -155,7 +167,7 @@ int mlcc_curves_and_caustics_host(const double *star_xy, const double *masses, i
                                   mlcc_stats *out_stats)
 {
     if (!star_xy || !masses || !out_roots) return invalid("null pointer");
-    if (N < 1 || N > (1 << 29)) return invalid("N out of range");
+    if (N < 1 || N > (1 << 28)) return invalid("N out of range");
     if (num_phi < 1) return invalid("num_phi < 1");
     const size_t n_pts = (size_t)num_phi * 2 * (size_t)N;
     DeviceBuffer d_xy, d_m, d_roots, d_caus;
@@ -166,15 +178,10 @@ int mlcc_curves_and_caustics_host(const double *star_xy, const double *masses, i
     MLCC_CUDA(cudaMemcpyAsync(d_xy.p, star_xy, sizeof(double) * 2 * (size_t)N, cudaMemcpyHostToDevice, 0));
     MLCC_CUDA(cudaMemcpyAsync(d_m.p, masses, sizeof(double) * (size_t)N, cudaMemcpyHostToDevice, 0));
     const int rc = critical_curves_impl(d_xy.as<double>(), d_m.as<double>(), N, kappa_s, gamma, num_phi, tol,
-                                        max_iter, d_roots.as<double>(), opt, nullptr, nullptr, nullptr,
-                                        out_stats, nullptr);
+                                        max_iter, d_roots.as<double>(), out_caustics ? d_caus.as<double>() : nullptr,
+                                        opt, nullptr, nullptr, nullptr, out_stats, nullptr);
     if (rc != MLCC_OK && rc != MLCC_ERR_NOT_CONVERGED && rc != MLCC_ERR_DEGENERATE) return rc;
     const std::string keep = g_last_error;
-    if (out_caustics) {
-        const int rc2 = caustics_impl(d_xy.as<double>(), d_m.as<double>(), N, kappa_s, gamma,
-                                      d_roots.as<double>(), (int64_t)n_pts, d_caus.as<double>(), nullptr);
-        if (rc2 != MLCC_OK) return rc2;
-    }
     MLCC_CUDA(cudaMemcpyAsync(out_roots, d_roots.p, sizeof(double) * 2 * n_pts, cudaMemcpyDeviceToHost, 0));
     if (out_caustics)
         MLCC_CUDA(cudaMemcpyAsync(out_caustics, d_caus.p, sizeof(double) * 2 * n_pts, cudaMemcpyDeviceToHost, 0));

@@ -173,10 +173,60 @@ def test_options_do_not_change_the_root_sets(api, orc):
             seen_iters[(order, nsub)] = st.root_iterations
     # the predictor only removes work
     assert seen_iters[(3, 1)] < seen_iters[(0, 1)]
-    for T in (1, 2, 4, 8, 16, 32, 64, 128, 256):
-        r, it, un, st = api.critical_curves_ex(dxy, dm, cfg.kappa_s, cfg.gamma, num_phi,
-                                               opt=api.options(num_subchains=4, min_lanes_per_root=T))
+    for T in (1, 2, 4, 8, 16, 32, 64, 128):
+        for prec in (32, 64):
+            r, it, un, st = api.critical_curves_ex(dxy, dm, cfg.kappa_s, cfg.gamma, num_phi,
+                                                   opt=api.options(num_subchains=4, min_lanes_per_root=T,
+                                                                   aberth_sum_precision=prec))
+            assert st.aberth_sum_precision == prec
+            assert_rows_match(orc, r.cpu().numpy(), ref)
+
+
+@pytest.mark.parametrize("name,num_phi", [("cfg1", 1000), ("cfg2", 400), ("cfg3", 24)])
+def test_aberth_sum_precision_changes_the_path_not_the_roots(api, orc, name, num_phi):
+    """DESIGN.md reading R19: A = sum 1/(z_k - z_r) multiplies F in the denominator of the update, so its
+    arithmetic (double-single FP32 or FP64 seed) may change iteration counts but not the fixed point."""
+    cfg = CONFIGS[name]
+    xy, m, R = field(orc, cfg)
+    rows = np.arange(num_phi)
+    ref, _, un = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, num_phi, rows, cfg.tol, cfg.max_iter)
+    assert un.sum() == 0
+    out = {}
+    for prec in (32, 64):
+        r, it, unc, st = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, num_phi, cfg.tol,
+                                                cfg.max_iter, opt=api.options(aberth_sum_precision=prec))
+        assert int(unc.sum()) == 0 and st.aberth_sum_precision == prec
         assert_rows_match(orc, r.cpu().numpy(), ref)
+        out[prec] = (r, st)
+    # the two paths agree with each other far inside the tolerance, and cost about the same work
+    err, bij = api.match_root_sets(out[32][0], out[64][0], 1e-13)
+    assert bool(bij.all())
+    assert abs(out[32][1].root_iterations - out[64][1].root_iterations) <= 0.02 * out[64][1].root_iterations
+
+
+@pytest.mark.parametrize("name,num_phi", [("cfg1", 1000), ("cfg2", 4000), ("cfg3", 16)])
+def test_fused_curves_and_caustics(api, orc, name, num_phi):
+    """mlcc_curves_and_caustics: same roots as mlcc_critical_curves_ex bit for bit; its caustic points
+    against the oracle's (1e-9) and against the stand-alone caustic kernel on the same roots."""
+    cfg = CONFIGS[name]
+    xy, m, R = field(orc, cfg)
+    dxy, dm = dev(xy), dev(m)
+    roots, caus, iters, unconv, st = api.curves_and_caustics(dxy, dm, cfg.kappa_s, cfg.gamma, num_phi,
+                                                             cfg.tol, cfg.max_iter)
+    assert int(unconv.sum()) == 0 and st.degenerate_roots == 0
+    plain, it2, un2, st2 = api.critical_curves_ex(dxy, dm, cfg.kappa_s, cfg.gamma, num_phi, cfg.tol, cfg.max_iter)
+    assert torch.equal(plain, roots) and torch.equal(iters, it2)
+    w_kernel = api.caustics(dxy, dm, cfg.kappa_s, cfg.gamma, roots)
+    scale = 1 + float(w_kernel.abs().max())
+    assert float((caus - w_kernel).abs().max()) <= 1e-12 * scale
+    rows = np.arange(num_phi) if cfg.N <= 200 else np.array([0, num_phi // 2, num_phi - 1])
+    step = max(1, len(rows) // 100)
+    rows = rows[::step]
+    ref, _, un = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, num_phi, rows, cfg.tol, cfg.max_iter)
+    w_ref = orc.caustics(xy, m, cfg.kappa_s, cfg.gamma, ref)
+    g, w = roots.cpu().numpy(), caus.cpu().numpy()
+    for i, j in enumerate(rows):
+        assert_caustics_match(g[j], w[j], ref[i], w_ref[i])
 
 
 def test_phase_offset_selects_rows_of_a_larger_grid(api, orc):
@@ -221,8 +271,8 @@ def test_smallest_problem_single_star_single_phase(api, orc):
 
 
 def test_ragged_sizes_span_tiles(api, orc):
-    """N chosen so that stars and roots straddle the 1024-wide shared-memory tiles with a ragged tail."""
-    for N, num_phi in ((513, 7), (1025, 5), (37, 33)):
+    """N chosen so that stars and roots straddle the 256-star shared-memory stages with a ragged tail."""
+    for N, num_phi in ((513, 7), (1025, 5), (37, 33), (255, 9), (256, 9), (257, 9)):
         xy, m, R = orc.star_field(11, N, 0.35, 1)
         ref, _, un = orc.critical_curves(xy, m, 0.05, 0.3, num_phi)
         assert un.sum() == 0
