@@ -164,8 +164,10 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     api.lib()
     n_r = 2 * cfg.N
+    from paper_2506_02121_b200 import sharding
+    phi_off, phi_total = sharding.phase_shard(rank, world, num_phi)
     opt = api.options(num_subchains=args.subchains, predictor_order=args.order, min_lanes_per_root=args.min_lanes,
-                      phi_index_offset=rank * num_phi, phi_index_total=world * num_phi,
+                      phi_index_offset=phi_off, phi_index_total=phi_total,
                       aberth_sum_precision=args.aberth_sum)
 
     roots = torch.empty((num_phi, n_r, 2), dtype=torch.float64, device="cuda")
