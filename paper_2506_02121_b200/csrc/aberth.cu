@@ -37,6 +37,16 @@ namespace mlcc {
 namespace {
 
 constexpr int CTA = 128;          // threads per CTA of the compute kernel
+#ifndef MLCC_ROOTS_PER_THREAD
+#define MLCC_ROOTS_PER_THREAD 2
+#endif
+#ifndef MLCC_MIN_CTAS
+#define MLCC_MIN_CTAS 3
+#endif
+#ifndef MLCC_FINE_FACTOR
+#define MLCC_FINE_FACTOR 4
+#endif
+constexpr int R = MLCC_ROOTS_PER_THREAD;   // roots per thread: every source read from shared memory is used R times
 constexpr int S_TILE = 256;       // stars per stage; a stage also holds the 2*S_TILE roots paired with them
 constexpr int STAGE_BYTES = S_TILE * 16 + S_TILE * 8 + 2 * S_TILE * 16;
 constexpr int BLOCK = 256;        // threads per CTA of the small kernels
@@ -56,14 +66,15 @@ struct DevState {
     int done;             // all steps finished
     int need_seed;        // the seed kernel must write starting values for this step
     int cur;              // which of the two active lists is current
-    int T;                // lanes per root of the next compute launch
+    int T;                // threads per root in the coarse tiles of the next compute launch
+    int Tf;               // threads per root in its fine tiles (the last, partial round of work)
+    int n_coarse;         // coarse tiles: tiles [0, n_coarse) are coarse, [n_coarse, n_tiles) fine
     int n_tiles;          // CTA tiles of the next compute launch
     int next_tile;        // tile counter of the running compute launch (atomic)
     int total_active;     // unfrozen roots over all slots
     int total_iterations;
     int unconverged_rows;
     int degenerate;
-    int pad_;
     long long root_iterations;
     long long launches_used;  // compute launches that did work
 };
@@ -82,7 +93,7 @@ struct Params {
     int max_iter_cold;
     int order;                // predictor order
     int min_T;
-    int tiles_target;         // the compute launch wants at least this many tiles
+    int grid_ctas;            // CTAs of the compute launch (all resident: one "round" = grid_ctas tiles)
     const double2 *rot;       // [num_phi]  (1-kappa_s) e^{-i phi_j}
     const double2 *init_roots;  // [n_r] or null
     double2 *roots;           // [num_phi][n_r]
@@ -108,7 +119,8 @@ struct Params {
     int *slot_dir;            // [MAX_SLOTS] -1, +1 (0 = centre)
     int *slot_iters;          // [MAX_SLOTS] iteration at which the slot last had unfrozen roots
     int *n_active;            // [2][MAX_SLOTS]
-    int *tile_start;          // [MAX_SLOTS + 1]
+    int *tile_start;          // [2][MAX_SLOTS + 1] first coarse / first fine tile of each slot
+    int *coarse_roots;        // [MAX_SLOTS] unfrozen roots of the slot covered by its coarse tiles
     int *list;                // [2][max_slots][n_r]
     double2 *delta;           // [max_slots][n_r]
     int max_slots;            // slots that can be live at once (2 n_sub)
@@ -349,26 +361,59 @@ struct __align__(128) Stage {
     float4 rp[2 * S_TILE];   // the slot's source entries 2 j0 .. 2 j0 + 2 S_TILE
 };
 
+// One Aberth step for the unfrozen root at position `pos` of the slot's list, from its reduced sums
+//   v[0..1] = Re S2, (Im S2)/2;  v[2..3] = S3;  v[4..5] = 2 S1 - A;  v[6..7] = Sm (CAUS only).
+template <bool CAUS>
+__device__ __forceinline__ void aberth_step(const Params &p, int slot, long long row, const int *list, int pos,
+                                            const double *v)
+{
+    const int k = list[pos];
+    const double2 z = p.roots[row * p.n_r + k];
+    const double2 rot = p.rot[row];
+    const double s2x = v[0], s2y = 2.0 * v[1], s3x = v[2], s3y = v[3], tx = v[4], ty = v[5];
+    const double fx_ = p.gamma + s2x - rot.x;   // F
+    const double fy_ = s2y - rot.y;
+    const double gx = -2.0 * s3x;               // F'
+    const double gy = -2.0 * s3y;
+    const double dnx = gx + (fx_ * tx - fy_ * ty);  // F' + F (2 S1 - A)
+    const double dny = gy + (fx_ * ty + fy_ * tx);
+    const double dn2 = dnx * dnx + dny * dny;
+    double2 d;
+    d.x = (fx_ * dnx + fy_ * dny) / dn2;          // F / den
+    d.y = (fy_ * dnx - fx_ * dny) / dn2;
+    p.delta[(long long)slot * p.n_r + pos] = d;
+    if (CAUS) {
+        // caustic point of z' = z - Delta (Eq. 12) from the sums at z:
+        // Sm(z') = Sm + Delta S2 + Delta^2 S3 + O(Delta^3 S4), Sm = sum m_i/(z - z_i);
+        // exact to rounding once the root freezes (|Delta| < tol).  Rewritten every iteration.
+        const double d2x = d.x * d.x - d.y * d.y, d2y = 2.0 * d.x * d.y;
+        const double mx = v[6] + (d.x * s2x - d.y * s2y) + (d2x * s3x - d2y * s3y);
+        const double my = v[7] + (d.x * s2y + d.y * s2x) + (d2x * s3y + d2y * s3x);
+        const double nx = z.x - d.x, ny = z.y - d.y;
+        double2 c;
+        c.x = fma(p.omk + p.gamma, nx, -mx);   // (1-kappa_s) x + gamma x - Re Sm
+        c.y = fma(p.omk - p.gamma, ny, my);    // (1-kappa_s) y - gamma y + Im Sm  (conj)
+        p.caustics[row * p.n_r + k] = c;
+    }
+}
+
+// Thread layout of a tile with T threads per root: G = CTA / T threads share one value of `sub`
+// (the share of the sources they sum: sources sub, sub + T, sub + 2T, ... of every stage) and
+// thread (sub, local) owns the R roots at tile positions local, G + local, ...  For T <= CTA / 32
+// a warp has ONE sub, so every shared-memory read in the pair loop is a warp-wide broadcast: a
+// read costs the same wavefronts whatever T is, and each value read is used for R roots.
 template <int MODE, bool CAUS>
-__global__ void __launch_bounds__(CTA, 4) k_compute(Params p)
+__global__ void __launch_bounds__(CTA, MLCC_MIN_CTAS) k_compute(Params p)
 {
     __shared__ Stage s_stage[2];
     __shared__ __align__(8) unsigned long long s_full[2];
-    __shared__ double s_red[CTA / 32][8];
     __shared__ int s_tile;
+    constexpr int NV = CAUS ? 8 : 6;
+    static_assert(sizeof(Stage) * 2 >= (size_t)NV * R * CTA * sizeof(double), "reduction scratch aliases the stages");
 
     const DevState st = *p.state;
     if (st.done) return;
-    const int T = st.T;                 // lanes per root (power of two, 1..CTA)
-    const int TL = T < 32 ? T : 32;     // of which inside one warp
-    const int W = T / TL;               // warps per root
-    const int roots_per_tile = CTA / T;
     const int tid = threadIdx.x;
-    const int lane = tid & 31;
-    const int warp = tid >> 5;
-    const int local_root = tid / T;     // position of this thread's root inside the tile
-    const int sub = tid % T;            // which share of the sources it sums
-    const int n_it = S_TILE / T;        // loop iterations per stage (>= 2)
     const int n_stage = p.N_pad / S_TILE;
     const int n_src = 2 * p.N_pad;
     const int *n_active = p.n_active + st.cur * MAX_SLOTS;
@@ -386,11 +431,21 @@ __global__ void __launch_bounds__(CTA, 4) k_compute(Params p)
         __syncthreads();
         const int tile = s_tile;
         if (tile >= st.n_tiles) break;
-        // slot of this tile: last slot with tile_start <= tile
-        int lo = 0, hi = st.n_slots;
+        // coarse tiles first (whole rounds of the grid), then fine tiles (more threads per root, fewer
+        // roots per tile) that even out the last, partial round
+        const bool fine = tile >= st.n_coarse;
+        const int T = fine ? st.Tf : st.T;   // threads per root (power of two, 1..CTA)
+        const int G = CTA / T;
+        const int sub = tid / G;
+        const int local = tid - sub * G;
+        const int n_it = S_TILE / T;         // pair-loop iterations per stage (even, >= 2)
+        const int tile_roots = R * G;
+        const int *tab = p.tile_start + (fine ? MAX_SLOTS + 1 : 0);
+        const int tt = fine ? tile - st.n_coarse : tile;
+        int lo = 0, hi = st.n_slots;         // slot of this tile: last slot with tab[slot] <= tt
         while (hi - lo > 1) {
             const int mid = (lo + hi) >> 1;
-            if (p.tile_start[mid] <= tile) lo = mid; else hi = mid;
+            if (tab[mid] <= tt) lo = mid; else hi = mid;
         }
         const int slot = lo;
         const long long row = p.slot_row[slot];
@@ -403,24 +458,32 @@ __global__ void __launch_bounds__(CTA, 4) k_compute(Params p)
             tma_load(s_stage[b].rp, slot_src, 2 * S_TILE * 16, &s_full[b]);
         }
         const int *list = p.list + ((long long)st.cur * p.max_slots + slot) * p.n_r;
-        const int pos = (tile - p.tile_start[slot]) * roots_per_tile + local_root;
-        const bool valid = pos < n_active[slot];
-        int k = 0;
-        double zx = 0.0, zy = 0.0;
-        if (valid) {
-            k = list[pos];
-            const double2 z = p.roots[row * p.n_r + k];
-            zx = z.x;
-            zy = z.y;
+        const int n_act = n_active[slot];
+        const int base = (fine ? p.coarse_roots[slot] : 0) + (tt - tab[slot]) * tile_roots;
+        const bool valid = base + local < n_act;   // this thread has at least its first root
+        double zx[R], zy[R];
+        float zxh[R], zxl[R], zyh[R], zyl[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            // a thread whose r-th position is past the end repeats its first root (result dropped)
+            const int pos = base + r * G + local;
+            const int pp = pos < n_act ? pos : base + local;
+            double2 z = make_double2(0.0, 0.0);
+            if (valid) z = p.roots[row * p.n_r + list[pp]];
+            zx[r] = z.x;
+            zy[r] = z.y;
+            split_ds(z.x, zxh[r], zxl[r]);
+            split_ds(z.y, zyh[r], zyl[r]);
         }
-        float zxh, zxl, zyh, zyl;
-        split_ds(zx, zxh, zxl);
-        split_ds(zy, zyh, zyl);
-        const float2 zxh2 = make_float2(zxh, zxh), zyh2 = make_float2(zyh, zyh);
-        const float2 zxl2 = make_float2(zxl, zxl), zyl2 = make_float2(zyl, zyl);
-        StarAcc acc = {0, 0, 0, 0, 0, 0, 0, 0};
-        double ax = 0, ay = 0, bx = 0, by = 0;                     // MODE_F64: two chains
-        float2 fx = make_float2(0.f, 0.f), fy = make_float2(0.f, 0.f);   // MODE_F32: packed lanes
+        StarAcc acc[R];
+        double ax[R], ay[R], bx[R], by[R];   // MODE_F64: two chains
+        float2 fx[R], fy[R];                 // MODE_F32: packed lanes
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            acc[r] = StarAcc{0, 0, 0, 0, 0, 0, 0, 0};
+            ax[r] = ay[r] = bx[r] = by[r] = 0.0;
+            fx[r] = fy[r] = make_float2(0.f, 0.f);
+        }
 
         for (int t = 0; t < n_stage; ++t, ++g) {
             const unsigned b = g & 1u;
@@ -434,176 +497,213 @@ __global__ void __launch_bounds__(CTA, 4) k_compute(Params p)
             mbar_wait(&s_full[b], (g >> 1) & 1u);
             if (valid) {
                 const Stage &sg = s_stage[b];
-                // blocks of independent (1 star + 2 roots) bodies with no exit in between, so that
-                // their dependent chains (|d|^2 -> reciprocal -> powers) interleave
-                if (n_it >= 4) {
-                    for (int i = 0; i < n_it; i += 4) {
-#pragma unroll
-                        for (int u = 0; u < 4; ++u) {
-                            const int j = sub + (i + u) * T;
-                            pair_star<CAUS>(zx, zy, sg.sxy[j], sg.sm[j], acc);
-                            if (MODE == MODE_F64) {
-                                const double2 *r = reinterpret_cast<const double2 *>(sg.rp);
-                                pair_root_f64(zx, zy, r[2 * j], ax, ay);
-                                pair_root_f64(zx, zy, r[2 * j + 1], bx, by);
-                            } else {
-                                pair_root2_f32(zxh2, zyh2, zxl2, zyl2, sg.rp[2 * j], sg.rp[2 * j + 1], fx, fy);
-                            }
-                        }
-                    }
-                } else {
+                // blocks of 2 sources x R roots: independent (1 star + 2 roots) bodies with no exit in
+                // between, so that their dependent chains (|d|^2 -> reciprocal -> powers) interleave
+                for (int i = 0; i < n_it; i += 2) {
 #pragma unroll
                     for (int u = 0; u < 2; ++u) {
-                        const int j = sub + u * T;
-                        pair_star<CAUS>(zx, zy, sg.sxy[j], sg.sm[j], acc);
+                        const int j = sub + (i + u) * T;
+                        const double2 sxy = sg.sxy[j];
+                        const double sm = sg.sm[j];
                         if (MODE == MODE_F64) {
-                            const double2 *r = reinterpret_cast<const double2 *>(sg.rp);
-                            pair_root_f64(zx, zy, r[2 * j], ax, ay);
-                            pair_root_f64(zx, zy, r[2 * j + 1], bx, by);
+                            const double2 *rr = reinterpret_cast<const double2 *>(sg.rp);
+                            const double2 ra = rr[2 * j], rb = rr[2 * j + 1];
+#pragma unroll
+                            for (int r = 0; r < R; ++r) {
+                                pair_star<CAUS>(zx[r], zy[r], sxy, sm, acc[r]);
+                                pair_root_f64(zx[r], zy[r], ra, ax[r], ay[r]);
+                                pair_root_f64(zx[r], zy[r], rb, bx[r], by[r]);
+                            }
                         } else {
-                            pair_root2_f32(zxh2, zyh2, zxl2, zyl2, sg.rp[2 * j], sg.rp[2 * j + 1], fx, fy);
+                            const float4 h = sg.rp[2 * j], l = sg.rp[2 * j + 1];
+#pragma unroll
+                            for (int r = 0; r < R; ++r) {
+                                pair_star<CAUS>(zx[r], zy[r], sxy, sm, acc[r]);
+                                pair_root2_f32(make_float2(zxh[r], zxh[r]), make_float2(zyh[r], zyh[r]),
+                                               make_float2(zxl[r], zxl[r]), make_float2(zyl[r], zyl[r]), h, l,
+                                               fx[r], fy[r]);
+                            }
                         }
                     }
                 }
             }
             __syncthreads();   // everyone is done with buffer b before it is refilled
         }
-        // ---- reduce the T partial sums ----
-        if (MODE == MODE_F32) {
-            ax = (double)fx.x + (double)fx.y;
-            ay = (double)fy.x + (double)fy.y;
+        // ---- this thread's partial sums ----
+        double v[R][NV];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            double sax, say;
+            if (MODE == MODE_F32) {
+                sax = (double)fx[r].x + (double)fx[r].y;
+                say = (double)fy[r].x + (double)fy[r].y;
+            } else {
+                sax = ax[r] + bx[r];
+                say = ay[r] + by[r];
+            }
+            v[r][0] = acc[r].s2x; v[r][1] = acc[r].s2h; v[r][2] = acc[r].s3x; v[r][3] = acc[r].s3y;
+            v[r][4] = 2.0 * acc[r].s1x - sax;   // 2 S1 - A
+            v[r][5] = 2.0 * acc[r].s1y - say;
+            if (CAUS) { v[r][NV - 2] = acc[r].smx; v[r][NV - 1] = acc[r].smy; }
+        }
+        if (T == 1) {
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const int pos = base + r * G + local;
+                if (pos < n_act) aberth_step<CAUS>(p, slot, row, list, pos, v[r]);
+            }
         } else {
-            ax += bx;
-            ay += by;
-        }
-        double v[8];
-        v[0] = acc.s2x; v[1] = acc.s2h; v[2] = acc.s3x; v[3] = acc.s3y;
-        v[4] = 2.0 * acc.s1x - ax;   // 2 S1 - A
-        v[5] = 2.0 * acc.s1y - ay;
-        v[6] = acc.smx; v[7] = acc.smy;
-        constexpr int NV = CAUS ? 8 : 6;
-        for (int o = TL >> 1; o > 0; o >>= 1) {
+            // combine the T shares through shared memory (the stage buffers are idle: every stage of
+            // this tile has been consumed and the next tile's first copy is issued after the barrier below)
+            double *red = reinterpret_cast<double *>(s_stage);   // [NV][T][tile_roots]
 #pragma unroll
-            for (int q = 0; q < NV; ++q) v[q] += __shfl_xor_sync(0xffffffffu, v[q], o);
-        }
-        if (W > 1) {
-            if (lane == 0) {
+            for (int r = 0; r < R; ++r)
 #pragma unroll
-                for (int q = 0; q < NV; ++q) s_red[warp][q] = v[q];
-            }
+                for (int q = 0; q < NV; ++q) red[(q * T + sub) * tile_roots + r * G + local] = v[r][q];
             __syncthreads();
-            if (sub == 0) {
-                for (int w2 = 1; w2 < W; ++w2) {
+            if (tid < tile_roots && base + tid < n_act) {
+                double w[NV];
 #pragma unroll
-                    for (int q = 0; q < NV; ++q) v[q] += s_red[warp + w2][q];
+                for (int q = 0; q < NV; ++q) {
+                    double sum = 0.0;
+                    for (int s2 = 0; s2 < T; ++s2) sum += red[(q * T + s2) * tile_roots + tid];
+                    w[q] = sum;
                 }
+                aberth_step<CAUS>(p, slot, row, list, base + tid, w);
             }
+            // order these generic-proxy accesses before the async-proxy (TMA) writes of the next tile
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         }
-        // ---- Aberth step ----
-        if (valid && sub == 0) {
-            const double2 rot = p.rot[row];
-            const double s2x = v[0], s2y = 2.0 * v[1], s3x = v[2], s3y = v[3], tx = v[4], ty = v[5];
-            const double fx_ = p.gamma + s2x - rot.x;   // F
-            const double fy_ = s2y - rot.y;
-            const double gx = -2.0 * s3x;               // F'
-            const double gy = -2.0 * s3y;
-            const double dnx = gx + (fx_ * tx - fy_ * ty);  // F' + F (2 S1 - A)
-            const double dny = gy + (fx_ * ty + fy_ * tx);
-            const double dn2 = dnx * dnx + dny * dny;
-            double2 d;
-            d.x = (fx_ * dnx + fy_ * dny) / dn2;          // F / den
-            d.y = (fy_ * dnx - fx_ * dny) / dn2;
-            p.delta[(long long)slot * p.n_r + pos] = d;
-            if (CAUS) {
-                // caustic point of z' = z - Delta (Eq. 12) from the sums at z:
-                // Sm(z') = Sm + Delta S2 + Delta^2 S3 + O(Delta^3 S4), Sm = sum m_i/(z - z_i);
-                // exact to rounding once the root freezes (|Delta| < tol).  Rewritten every iteration.
-                const double d2x = d.x * d.x - d.y * d.y, d2y = 2.0 * d.x * d.y;
-                const double mx = v[6] + (d.x * s2x - d.y * s2y) + (d2x * s3x - d2y * s3y);
-                const double my = v[7] + (d.x * s2y + d.y * s2x) + (d2x * s3y + d2y * s3x);
-                const double nx = zx - d.x, ny = zy - d.y;
-                double2 c;
-                c.x = fma(p.omk + p.gamma, nx, -mx);   // (1-kappa_s) x + gamma x - Re Sm
-                c.y = fma(p.omk - p.gamma, ny, my);    // (1-kappa_s) y - gamma y + Im Sm  (conj)
-                p.caustics[row * p.n_r + k] = c;
-            }
-        }
-        __syncthreads();   // s_tile and s_red are rewritten by the next tile
+        __syncthreads();   // s_tile and the stage buffers are rewritten by the next tile
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// apply kernel: z_k -= Delta_k, freeze converged roots, compact the list of unfrozen roots
-// grid: (ceil(n_r / BLOCK), max_slots)
+// apply kernel: z_k -= Delta_k, freeze converged roots, compact the list of unfrozen roots.
+// One CTA per slot walks the slot's list in chunks and keeps the survivors IN ORDER (block-wide
+// exclusive scan), so the next iteration's tiles -- and with them the summation order of every
+// root -- do not depend on the timing of this launch: two runs give the same bits.
+// grid: max_slots CTAs of APPLY_THREADS threads
 // ------------------------------------------------------------------------------------------------
+constexpr int APPLY_THREADS = 1024;
+constexpr int APPLY_ITEMS = 4;
+
 template <int MODE>
-__global__ void k_apply(Params p)
+__global__ void __launch_bounds__(APPLY_THREADS) k_apply(Params p)
 {
+    __shared__ int s_warp[32];
+    __shared__ int s_total;
     const DevState st = *p.state;
     if (st.done) return;
-    const int slot = blockIdx.y;
+    const int slot = blockIdx.x;
     if (slot >= st.n_slots) return;
     const int n_act = p.n_active[st.cur * MAX_SLOTS + slot];
-    const int pos = blockIdx.x * blockDim.x + threadIdx.x;
-    if (blockIdx.x * blockDim.x >= n_act) return;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int *list = p.list + ((long long)st.cur * p.max_slots + slot) * p.n_r;
     int *next = p.list + ((long long)(st.cur ^ 1) * p.max_slots + slot) * p.n_r;
-    bool keep = false;
-    int k = 0;
-    if (pos < n_act) {
-        k = list[pos];
-        const double2 d = p.delta[(long long)slot * p.n_r + pos];
-        const double d2 = d.x * d.x + d.y * d.y;
-        double2 *zp = p.roots + p.slot_row[slot] * p.n_r + k;
-        if (d2 <= 1.79769313486231570e308) {   // finite step
-            double2 z = *zp;
-            z.x -= d.x;
-            z.y -= d.y;
-            *zp = z;
-            store_src<MODE>(p.src + (size_t)slot * 2 * p.N_pad, k, z);
-            keep = !(d2 < p.tol2);
-        } else {                                // NaN / Inf: freeze where it is, report
-            atomicAdd(&p.state->degenerate, 1);
-        }
-    }
-    const unsigned mask = __ballot_sync(0xffffffffu, keep);
-    const int lane = threadIdx.x & 31;
+    const double2 *delta = p.delta + (long long)slot * p.n_r;
+    double2 *row = p.roots + p.slot_row[slot] * p.n_r;
+    float4 *slot_src = p.src + (size_t)slot * 2 * p.N_pad;
     int base = 0;
-    if (lane == 0 && mask) base = atomicAdd(&p.n_active[(st.cur ^ 1) * MAX_SLOTS + slot], __popc(mask));
-    base = __shfl_sync(0xffffffffu, base, 0);
-    if (keep) next[base + __popc(mask & ((1u << lane) - 1u))] = k;
+    for (int c0 = 0; c0 < n_act; c0 += APPLY_THREADS * APPLY_ITEMS) {
+        int ks[APPLY_ITEMS];
+        bool keep[APPLY_ITEMS];
+        int cnt = 0;
+#pragma unroll
+        for (int i = 0; i < APPLY_ITEMS; ++i) {
+            const int pos = c0 + tid * APPLY_ITEMS + i;
+            keep[i] = false;
+            ks[i] = 0;
+            if (pos < n_act) {
+                const int k = list[pos];
+                const double2 d = delta[pos];
+                const double d2 = d.x * d.x + d.y * d.y;
+                if (d2 <= 1.79769313486231570e308) {   // finite step
+                    double2 z = row[k];
+                    z.x -= d.x;
+                    z.y -= d.y;
+                    row[k] = z;
+                    store_src<MODE>(slot_src, k, z);
+                    keep[i] = !(d2 < p.tol2);
+                } else {                                // NaN / Inf: freeze where it is, report
+                    atomicAdd(&p.state->degenerate, 1);
+                }
+                ks[i] = k;
+                cnt += keep[i] ? 1 : 0;
+            }
+        }
+        int incl = cnt;   // inclusive scan over the warp, then over the warps
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int n = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += n;
+        }
+        if (lane == 31) s_warp[warp] = incl;
+        __syncthreads();
+        if (warp == 0) {
+            const int w = s_warp[lane];
+            int wi = w;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int n = __shfl_up_sync(0xffffffffu, wi, o);
+                if (lane >= o) wi += n;
+            }
+            s_warp[lane] = wi - w;
+            if (lane == 31) s_total = wi;
+        }
+        __syncthreads();
+        int off = base + s_warp[warp] + incl - cnt;
+#pragma unroll
+        for (int i = 0; i < APPLY_ITEMS; ++i)
+            if (keep[i]) next[off++] = ks[i];
+        base += s_total;
+        __syncthreads();
+    }
+    if (tid == 0) p.n_active[(st.cur ^ 1) * MAX_SLOTS + slot] = base;
 }
 
 // ------------------------------------------------------------------------------------------------
 // finalize kernel (one thread): advances the state machine
 // ------------------------------------------------------------------------------------------------
-// lanes per root: the smallest power of two that cuts the unfrozen roots into at least
-// tiles_target tiles (many more tiles than SMs: the atomic tile counter then balances the SMs to
-// within one tile), so a launch with few unfrozen roots still uses the whole machine
-__device__ int pick_T(const Params &p, int total_active)
-{
-    int T = 1;
-    while (T < CTA && ((long long)total_active * T + CTA - 1) / CTA < p.tiles_target) T <<= 1;
-    if (T < p.min_T) T = p.min_T;
-    return T;
-}
-
-// one thread: tile table for the counts in n_active[cur]
+// One thread: the tile table of the next compute launch for the counts in n_active[cur].
+// All grid_ctas CTAs are resident and pull tiles from one atomic counter, and tiles of one kind take the
+// same time, so a launch lasts ceil(tiles / grid_ctas) tile-times: with a handful of tiles per CTA
+// the last, partial round costs up to a whole round.  Hence two kinds of tile:
+//   coarse: T threads per root, R CTA / T roots per tile, T the smallest power of two that gives at
+//           least two rounds; only WHOLE rounds of them are handed out;
+//   fine:   Tf = MLCC_FINE_FACTOR T threads per root for what is left of every slot's list, so the
+//           partial round is quantised in units of 1 / MLCC_FINE_FACTOR of a coarse tile.
 __device__ void build_tiles(const Params &p, DevState &st)
 {
     const int *n_active = p.n_active + st.cur * MAX_SLOTS;
-    int total = 0;
+    long long total = 0;
     for (int s = 0; s < st.n_slots; ++s) total += n_active[s];
-    st.total_active = total;
-    st.T = pick_T(p, total);
-    const int rpt = CTA / st.T;
-    int t = 0;
+    st.total_active = (int)total;
+    int T = 1;
+    while (T < CTA && total * T / (R * CTA) < 2LL * p.grid_ctas) T <<= 1;
+    if (T < p.min_T) T = p.min_T;
+    int Tf = T * MLCC_FINE_FACTOR;
+    if (Tf > CTA) Tf = CTA;
+    const int tile_c = R * CTA / T, tile_f = R * CTA / Tf;
+    long long W = 0;   // coarse tiles if every slot were cut into coarse tiles only (whole tiles)
+    for (int s = 0; s < st.n_slots; ++s) W += n_active[s] / tile_c;
+    const long long C = (W / p.grid_ctas) * p.grid_ctas;   // whole rounds
+    int *tab_c = p.tile_start, *tab_f = p.tile_start + MAX_SLOTS + 1;
+    int tc = 0, tf = 0;
     for (int s = 0; s < st.n_slots; ++s) {
-        p.tile_start[s] = t;
-        t += (n_active[s] + rpt - 1) / rpt;
+        const int c_s = (W > 0 && Tf != T) ? (int)((long long)(n_active[s] / tile_c) * C / W) : 0;
+        tab_c[s] = tc;
+        tc += c_s;
+        p.coarse_roots[s] = c_s * tile_c;
+        tab_f[s] = tf;
+        tf += (n_active[s] - c_s * tile_c + tile_f - 1) / tile_f;
     }
-    p.tile_start[st.n_slots] = t;
-    st.n_tiles = t;
+    tab_c[st.n_slots] = tc;
+    tab_f[st.n_slots] = tf;
+    st.T = T;
+    st.Tf = Tf;
+    st.n_coarse = tc;
+    st.n_tiles = tc + tf;
     st.next_tile = 0;
 }
 
@@ -667,8 +767,8 @@ __global__ void k_init(Params p)
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     DevState st;
     st.step = 0; st.iter = 0; st.n_slots = 0; st.done = 0; st.need_seed = 1; st.cur = 0;
-    st.T = 1; st.n_tiles = 0; st.next_tile = 0; st.total_active = 0; st.total_iterations = 0;
-    st.unconverged_rows = 0; st.degenerate = 0; st.pad_ = 0; st.root_iterations = 0; st.launches_used = 0;
+    st.T = 1; st.Tf = 1; st.n_coarse = 0; st.n_tiles = 0; st.next_tile = 0; st.total_active = 0; st.total_iterations = 0;
+    st.unconverged_rows = 0; st.degenerate = 0; st.root_iterations = 0; st.launches_used = 0;
     build_slots(p, st);
     build_tiles(p, st);
     *p.state = st;
@@ -840,7 +940,8 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
         (e = ws.alloc(&p.slot_dir, MAX_SLOTS)) != cudaSuccess ||
         (e = ws.alloc(&p.slot_iters, MAX_SLOTS)) != cudaSuccess ||
         (e = ws.alloc(&p.n_active, 2 * MAX_SLOTS)) != cudaSuccess ||
-        (e = ws.alloc(&p.tile_start, MAX_SLOTS + 1)) != cudaSuccess ||
+        (e = ws.alloc(&p.tile_start, 2 * (MAX_SLOTS + 1))) != cudaSuccess ||
+        (e = ws.alloc(&p.coarse_roots, MAX_SLOTS)) != cudaSuccess ||
         (e = ws.alloc(&p.list, (size_t)2 * max_slots * n_r)) != cudaSuccess ||
         (e = ws.alloc(&p.delta, (size_t)max_slots * n_r)) != cudaSuccess) {
         if (e == cudaErrorMemoryAllocation) {
@@ -895,7 +996,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     p.max_iter_cold = opt.max_iter_cold > 0 ? opt.max_iter_cold : max_iter;
     p.order = order;
     p.min_T = min_T;
-    p.tiles_target = 12 * sms;
+    p.grid_ctas = grid_compute;
     p.rot = d_rot;
     p.init_roots = reinterpret_cast<const double2 *>(init_roots);
     p.roots = reinterpret_cast<double2 *>(out_roots);
@@ -922,7 +1023,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     const int grid_seed = sms * 4;
     ks.prepare<<<grid_seed, BLOCK, 0, stream>>>(p);
     k_init<<<1, 32, 0, stream>>>(p);
-    const dim3 grid_apply((unsigned)((n_r + BLOCK - 1) / BLOCK), (unsigned)max_slots);
+    const int grid_apply = max_slots;
     int64_t launches = 3;   // check, prepare, init
     // Upper bound on iteration groups, so that a device-side fault cannot spin the host forever.
     const long long max_groups = (long long)(max_steps + 1) * (long long)(p.max_iter > p.max_iter_cold ? p.max_iter : p.max_iter_cold) + 8;
@@ -935,7 +1036,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
         for (int g = 0; g < chunk; ++g) {
             ks.seed<<<grid_seed, BLOCK, 0, stream>>>(p);
             ks.compute<<<grid_compute, CTA, 0, stream>>>(p);
-            ks.apply<<<grid_apply, BLOCK, 0, stream>>>(p);
+            ks.apply<<<grid_apply, APPLY_THREADS, 0, stream>>>(p);
             k_finalize<<<1, 32, 0, stream>>>(p);
         }
         launches += 4 * chunk;
