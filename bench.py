@@ -49,6 +49,9 @@ def parse():
     ap.add_argument("--min-lanes", type=int, default=0)
     ap.add_argument("--aberth-sum", type=int, default=0, choices=[0, 32, 64],
                     help="arithmetic of the Aberth sum: 32 = double-single FP32 (default), 64 = FP64 seed form")
+    ap.add_argument("--star-sums", default="direct", choices=["direct", "fmm"],
+                    help="direct: O(N) star sums as BASELINE.json fixes (headline); fmm: the paper's near/far split "
+                         "(PAPER.md:188-195) -- the roofline object then counts the root pairs only")
     ap.add_argument("--separate-caustics", action="store_true",
                     help="run mlcc_critical_curves_ex + mlcc_caustics instead of the fused call")
     return ap.parse_args()
@@ -168,7 +171,8 @@ def main():
     phi_off, phi_total = sharding.phase_shard(rank, world, num_phi)
     opt = api.options(num_subchains=args.subchains, predictor_order=args.order, min_lanes_per_root=args.min_lanes,
                       phi_index_offset=phi_off, phi_index_total=phi_total,
-                      aberth_sum_precision=args.aberth_sum)
+                      aberth_sum_precision=args.aberth_sum,
+                      star_sum_mode=api.MLCC_STAR_SUMS_FMM if args.star_sums == "fmm" else api.MLCC_STAR_SUMS_DIRECT)
 
     roots = torch.empty((num_phi, n_r, 2), dtype=torch.float64, device="cuda")
     prev = torch.empty_like(roots)
@@ -213,7 +217,7 @@ def main():
         st = step()
         solve_ms += st.solve_ms
         launches += st.kernel_launches + 3 + 1 + (1 if args.separate_caustics else 0)   # star field (3), matcher, caustics
-        alg_flop += FLOP_PER_STAR_PAIR * st.star_pairs + FLOP_PER_ROOT_PAIR * st.root_pairs
+        alg_flop += (0.0 if args.star_sums == "fmm" else FLOP_PER_STAR_PAIR * st.star_pairs) + FLOP_PER_ROOT_PAIR * st.root_pairs
         compute_launches += st.total_iterations
     ev1.record()
     barrier()
@@ -290,7 +294,7 @@ def main():
                                        f"kappa_s={cfg.kappa_s}, gamma={cfg.gamma}, tol={cfg.tol}, max_iter={cfg.max_iter}, seed={cfg.seed}",
                            "step": ("star_field + critical_curves_ex + caustics + match_root_sets" if args.separate_caustics
                                     else "star_field + curves_and_caustics (fused) + match_root_sets"),
-                           "aberth_sum_precision": st.aberth_sum_precision,
+                           "aberth_sum_precision": st.aberth_sum_precision, "star_sums": args.star_sums,
                            "subchains": st.subchains, "predictor_order": st.predictor_order,
                            "l2": f"inputs larger than L2: each step writes {2 * num_phi * n_r * 16 / 1e9:.2f} GB of roots and caustics "
                                  f"and reads a {num_phi * n_r * 16 / 1e9:.2f} GB comparison set (L2 is 126 MB)",

@@ -54,6 +54,15 @@ typedef enum mlcc_status {
 /* Mass models of the star-field generator (BASELINE.json configs; the paper names none). */
 enum { MLCC_MASS_EQUAL = 0, MLCC_MASS_POWER_LAW = 1, MLCC_MASS_BROKEN_POWER_LAW = 2 };
 
+/* How the star sums S1, S2, S3, Sm are evaluated (mlcc_options.star_sum_mode, mlcc_star_sums).
+ * DIRECT: the O(N) sums over all stars as Eq. 15 / Eq. 19 are written (BASELINE.json north_star).
+ * FMM:    the paper's own split (Section 4.1): stars in the 5 x 5 grid nodes around
+ *         the point directly, all other stars through the node's Taylor series.  The truncation
+ *         error is bounded by rho^(order+1), rho = 0.283; with the default
+ *         order 31 it is below FP64 rounding, so the root sets are the same within the parity
+ *         tolerance.  The Aberth sum over the other roots stays direct in both modes.             */
+enum { MLCC_STAR_SUMS_DIRECT = 0, MLCC_STAR_SUMS_FMM = 1 };
+
 /* Options of mlcc_critical_curves_ex.  Zero-initialise, or call mlcc_options_default(). */
 typedef struct mlcc_options {
     int32_t struct_size;      /* = sizeof(mlcc_options)                                             */
@@ -75,6 +84,11 @@ typedef struct mlcc_options {
                                    0 or 32 = double-single FP32 (z = hi + lo, differences exact to
                                    ~2^-23 |z_k - z_r|); 64 = FP64 differences with the 20-bit
                                    reciprocal seed.  Star sums (F, F') are FP64 in both.            */
+    int32_t star_sum_mode;    /* MLCC_STAR_SUMS_DIRECT (default) or MLCC_STAR_SUMS_FMM               */
+    int32_t fmm_order;        /* Taylor order of the node series (1..63); 0 = 31                     */
+    int32_t fmm_stars_per_node; /* mean stars per grid node (the grid has ~N / this many nodes);
+                                   0 = 4                                                             */
+    int32_t reserved_;        /* 0                                                                   */
 } mlcc_options;
 
 /* Counters of one mlcc_critical_curves_ex call (host struct, filled on return). */
@@ -164,6 +178,19 @@ int mlcc_caustics(const double *star_xy, const double *masses, int64_t N, double
                   double gamma, const double *points, int64_t P, double *out_caustics,
                   void *stream);
 
+/* a2 on its own  The four star sums at arbitrary points (Eq. 15 at PAPER.md:128, Eq. 19 at :170,
+ * Eq. 12 at :114):  S1 = sum 1/(z-z_i), S2 = sum m_i/(z-z_i)^2, S3 = sum m_i/(z-z_i)^3,
+ * Sm = sum m_i/(z-z_i), so that F = gamma + S2 - (1-kappa_s) e^{-i phi}, F' = -2 S3,
+ * w = (1-kappa_s) z + gamma conj(z) - conj(Sm).  `mode` is MLCC_STAR_SUMS_DIRECT or
+ * MLCC_STAR_SUMS_FMM (`fmm_order`, `fmm_stars_per_node` as in mlcc_options; 0 = defaults).
+ *   points [P][2]: device, read.
+ *   out_sums [P][8]: device, written: Re S1, Im S1, Re S2, Im S2, Re S3, Im S3, Re Sm, Im Sm.
+ * A point that coincides with a star gives non-finite sums.  Asynchronous on `stream`.
+ * Errors: INVALID_ARG, CUDA, NOMEM.                                                              */
+int mlcc_star_sums(const double *star_xy, const double *masses, int64_t N, const double *points,
+                   int64_t P, int mode, int fmm_order, int fmm_stars_per_node, double *out_sums,
+                   void *stream);
+
 /* a8  Root-set matching validator (BASELINE.json north_star: "root sets per phase are compared
  * after optimal nearest-neighbour matching").  For each of S sets, every a_i is paired with its
  * nearest b_j (uniform-grid search).  If that map is a bijection it is the matching that
@@ -203,6 +230,16 @@ int mlcc_curves_and_caustics_host(const double *star_xy, const double *masses, i
  * *out_tflops (host).  This is the measured denominator of the "alu" roofline in bench.py
  * (MEASURED_PEAKS.json has no FP64 entry).  Synchronises `stream`.                               */
 int mlcc_fp64_peak(double ms_target, double *out_tflops, void *stream);
+
+/* Measurement helper behind DESIGN.md "Measured issue model": the same loop with other operand forms,
+ * rate returned as 2 x FP64 instructions per second / 1e12 (so form 0 equals mlcc_fp64_peak).
+ *   form 0: DFMA, two distinct register sources (the peak form)
+ *   form 1: DFMA, three distinct register sources
+ *   form 2: DADD, two distinct register sources
+ *   form 3: form 0 interleaved 1:1 with packed FP32 FMAs (fma.f32x2, three 64-bit sources); the
+ *           rate counts the FP64 instructions only
+ * Synchronises `stream`.  Errors: INVALID_ARG, CUDA.                                              */
+int mlcc_fp64_issue_probe(int form, double ms_target, double *out_rate, void *stream);
 
 #ifdef __cplusplus
 }

@@ -33,6 +33,8 @@ def lib():
         for f in (L.orc_residuals, L.orc_residuals_ld):
             f.argtypes = [_pd, _pd, C.c_int64, C.c_double, C.c_double, C.c_double, C.c_double,
                           _pd, C.c_int64, _pd]
+        for f in (L.orc_star_sums, L.orc_star_sums_ld):
+            f.argtypes = [_pd, _pd, C.c_int64, _pd, C.c_int64, _pd]
         L.orc_match_root_sets.argtypes = [_pd, _pd, C.c_int64, C.c_int64, C.c_double, _pd, _pi32]
         L.orc_star_field.argtypes = [C.c_uint64, C.c_int64, C.c_double, C.c_int, C.c_void_p,
                                      _pd, _pd, C.POINTER(C.c_double)]
@@ -132,6 +134,16 @@ def residuals(star_xy, masses, kappa_s, gamma, phi_index, num_phi_total, points,
              flat.shape[0], out), "residuals")
     return {"F": out[:, 0] + 1j * out[:, 1], "Fp": out[:, 2] + 1j * out[:, 3],
             "inv_mu": out[:, 4].copy(), "newton": out[:, 5].copy()}
+
+
+def star_sums(star_xy, masses, points, long_double=True):
+    """-> [P, 8]: Re/Im of S1 = sum 1/(z-z_i), S2 = sum m/(z-z_i)^2, S3 = sum m/(z-z_i)^3, Sm = sum m/(z-z_i)."""
+    xy, m, N = _stars(star_xy, masses)
+    flat = np.ascontiguousarray(points, _d).reshape(-1, 2)
+    out = np.empty((flat.shape[0], 8), _d)
+    f = lib().orc_star_sums_ld if long_double else lib().orc_star_sums
+    _check(f(xy, m, N, flat, flat.shape[0], out), "star_sums")
+    return out
 
 
 def match_root_sets(a, b, rel_tol):

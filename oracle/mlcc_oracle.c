@@ -158,6 +158,23 @@ int orc_residuals(const double *star_xy, const double *masses, int64_t N, double
     return 0;
 }
 
+/* S1, S2, S3, Sm at given points (double / long double accumulation). */
+int orc_star_sums(const double *star_xy, const double *masses, int64_t N, const double *points,
+                  int64_t P, double *out)
+{
+    if (N < 1 || P < 0) return -2;
+    star_sums_at_d(star_xy, masses, N, points, P, out);
+    return 0;
+}
+
+int orc_star_sums_ld(const double *star_xy, const double *masses, int64_t N, const double *points,
+                     int64_t P, double *out)
+{
+    if (N < 1 || P < 0) return -2;
+    star_sums_at_ld(star_xy, masses, N, points, P, out);
+    return 0;
+}
+
 /* ------------------------------------------------------------------------------------------
  * Root-set matching (BASELINE.json north_star: "root sets per phase are compared after optimal
  * nearest-neighbour matching").  Brute force: for each a_i the nearest b_j over all j.  If

@@ -21,6 +21,8 @@ MLCC_ERR_CUDA = 2
 MLCC_ERR_NOMEM = 3
 MLCC_ERR_NOT_CONVERGED = 4
 MLCC_ERR_DEGENERATE = 5
+MLCC_STAR_SUMS_DIRECT = 0
+MLCC_STAR_SUMS_FMM = 1
 
 
 class MlccError(RuntimeError):
@@ -33,7 +35,9 @@ class mlcc_options(C.Structure):
     _fields_ = [("struct_size", C.c_int32), ("num_subchains", C.c_int32),
                 ("predictor_order", C.c_int32), ("max_iter_cold", C.c_int32),
                 ("phi_index_offset", C.c_int64), ("phi_index_total", C.c_int64),
-                ("min_lanes_per_root", C.c_int32), ("aberth_sum_precision", C.c_int32)]
+                ("min_lanes_per_root", C.c_int32), ("aberth_sum_precision", C.c_int32),
+                ("star_sum_mode", C.c_int32), ("fmm_order", C.c_int32),
+                ("fmm_stars_per_node", C.c_int32), ("reserved_", C.c_int32)]
 
 
 class mlcc_stats(C.Structure):
@@ -89,12 +93,14 @@ def lib() -> C.CDLL:
                                                C.POINTER(mlcc_stats), vp]
         L.mlcc_caustics.argtypes = [vp, vp, i64, dbl, dbl, vp, i64, vp, vp]
         L.mlcc_match_root_sets.argtypes = [vp, vp, i64, i64, dbl, vp, vp, vp]
+        L.mlcc_star_sums.argtypes = [vp, vp, i64, vp, i64, C.c_int, C.c_int, C.c_int, vp, vp]
         L.mlcc_plan_subchains.argtypes = [i64, i64, i32, i32, vp, vp, vp]
         L.mlcc_critical_curves_host.argtypes = [vp, vp, i64, dbl, dbl, i64, dbl, i32, vp]
         L.mlcc_caustics_host.argtypes = [vp, vp, i64, dbl, dbl, vp, i64, vp]
         L.mlcc_curves_and_caustics_host.argtypes = [vp, vp, i64, dbl, dbl, i64, dbl, i32,
                                                     C.POINTER(mlcc_options), vp, vp, C.POINTER(mlcc_stats)]
         L.mlcc_fp64_peak.argtypes = [dbl, C.POINTER(dbl), vp]
+        L.mlcc_fp64_issue_probe.argtypes = [C.c_int, dbl, C.POINTER(dbl), vp]
         _lib = L
     return _lib
 
@@ -128,7 +134,8 @@ def last_error() -> str:
 
 
 def options(num_subchains=0, predictor_order=-1, max_iter_cold=0, phi_index_offset=0,
-            phi_index_total=0, min_lanes_per_root=0, aberth_sum_precision=0) -> mlcc_options:
+            phi_index_total=0, min_lanes_per_root=0, aberth_sum_precision=0, star_sum_mode=0, fmm_order=0,
+            fmm_stars_per_node=0) -> mlcc_options:
     o = mlcc_options()
     lib().mlcc_options_default(C.byref(o))
     o.num_subchains = num_subchains
@@ -138,6 +145,9 @@ def options(num_subchains=0, predictor_order=-1, max_iter_cold=0, phi_index_offs
     o.phi_index_total = phi_index_total
     o.min_lanes_per_root = min_lanes_per_root
     o.aberth_sum_precision = aberth_sum_precision
+    o.star_sum_mode = star_sum_mode
+    o.fmm_order = fmm_order
+    o.fmm_stars_per_node = fmm_stars_per_node
     return o
 
 
@@ -241,6 +251,19 @@ def caustics(star_xy, masses, kappa_s, gamma, points, out=None):
     return out
 
 
+def star_sums(star_xy, masses, points, mode=MLCC_STAR_SUMS_DIRECT, fmm_order=0, fmm_stars_per_node=0):
+    """mlcc_star_sums: points [P, 2] -> [P, 8] = (S1, S2, S3, Sm) as (re, im) pairs (asynchronous on the current stream)."""
+    N = masses.shape[0]
+    P = points.numel() // 2
+    out = torch.empty((P, 8), dtype=torch.float64, device=masses.device)
+    rc = lib().mlcc_star_sums(_dev(star_xy, name="star_xy"), _dev(masses, name="masses"), N,
+                              _dev(points, name="points"), P, int(mode), int(fmm_order), int(fmm_stars_per_node),
+                              out.data_ptr(), _stream())
+    if rc != MLCC_OK:
+        _raise(rc)
+    return out
+
+
 def match_root_sets(a, b, rel_tol):
     """mlcc_match_root_sets: a, b [S,n,2] -> (max_err [S] f64, bijective [S] i32)."""
     if a.shape != b.shape or a.dim() != 3 or a.shape[2] != 2:
@@ -312,6 +335,15 @@ def caustics_host(star_xy: np.ndarray, masses: np.ndarray, kappa_s, gamma, point
     if rc != MLCC_OK:
         _raise(rc)
     return out
+
+
+def fp64_issue_probe(form: int, ms_target: float = 20.0) -> float:
+    """mlcc_fp64_issue_probe: 2 x FP64 instructions/s / 1e12 of operand form 0..3 (see include/mlcc.h)."""
+    v = C.c_double(0.0)
+    rc = lib().mlcc_fp64_issue_probe(int(form), float(ms_target), C.byref(v), _stream())
+    if rc != MLCC_OK:
+        _raise(rc)
+    return v.value
 
 
 def fp64_peak(ms_target: float = 50.0) -> float:

@@ -17,18 +17,24 @@
 //     [seed, compute, apply, finalize] groups and polls one flag per chunk.  No host round trip
 //     sits inside the iteration loop.
 //   * compute: persistent CTAs of 128 threads pull tiles of unfrozen roots from an atomic counter.
-//     A root's sums are split over T lanes (T = 1..128, chosen on the device so that there are
-//     many more tiles than SMs).  Sources stream through shared memory in double-buffered stages
-//     of 256 stars + 512 roots, each stage filled by three TMA bulk copies (cp.async.bulk) that
-//     complete on an mbarrier, so no thread spends issue slots on loads.  One loop iteration
-//     evaluates one (root, star) pair in FP64 and two (root, root) pairs: the star sums carry F and
-//     must be FP64; the Aberth sum A only steers the convergence RATE (it multiplies F in the
-//     denominator) and is evaluated in double-single FP32 with packed f32x2 instructions, which
-//     read half the register-file bytes of the FP64 form (the register-file read ports, not the
-//     FP64 pipe, bound this kernel: DESIGN.md "Measured issue model").
+//     A thread owns R roots (R = 2), and a root's sums are split over T threads (T = 1..128): the
+//     T shares sit in different warps whenever T <= 4, so every shared-memory read of the pair loop
+//     is a warp-wide broadcast and every value read is used for R roots.  Whole rounds of coarse
+//     tiles are followed by fine tiles (4 T threads per root) that even out the last round.
+//     Sources stream through shared memory in double-buffered stages of 256 stars + 512 roots,
+//     each stage filled by three TMA bulk copies (cp.async.bulk) that complete on an mbarrier, so
+//     no thread spends issue slots on loads.  One loop body evaluates one (root, star) pair in FP64
+//     and two (root, root) pairs: the star sums carry F and must be FP64; the Aberth sum A only
+//     steers the convergence RATE (it multiplies F in the denominator) and is evaluated in
+//     double-single FP32 with packed f32x2 instructions, which read half the register-file bytes
+//     of the FP64 form (register-operand bandwidth, one 64-bit operand per clock per SM
+//     sub-partition, bounds this kernel: DESIGN.md "Measured issue model").
+//   * Far-field mode: k_star_sums evaluates the star sums of every unfrozen root
+//     from the near stars and the node's Taylor series (star_sums.cuh, fmm.cu); the compute kernel
+//     then sums root pairs only (R = 8).
 //   * Jacobi: updates go to a side buffer and are applied by `apply`, which also refreshes the
-//     per-slot source copy of the row and compacts the list of unfrozen roots.
-#include "mlcc_common.cuh"
+//     per-slot source copy of the row and compacts the list of unfrozen roots in order.
+#include "star_sums.cuh"
 
 #include <math.h>
 #include <vector>
@@ -46,7 +52,9 @@ constexpr int CTA = 128;          // threads per CTA of the compute kernel
 #ifndef MLCC_FINE_FACTOR
 #define MLCC_FINE_FACTOR 4
 #endif
-constexpr int R = MLCC_ROOTS_PER_THREAD;   // roots per thread: every source read from shared memory is used R times
+constexpr int R_STARS = MLCC_ROOTS_PER_THREAD;   // roots per thread: every source read from shared memory is used R times
+constexpr int R_ROOTS_F32 = 8;    // ... of the kernel that sums root pairs only (star sums from the node series)
+constexpr int R_ROOTS_F64 = 4;
 constexpr int S_TILE = 256;       // stars per stage; a stage also holds the 2*S_TILE roots paired with them
 constexpr int STAGE_BYTES = S_TILE * 16 + S_TILE * 8 + 2 * S_TILE * 16;
 constexpr int BLOCK = 256;        // threads per CTA of the small kernels
@@ -75,6 +83,7 @@ struct DevState {
     int total_iterations;
     int unconverged_rows;
     int degenerate;
+    int n_outside;        // far-field mode: roots of this iteration that lie outside the node grid (atomic)
     long long root_iterations;
     long long launches_used;  // compute launches that did work
 };
@@ -124,6 +133,11 @@ struct Params {
     int *list;                // [2][max_slots][n_r]
     double2 *delta;           // [max_slots][n_r]
     int max_slots;            // slots that can be live at once (2 n_sub)
+    int R;                    // roots per thread of the compute kernel in use
+    // far-field mode (MLCC_STAR_SUMS_FMM): star sums come from k_star_sums, the compute kernel sums root pairs only
+    double *ssum;             // [max_slots][n_r][8] star sums of the unfrozen roots, by list position
+    int2 *outside;            // [max_slots * n_r] (slot, position) of the roots outside the node grid
+    FmmGrid fmm;
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -210,44 +224,6 @@ __device__ __forceinline__ void store_src(float4 *slot_src, int k, double2 z)
 // ------------------------------------------------------------------------------------------------
 // pair bodies
 // ------------------------------------------------------------------------------------------------
-struct StarAcc {
-    double s1x, s1y;   // S1
-    double s2x, s2h;   // Re S2, (Im S2)/2
-    double s3x, s3y;   // S3
-    double smx, smy;   // sum m/(z-z_i) (caustic map; only with CAUS)
-};
-
-// (root, star): with d = z - z_i, w = 1/d = conj(d)/|d|^2 = (wx, wy)  [dy is taken as y_i - y],
-//   S1 += w,  S2 += m w^2 = m (wx^2 - wy^2, 2 wx wy),  S3 += m w^3 = m (wx (wx^2 - 3 wy^2), wy (3 wx^2 - wy^2)).
-// 22 FP64 instructions + 1 MUFU; 18 of them name at most two distinct register sources.
-template <bool CAUS>
-__device__ __forceinline__ void pair_star(double zx, double zy, double2 s, double m, StarAcc &a)
-{
-    const double dx = zx - s.x;
-    const double dy = s.y - zy;
-    const double r2 = fma(dy, dy, dx * dx);
-    const double inv = rcp_full(r2);
-    const double wx = dx * inv;
-    const double wy = dy * inv;
-    a.s1x += wx;
-    a.s1y += wy;
-    const double ux = m * wx;
-    const double uy = m * wy;
-    if (CAUS) {
-        a.smx += ux;
-        a.smy += uy;
-    }
-    const double A = wx * wx;
-    const double B = wy * wy;
-    const double g = fma(-3.0, B, A);
-    const double h = fma(3.0, A, -B);
-    const double c = A - B;
-    a.s2x = fma(m, c, a.s2x);
-    a.s2h = fma(ux, wy, a.s2h);
-    a.s3x = fma(ux, g, a.s3x);
-    a.s3y = fma(uy, h, a.s3y);
-}
-
 // (root, root) in FP64: A += 1/(z_k - z_r) with the 20-bit reciprocal seed.  Only the convergence
 // RATE depends on A (the fixed point of the update is F = 0 whatever A is).  A root paired with
 // itself has d = 0 exactly: |d|^2 + TINY = 1e-300, the seed is finite, the pair contributes 0.
@@ -361,16 +337,17 @@ struct __align__(128) Stage {
     float4 rp[2 * S_TILE];   // the slot's source entries 2 j0 .. 2 j0 + 2 S_TILE
 };
 
-// One Aberth step for the unfrozen root at position `pos` of the slot's list, from its reduced sums
-//   v[0..1] = Re S2, (Im S2)/2;  v[2..3] = S3;  v[4..5] = 2 S1 - A;  v[6..7] = Sm (CAUS only).
+// One Aberth step for the unfrozen root at position `pos` of the slot's list, from its sums:
+//   t = 2 S1 - A,  S2 = (s2x, 2 s2h),  S3,  Sm (CAUS only).
 template <bool CAUS>
 __device__ __forceinline__ void aberth_step(const Params &p, int slot, long long row, const int *list, int pos,
-                                            const double *v)
+                                            double tx, double ty, double s2x, double s2h, double s3x, double s3y,
+                                            double smx, double smy)
 {
     const int k = list[pos];
     const double2 z = p.roots[row * p.n_r + k];
     const double2 rot = p.rot[row];
-    const double s2x = v[0], s2y = 2.0 * v[1], s3x = v[2], s3y = v[3], tx = v[4], ty = v[5];
+    const double s2y = 2.0 * s2h;
     const double fx_ = p.gamma + s2x - rot.x;   // F
     const double fy_ = s2y - rot.y;
     const double gx = -2.0 * s3x;               // F'
@@ -387,8 +364,8 @@ __device__ __forceinline__ void aberth_step(const Params &p, int slot, long long
         // Sm(z') = Sm + Delta S2 + Delta^2 S3 + O(Delta^3 S4), Sm = sum m_i/(z - z_i);
         // exact to rounding once the root freezes (|Delta| < tol).  Rewritten every iteration.
         const double d2x = d.x * d.x - d.y * d.y, d2y = 2.0 * d.x * d.y;
-        const double mx = v[6] + (d.x * s2x - d.y * s2y) + (d2x * s3x - d2y * s3y);
-        const double my = v[7] + (d.x * s2y + d.y * s2x) + (d2x * s3y + d2y * s3x);
+        const double mx = smx + (d.x * s2x - d.y * s2y) + (d2x * s3x - d2y * s3y);
+        const double my = smy + (d.x * s2y + d.y * s2x) + (d2x * s3y + d2y * s3x);
         const double nx = z.x - d.x, ny = z.y - d.y;
         double2 c;
         c.x = fma(p.omk + p.gamma, nx, -mx);   // (1-kappa_s) x + gamma x - Re Sm
@@ -397,18 +374,78 @@ __device__ __forceinline__ void aberth_step(const Params &p, int slot, long long
     }
 }
 
+// Far-field mode: the star sums of every unfrozen root, one thread per root (near stars directly, distant
+// stars from the node series: star_sums.cuh), written by list position for the compute kernel.
+// grid: (ceil(n_r / BLOCK), max_slots)
+__global__ void __launch_bounds__(BLOCK) k_star_sums(Params p)
+{
+    const DevState st = *p.state;
+    if (st.done) return;
+    const int slot = blockIdx.y;
+    if (slot >= st.n_slots) return;
+    const int n_act = p.n_active[st.cur * MAX_SLOTS + slot];
+    const int pos = blockIdx.x * blockDim.x + threadIdx.x;
+    if (pos >= n_act) return;
+    const int *list = p.list + ((long long)st.cur * p.max_slots + slot) * p.n_r;
+    const double2 z = p.roots[p.slot_row[slot] * p.n_r + list[pos]];
+    StarAcc a = {0, 0, 0, 0, 0, 0, 0, 0};
+    if (!fmm_star_sums(p.fmm, z.x, z.y, a)) {   // no node: queued for k_star_sums_outside
+        p.outside[atomicAdd(&p.state->n_outside, 1)] = make_int2(slot, pos);
+        return;
+    }
+    double2 *o = reinterpret_cast<double2 *>(p.ssum + ((size_t)slot * p.n_r + pos) * 8);
+    o[0] = make_double2(a.s1x, a.s1y);
+    o[1] = make_double2(a.s2x, a.s2h);
+    o[2] = make_double2(a.s3x, a.s3y);
+    o[3] = make_double2(a.smx, a.smy);
+}
+
+// The queued roots, one CTA per root: all stars directly, the CTA's shares added in a fixed tree.
+__global__ void __launch_bounds__(BLOCK) k_star_sums_outside(Params p)
+{
+    __shared__ double s_red[BLOCK / 32][8];
+    const DevState st = *p.state;
+    if (st.done) return;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (int q = blockIdx.x; q < st.n_outside; q += gridDim.x) {
+        const int2 e = p.outside[q];
+        const int *list = p.list + ((long long)st.cur * p.max_slots + e.x) * p.n_r;
+        const double2 z = p.roots[p.slot_row[e.x] * p.n_r + list[e.y]];
+        StarAcc a = {0, 0, 0, 0, 0, 0, 0, 0};
+        for (int i = tid; i < p.N; i += BLOCK) pair_star<true>(z.x, z.y, p.stars[i], p.masses[i], a);
+        double v[8] = {a.s1x, a.s1y, a.s2x, a.s2h, a.s3x, a.s3y, a.smx, a.smy};
+#pragma unroll
+        for (int c = 0; c < 8; ++c)
+            for (int o = 16; o > 0; o >>= 1) v[c] += __shfl_xor_sync(0xffffffffu, v[c], o);
+        __syncthreads();
+        if (lane == 0) {
+#pragma unroll
+            for (int c = 0; c < 8; ++c) s_red[warp][c] = v[c];
+        }
+        __syncthreads();
+        if (tid < 8) {
+            double sum = 0.0;
+            for (int w = 0; w < BLOCK / 32; ++w) sum += s_red[w][tid];
+            p.ssum[((size_t)e.x * p.n_r + e.y) * 8 + tid] = sum;
+        }
+    }
+}
+
 // Thread layout of a tile with T threads per root: G = CTA / T threads share one value of `sub`
 // (the share of the sources they sum: sources sub, sub + T, sub + 2T, ... of every stage) and
 // thread (sub, local) owns the R roots at tile positions local, G + local, ...  For T <= CTA / 32
 // a warp has ONE sub, so every shared-memory read in the pair loop is a warp-wide broadcast: a
 // read costs the same wavefronts whatever T is, and each value read is used for R roots.
-template <int MODE, bool CAUS>
-__global__ void __launch_bounds__(CTA, MLCC_MIN_CTAS) k_compute(Params p)
+// STARS = false (far-field mode): the stages carry root entries only and the star sums are read
+// from p.ssum; the loop body is then two packed FP32 root pairs per root, hence the larger R.
+template <int MODE, bool CAUS, bool STARS, int R>
+__global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Params p)
 {
     __shared__ Stage s_stage[2];
     __shared__ __align__(8) unsigned long long s_full[2];
     __shared__ int s_tile;
-    constexpr int NV = CAUS ? 8 : 6;
+    constexpr int NV = STARS ? (CAUS ? 8 : 6) : 2;
+    constexpr unsigned STAGE_TX = STARS ? STAGE_BYTES : 2 * S_TILE * 16;
     static_assert(sizeof(Stage) * 2 >= (size_t)NV * R * CTA * sizeof(double), "reduction scratch aliases the stages");
 
     const DevState st = *p.state;
@@ -452,9 +489,11 @@ __global__ void __launch_bounds__(CTA, MLCC_MIN_CTAS) k_compute(Params p)
         const float4 *slot_src = p.src + (size_t)slot * n_src;
         if (tid == 0) {   // first stage of this tile
             const unsigned b = g & 1u;
-            mbar_expect_tx(&s_full[b], STAGE_BYTES);
-            tma_load(s_stage[b].sxy, p.stars_pad, S_TILE * 16, &s_full[b]);
-            tma_load(s_stage[b].sm, p.mass_pad, S_TILE * 8, &s_full[b]);
+            mbar_expect_tx(&s_full[b], STAGE_TX);
+            if (STARS) {
+                tma_load(s_stage[b].sxy, p.stars_pad, S_TILE * 16, &s_full[b]);
+                tma_load(s_stage[b].sm, p.mass_pad, S_TILE * 8, &s_full[b]);
+            }
             tma_load(s_stage[b].rp, slot_src, 2 * S_TILE * 16, &s_full[b]);
         }
         const int *list = p.list + ((long long)st.cur * p.max_slots + slot) * p.n_r;
@@ -475,12 +514,12 @@ __global__ void __launch_bounds__(CTA, MLCC_MIN_CTAS) k_compute(Params p)
             split_ds(z.x, zxh[r], zxl[r]);
             split_ds(z.y, zyh[r], zyl[r]);
         }
-        StarAcc acc[R];
+        StarAcc acc[STARS ? R : 1];
         double ax[R], ay[R], bx[R], by[R];   // MODE_F64: two chains
         float2 fx[R], fy[R];                 // MODE_F32: packed lanes
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            acc[r] = StarAcc{0, 0, 0, 0, 0, 0, 0, 0};
+            if (STARS) acc[r] = StarAcc{0, 0, 0, 0, 0, 0, 0, 0};
             ax[r] = ay[r] = bx[r] = by[r] = 0.0;
             fx[r] = fy[r] = make_float2(0.f, 0.f);
         }
@@ -489,9 +528,11 @@ __global__ void __launch_bounds__(CTA, MLCC_MIN_CTAS) k_compute(Params p)
             const unsigned b = g & 1u;
             if (tid == 0 && t + 1 < n_stage) {   // prefetch: buffer b^1 was last read in stage g-1, closed by a barrier
                 const unsigned nb = b ^ 1u;
-                mbar_expect_tx(&s_full[nb], STAGE_BYTES);
-                tma_load(s_stage[nb].sxy, p.stars_pad + (size_t)(t + 1) * S_TILE, S_TILE * 16, &s_full[nb]);
-                tma_load(s_stage[nb].sm, p.mass_pad + (size_t)(t + 1) * S_TILE, S_TILE * 8, &s_full[nb]);
+                mbar_expect_tx(&s_full[nb], STAGE_TX);
+                if (STARS) {
+                    tma_load(s_stage[nb].sxy, p.stars_pad + (size_t)(t + 1) * S_TILE, S_TILE * 16, &s_full[nb]);
+                    tma_load(s_stage[nb].sm, p.mass_pad + (size_t)(t + 1) * S_TILE, S_TILE * 8, &s_full[nb]);
+                }
                 tma_load(s_stage[nb].rp, slot_src + (size_t)(t + 1) * 2 * S_TILE, 2 * S_TILE * 16, &s_full[nb]);
             }
             mbar_wait(&s_full[b], (g >> 1) & 1u);
@@ -503,14 +544,18 @@ __global__ void __launch_bounds__(CTA, MLCC_MIN_CTAS) k_compute(Params p)
 #pragma unroll
                     for (int u = 0; u < 2; ++u) {
                         const int j = sub + (i + u) * T;
-                        const double2 sxy = sg.sxy[j];
-                        const double sm = sg.sm[j];
+                        double2 sxy = make_double2(0.0, 0.0);
+                        double sm = 0.0;
+                        if (STARS) {
+                            sxy = sg.sxy[j];
+                            sm = sg.sm[j];
+                        }
                         if (MODE == MODE_F64) {
                             const double2 *rr = reinterpret_cast<const double2 *>(sg.rp);
                             const double2 ra = rr[2 * j], rb = rr[2 * j + 1];
 #pragma unroll
                             for (int r = 0; r < R; ++r) {
-                                pair_star<CAUS>(zx[r], zy[r], sxy, sm, acc[r]);
+                                if (STARS) pair_star<CAUS>(zx[r], zy[r], sxy, sm, acc[r]);
                                 pair_root_f64(zx[r], zy[r], ra, ax[r], ay[r]);
                                 pair_root_f64(zx[r], zy[r], rb, bx[r], by[r]);
                             }
@@ -518,7 +563,7 @@ __global__ void __launch_bounds__(CTA, MLCC_MIN_CTAS) k_compute(Params p)
                             const float4 h = sg.rp[2 * j], l = sg.rp[2 * j + 1];
 #pragma unroll
                             for (int r = 0; r < R; ++r) {
-                                pair_star<CAUS>(zx[r], zy[r], sxy, sm, acc[r]);
+                                if (STARS) pair_star<CAUS>(zx[r], zy[r], sxy, sm, acc[r]);
                                 pair_root2_f32(make_float2(zxh[r], zxh[r]), make_float2(zyh[r], zyh[r]),
                                                make_float2(zxl[r], zxl[r]), make_float2(zyl[r], zyl[r]), h, l,
                                                fx[r], fy[r]);
@@ -529,7 +574,7 @@ __global__ void __launch_bounds__(CTA, MLCC_MIN_CTAS) k_compute(Params p)
             }
             __syncthreads();   // everyone is done with buffer b before it is refilled
         }
-        // ---- this thread's partial sums ----
+        // ---- this thread's partial sums: v = (2 S1 - A, S2, S3, Sm), or (-A) alone without STARS ----
         double v[R][NV];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
@@ -541,16 +586,33 @@ __global__ void __launch_bounds__(CTA, MLCC_MIN_CTAS) k_compute(Params p)
                 sax = ax[r] + bx[r];
                 say = ay[r] + by[r];
             }
-            v[r][0] = acc[r].s2x; v[r][1] = acc[r].s2h; v[r][2] = acc[r].s3x; v[r][3] = acc[r].s3y;
-            v[r][4] = 2.0 * acc[r].s1x - sax;   // 2 S1 - A
-            v[r][5] = 2.0 * acc[r].s1y - say;
-            if (CAUS) { v[r][NV - 2] = acc[r].smx; v[r][NV - 1] = acc[r].smy; }
+            if (STARS) {
+                v[r][0] = 2.0 * acc[r].s1x - sax;
+                v[r][1] = 2.0 * acc[r].s1y - say;
+                v[r][2] = acc[r].s2x; v[r][3] = acc[r].s2h; v[r][4] = acc[r].s3x; v[r][5] = acc[r].s3y;
+                if (CAUS) { v[r][NV - 2] = acc[r].smx; v[r][NV - 1] = acc[r].smy; }
+            } else {
+                v[r][0] = -sax;
+                v[r][1] = -say;
+            }
         }
+        // the step of the root at list position `pos` from its combined sums w[0..NV)
+        auto finish = [&](int pos, const double *w) {
+            if (STARS) {
+                aberth_step<CAUS>(p, slot, row, list, pos, w[0], w[1], w[2], w[3], w[4], w[5],
+                                  CAUS ? w[NV - 2] : 0.0, CAUS ? w[NV - 1] : 0.0);
+            } else {
+                const double2 *s = reinterpret_cast<const double2 *>(p.ssum + ((size_t)slot * p.n_r + pos) * 8);
+                const double2 s1 = s[0], s2 = s[1], s3 = s[2], smm = s[3];
+                aberth_step<CAUS>(p, slot, row, list, pos, fma(2.0, s1.x, w[0]), fma(2.0, s1.y, w[1]), s2.x, s2.y,
+                                  s3.x, s3.y, smm.x, smm.y);
+            }
+        };
         if (T == 1) {
 #pragma unroll
             for (int r = 0; r < R; ++r) {
                 const int pos = base + r * G + local;
-                if (pos < n_act) aberth_step<CAUS>(p, slot, row, list, pos, v[r]);
+                if (pos < n_act) finish(pos, v[r]);
             }
         } else {
             // combine the T shares through shared memory (the stage buffers are idle: every stage of
@@ -561,15 +623,15 @@ __global__ void __launch_bounds__(CTA, MLCC_MIN_CTAS) k_compute(Params p)
 #pragma unroll
                 for (int q = 0; q < NV; ++q) red[(q * T + sub) * tile_roots + r * G + local] = v[r][q];
             __syncthreads();
-            if (tid < tile_roots && base + tid < n_act) {
+            for (int e = tid; e < tile_roots && base + e < n_act; e += CTA) {   // tile_roots > CTA when T < R
                 double w[NV];
 #pragma unroll
                 for (int q = 0; q < NV; ++q) {
                     double sum = 0.0;
-                    for (int s2 = 0; s2 < T; ++s2) sum += red[(q * T + s2) * tile_roots + tid];
+                    for (int s2 = 0; s2 < T; ++s2) sum += red[(q * T + s2) * tile_roots + e];
                     w[q] = sum;
                 }
-                aberth_step<CAUS>(p, slot, row, list, base + tid, w);
+                finish(base + e, w);
             }
             // order these generic-proxy accesses before the async-proxy (TMA) writes of the next tile
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -680,11 +742,11 @@ __device__ void build_tiles(const Params &p, DevState &st)
     for (int s = 0; s < st.n_slots; ++s) total += n_active[s];
     st.total_active = (int)total;
     int T = 1;
-    while (T < CTA && total * T / (R * CTA) < 2LL * p.grid_ctas) T <<= 1;
+    while (T < CTA && total * T / (p.R * CTA) < 2LL * p.grid_ctas) T <<= 1;
     if (T < p.min_T) T = p.min_T;
     int Tf = T * MLCC_FINE_FACTOR;
     if (Tf > CTA) Tf = CTA;
-    const int tile_c = R * CTA / T, tile_f = R * CTA / Tf;
+    const int tile_c = p.R * CTA / T, tile_f = p.R * CTA / Tf;
     long long W = 0;   // coarse tiles if every slot were cut into coarse tiles only (whole tiles)
     for (int s = 0; s < st.n_slots; ++s) W += n_active[s] / tile_c;
     const long long C = (W / p.grid_ctas) * p.grid_ctas;   // whole rounds
@@ -768,7 +830,7 @@ __global__ void k_init(Params p)
     DevState st;
     st.step = 0; st.iter = 0; st.n_slots = 0; st.done = 0; st.need_seed = 1; st.cur = 0;
     st.T = 1; st.Tf = 1; st.n_coarse = 0; st.n_tiles = 0; st.next_tile = 0; st.total_active = 0; st.total_iterations = 0;
-    st.unconverged_rows = 0; st.degenerate = 0; st.root_iterations = 0; st.launches_used = 0;
+    st.unconverged_rows = 0; st.degenerate = 0; st.n_outside = 0; st.root_iterations = 0; st.launches_used = 0;
     build_slots(p, st);
     build_tiles(p, st);
     *p.state = st;
@@ -785,6 +847,7 @@ __global__ void k_finalize(Params p)
     st.root_iterations += st.total_active;
     st.launches_used += 1;
     st.need_seed = 0;
+    st.n_outside = 0;
     int *cur = p.n_active + st.cur * MAX_SLOTS;
     int *nxt = p.n_active + (st.cur ^ 1) * MAX_SLOTS;
     int remaining = 0;
@@ -818,17 +881,30 @@ struct KernelSet {
     void (*seed)(Params);
     void (*compute)(Params);
     void (*apply)(Params);
+    int R;   // roots per thread of `compute`
 };
 
-KernelSet kernel_set(int mode, bool caus)
+KernelSet kernel_set(int mode, bool caus, bool fmm)
 {
     KernelSet k;
     if (mode == MODE_F64) {
         k.prepare = k_prepare<MODE_F64>; k.seed = k_seed<MODE_F64>; k.apply = k_apply<MODE_F64>;
-        k.compute = caus ? k_compute<MODE_F64, true> : k_compute<MODE_F64, false>;
+        if (fmm) {
+            k.compute = caus ? k_compute<MODE_F64, true, false, R_ROOTS_F64> : k_compute<MODE_F64, false, false, R_ROOTS_F64>;
+            k.R = R_ROOTS_F64;
+        } else {
+            k.compute = caus ? k_compute<MODE_F64, true, true, R_STARS> : k_compute<MODE_F64, false, true, R_STARS>;
+            k.R = R_STARS;
+        }
     } else {
         k.prepare = k_prepare<MODE_F32>; k.seed = k_seed<MODE_F32>; k.apply = k_apply<MODE_F32>;
-        k.compute = caus ? k_compute<MODE_F32, true> : k_compute<MODE_F32, false>;
+        if (fmm) {
+            k.compute = caus ? k_compute<MODE_F32, true, false, R_ROOTS_F32> : k_compute<MODE_F32, false, false, R_ROOTS_F32>;
+            k.R = R_ROOTS_F32;
+        } else {
+            k.compute = caus ? k_compute<MODE_F32, true, true, R_STARS> : k_compute<MODE_F32, false, true, R_STARS>;
+            k.R = R_STARS;
+        }
     }
     return k;
 }
@@ -894,6 +970,8 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     if (opt.aberth_sum_precision != 0 && opt.aberth_sum_precision != 32 && opt.aberth_sum_precision != 64)
         return invalid("aberth_sum_precision must be 0, 32 or 64");
     const int mode = opt.aberth_sum_precision == 64 ? MODE_F64 : MODE_F32;
+    if (opt.star_sum_mode != MLCC_STAR_SUMS_DIRECT && opt.star_sum_mode != MLCC_STAR_SUMS_FMM)
+        return invalid("star_sum_mode");
 
     // phase table (1-kappa_s) e^{-i phi_j}; c(phi_j) = 0 on a row is rejected (degree drop)
     std::vector<double2> rot((size_t)num_phi);
@@ -977,7 +1055,8 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
         }
     }
 
-    const KernelSet ks = kernel_set(mode, out_caustics != nullptr);
+    const bool use_fmm = opt.star_sum_mode == MLCC_STAR_SUMS_FMM;
+    const KernelSet ks = kernel_set(mode, out_caustics != nullptr, use_fmm);
     int blocks_per_sm = 0;
     MLCC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, ks.compute, CTA, 0));
     if (blocks_per_sm < 1) blocks_per_sm = 1;
@@ -997,6 +1076,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     p.order = order;
     p.min_T = min_T;
     p.grid_ctas = grid_compute;
+    p.R = ks.R;
     p.rot = d_rot;
     p.init_roots = reinterpret_cast<const double2 *>(init_roots);
     p.roots = reinterpret_cast<double2 *>(out_roots);
@@ -1020,11 +1100,24 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     h_state[0].done = h_state[1].done = 0;
 
     MLCC_CUDA(cudaEventRecord(ev0, stream));
+    int64_t launches = 3;   // check, prepare, init
+    if (use_fmm) {   // grid + node series of the far field, once per call (inside the timed region)
+        MLCC_CUDA(ws.alloc(&p.ssum, (size_t)max_slots * n_r * 8));
+        MLCC_CUDA(ws.alloc(&p.outside, (size_t)max_slots * n_r));
+        const int frc = fmm_build(p.stars, masses, (int)N, opt.fmm_order, opt.fmm_stars_per_node, ws, &p.fmm, stream);
+        if (frc != MLCC_OK) {
+            cudaEventDestroy(ev0); cudaEventDestroy(ev1);
+            cudaEventDestroy(ev_poll[0]); cudaEventDestroy(ev_poll[1]);
+            cudaFreeHost(h_state);
+            return frc;
+        }
+        launches += 9;
+    }
     const int grid_seed = sms * 4;
     ks.prepare<<<grid_seed, BLOCK, 0, stream>>>(p);
     k_init<<<1, 32, 0, stream>>>(p);
     const int grid_apply = max_slots;
-    int64_t launches = 3;   // check, prepare, init
+    const dim3 grid_star((unsigned)((n_r + BLOCK - 1) / BLOCK), (unsigned)max_slots);
     // Upper bound on iteration groups, so that a device-side fault cannot spin the host forever.
     const long long max_groups = (long long)(max_steps + 1) * (long long)(p.max_iter > p.max_iter_cold ? p.max_iter : p.max_iter_cold) + 8;
     const int chunk = 16;
@@ -1035,11 +1128,15 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     while (!finished && groups < max_groups + 2 * chunk) {
         for (int g = 0; g < chunk; ++g) {
             ks.seed<<<grid_seed, BLOCK, 0, stream>>>(p);
+            if (use_fmm) {
+                k_star_sums<<<grid_star, BLOCK, 0, stream>>>(p);
+                k_star_sums_outside<<<sms, BLOCK, 0, stream>>>(p);
+            }
             ks.compute<<<grid_compute, CTA, 0, stream>>>(p);
             ks.apply<<<grid_apply, APPLY_THREADS, 0, stream>>>(p);
             k_finalize<<<1, 32, 0, stream>>>(p);
         }
-        launches += 4 * chunk;
+        launches += (use_fmm ? 6 : 4) * chunk;
         groups += chunk;
         cudaMemcpyAsync(&h_state[which], p.state, sizeof(DevState), cudaMemcpyDeviceToHost, stream);
         cudaEventRecord(ev_poll[which], stream);

@@ -35,6 +35,8 @@ int critical_curves_impl(const double *, const double *, int64_t, double, double
 int caustics_impl(const double *, const double *, int64_t, double, double, const double *, int64_t, double *,
                   cudaStream_t);
 int star_field_impl(uint64_t, int64_t, double, int, const double *, double *, double *, double *, cudaStream_t);
+int star_sums_impl(const double *, const double *, int64_t, const double *, int64_t, int, int, int, double *,
+                   cudaStream_t);
 int match_root_sets_impl(const double *, const double *, int64_t, int64_t, double, double *, int32_t *,
                          cudaStream_t);
 
@@ -57,6 +59,43 @@ __global__ void __launch_bounds__(256) k_dfma_peak(double *sink, int iters, doub
         }
     }
     const double s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+    if (s == 1.2345e-300) sink[0] = s;  // never true; keeps the chains alive
+}
+
+// Issue-model probes (mlcc_fp64_issue_probe): the same loop shape as k_dfma_peak with other operand forms.
+// FORM 1: DFMA with three distinct register sources.  FORM 2: DADD with two distinct sources.
+// FORM 3: the peak form interleaved 1:1 with packed FP32 FMAs (fma.rn.f32x2, three 64-bit sources): shows
+// that the FP32 instructions draw on the same register-operand bandwidth as the FP64 ones.
+template <int FORM>
+__global__ void __launch_bounds__(256) k_issue_probe(double *sink, int iters, double a)
+{
+    const double t = threadIdx.x * 1e-12;
+    double x[8], y[8], z[8];
+    unsigned long long f[8], gq[8], hq[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+        x[u] = t + u; y[u] = a + (u + 1) * t; z[u] = a * 0.5 + (u + 2) * t;
+        f[u] = (unsigned long long)__double_as_longlong(1.0 + u + t);
+        gq[u] = (unsigned long long)__double_as_longlong(0.5 + t);
+        hq[u] = (unsigned long long)__double_as_longlong(0.25 + u * t);
+    }
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                if (FORM == 1) x[u] = fma(x[u], y[u], z[u]);
+                else if (FORM == 2) x[u] = x[u] + y[u];
+                else {
+                    x[u] = fma(x[u], y[u], x[u]);
+                    asm volatile("fma.rn.ftz.f32x2 %0, %0, %1, %2;" : "+l"(f[u]) : "l"(gq[u]), "l"(hq[u]));
+                }
+            }
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int u = 0; u < 8; ++u) s += x[u] + __longlong_as_double((long long)f[u]);
     if (s == 1.2345e-300) sink[0] = s;  // never true; keeps the chains alive
 }
 
@@ -103,6 +142,10 @@ void mlcc_options_default(mlcc_options *opt)
     opt->phi_index_total = 0;
     opt->min_lanes_per_root = 0;
     opt->aberth_sum_precision = 0;
+    opt->star_sum_mode = MLCC_STAR_SUMS_DIRECT;
+    opt->fmm_order = 0;
+    opt->fmm_stars_per_node = 0;
+    opt->reserved_ = 0;
 }
 
 int mlcc_star_field(uint64_t seed, int64_t N, double kappa_star, int mass_model, const double *mass_params,
@@ -145,6 +188,13 @@ int mlcc_caustics(const double *star_xy, const double *masses, int64_t N, double
 {
     return caustics_impl(star_xy, masses, N, kappa_s, gamma, points, P, out_caustics,
                          static_cast<cudaStream_t>(stream));
+}
+
+int mlcc_star_sums(const double *star_xy, const double *masses, int64_t N, const double *points, int64_t P,
+                   int mode, int fmm_order, int fmm_stars_per_node, double *out_sums, void *stream)
+{
+    return star_sums_impl(star_xy, masses, N, points, P, mode, fmm_order, fmm_stars_per_node, out_sums,
+                          static_cast<cudaStream_t>(stream));
 }
 
 int mlcc_match_root_sets(const double *a, const double *b, int64_t S, int64_t n, double rel_tol,
@@ -221,7 +271,22 @@ int mlcc_caustics_host(const double *star_xy, const double *masses, int64_t N, d
     return MLCC_OK;
 }
 
+static int fp64_probe(int form, double ms_target, double *out_tflops, void *stream_);
+
 int mlcc_fp64_peak(double ms_target, double *out_tflops, void *stream_)
+{
+    return fp64_probe(0, ms_target, out_tflops, stream_);
+}
+
+int mlcc_fp64_issue_probe(int form, double ms_target, double *out_rate, void *stream_)
+{
+    if (form < 0 || form > 3) return invalid("form must be 0..3");
+    return fp64_probe(form, ms_target, out_rate, stream_);
+}
+
+}  // extern "C"
+
+static int fp64_probe(int form, double ms_target, double *out_tflops, void *stream_)
 {
     if (!out_tflops) return invalid("null pointer");
     if (!(ms_target > 0.0) || ms_target > 10000.0) return invalid("ms_target out of range");
@@ -238,7 +303,10 @@ int mlcc_fp64_peak(double ms_target, double *out_tflops, void *stream_)
     double best = 0.0;
     for (int rep = 0; rep < 6; ++rep) {
         cudaEventRecord(e0, stream);
-        k_dfma_peak<<<grid, block, 0, stream>>>(sink, iters, -1e-7);
+        if (form == 0) k_dfma_peak<<<grid, block, 0, stream>>>(sink, iters, -1e-7);
+        else if (form == 1) k_issue_probe<1><<<grid, block, 0, stream>>>(sink, iters, -1e-7);
+        else if (form == 2) k_issue_probe<2><<<grid, block, 0, stream>>>(sink, iters, -1e-7);
+        else k_issue_probe<3><<<grid, block, 0, stream>>>(sink, iters, -1e-7);
         cudaEventRecord(e1, stream);
         cudaError_t es = cudaEventSynchronize(e1);
         if (es != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); return cuda_fail(es, "peak probe", __FILE__, __LINE__); }
@@ -259,5 +327,3 @@ int mlcc_fp64_peak(double ms_target, double *out_tflops, void *stream_)
     *out_tflops = best;
     return MLCC_OK;
 }
-
-}  // extern "C"

@@ -28,7 +28,7 @@ inline int invalid(const char *msg)
 // Stream-ordered workspace that frees itself (cudaFreeAsync) when it goes out of scope.
 struct Workspace {
     cudaStream_t stream;
-    void *ptrs[32];
+    void *ptrs[48];
     int n = 0;
     explicit Workspace(cudaStream_t s) : stream(s) {}
     ~Workspace()
@@ -41,7 +41,7 @@ struct Workspace {
         void *p = nullptr;
         cudaError_t e = cudaMallocAsync(&p, count * sizeof(T) > 0 ? count * sizeof(T) : 16, stream);
         if (e != cudaSuccess) return e;
-        if (n < 32) ptrs[n++] = p;
+        if (n < 48) ptrs[n++] = p;
         *out = static_cast<T *>(p);
         return cudaSuccess;
     }

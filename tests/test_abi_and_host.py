@@ -44,7 +44,7 @@ def test_version_and_status_strings(lib):
 def test_options_default_and_struct_layout(lib):
     from paper_2506_02121_b200 import api
     o = api.options()
-    assert o.struct_size == C.sizeof(api.mlcc_options) == 40
+    assert o.struct_size == C.sizeof(api.mlcc_options) == 56
     assert o.predictor_order == -1 and o.num_subchains == 0 and o.phi_index_total == 0
     assert C.sizeof(api.mlcc_stats) == 64
 
@@ -109,6 +109,13 @@ def test_invalid_arguments_fail_before_any_cuda_call(lib):
     assert L.mlcc_star_field(0, 5, -1.0, 0, None, one, one, None, None) == api.MLCC_ERR_INVALID_ARG
     assert L.mlcc_star_field(0, 5, 0.4, 7, None, one, one, None, None) == api.MLCC_ERR_INVALID_ARG
     assert L.mlcc_fp64_peak(50.0, None, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_star_sums(None, one, 3, one, 5, 0, 0, 0, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_star_sums(one, one, 3, one, 5, 2, 0, 0, one, None) == api.MLCC_ERR_INVALID_ARG   # unknown mode
+    assert L.mlcc_star_sums(one, one, 3, one, -1, 0, 0, 0, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_star_sums(one, one, 3, None, 0, 1, 0, 0, None, None) == api.MLCC_OK              # P = 0
+    o = api.mlcc_options()
+    L.mlcc_options_default(C.byref(o))
+    assert o.struct_size == C.sizeof(api.mlcc_options) and o.star_sum_mode == api.MLCC_STAR_SUMS_DIRECT
 
 
 def test_product_does_not_import_the_oracle():

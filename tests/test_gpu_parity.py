@@ -380,3 +380,106 @@ def test_host_buffer_entry_points(api, orc):
 def test_fp64_peak_probe_is_plausible(api):
     tf = api.fp64_peak(20.0)
     assert 5.0 < tf < 80.0, tf
+
+
+# ---------------------------------------------------------------------------------------------
+# far-field split of the star sums (Section 4.1)
+# ---------------------------------------------------------------------------------------------
+def _points_for_star_sums(xy, R, n, seed):
+    """Points shaped like critical points: most within ~1 Einstein radius of a star, some anywhere in the field,
+    a few outside the stars' bounding square (the outer root pair) and on the grid's edge."""
+    rng = np.random.default_rng(seed)
+    near = xy[rng.integers(0, len(xy), n)] + rng.normal(size=(n, 2)) * 0.7
+    anywhere = rng.uniform(-R, R, size=(n // 2, 2))
+    outside = rng.normal(size=(16, 2))
+    outside = outside / np.linalg.norm(outside, axis=1, keepdims=True) * R * rng.uniform(1.5, 3.0, size=(16, 1))
+    corner = np.array([[xy[:, 0].min(), xy[:, 1].min()], [xy[:, 0].max(), xy[:, 1].max()],
+                       [xy[:, 0].max() + 1e-9, 0.0], [0.0, xy[:, 1].min() - 1e-9]])
+    return np.concatenate([near, anywhere, outside, corner])
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3", "cfg4"])
+def test_star_sums_direct_and_fmm_against_oracle(api, orc, name):
+    """mlcc_star_sums in both modes against the oracle's long-double straight sums.  Tolerance: the sums are
+    N terms of size ~ m/d^k accumulated in FP64, so 1e-12 relative to sum |term| is ~100 ulp-sums; the split's
+    truncation (rho^32 = 3e-18) must not show at that level."""
+    cfg = CONFIGS[name]
+    xy, m, R = field(orc, cfg)
+    pts = _points_for_star_sums(xy, R, 600, cfg.N)
+    ref = orc.star_sums(xy, m, pts, long_double=True)
+    z = pts[:, 0] + 1j * pts[:, 1]
+    d = np.abs(z[:, None] - (xy[:, 0] + 1j * xy[:, 1])[None, :])
+    scale = np.stack([(1 / d).sum(1), (m / d ** 2).sum(1), (m / d ** 3).sum(1), (m / d).sum(1)], axis=1)
+    scale = np.repeat(scale, 2, axis=1)
+    for mode in (api.MLCC_STAR_SUMS_DIRECT, api.MLCC_STAR_SUMS_FMM):
+        got = api.star_sums(dev(xy), dev(m), dev(pts), mode=mode).cpu().numpy()
+        assert np.isfinite(got).all()
+        assert (np.abs(got - ref) / scale).max() < 1e-12, (mode, (np.abs(got - ref) / scale).max())
+
+
+def test_fmm_truncation_follows_the_geometric_bound(api, orc):
+    """Order p leaves an error below C rho^(p+1), rho = (1/sqrt 2)/2.5 = 0.283: each
+    8 more terms must gain ~4 decimal digits until FP64 rounding is reached.  Also other node sizes."""
+    cfg = CONFIGS["cfg3"]
+    xy, m, R = field(orc, cfg)
+    pts = _points_for_star_sums(xy, R, 400, 5)[:600]          # inside points only matter here
+    ref = orc.star_sums(xy, m, pts, long_double=True)
+    errs = {}
+    for order in (7, 15, 23, 31):
+        got = api.star_sums(dev(xy), dev(m), dev(pts), mode=api.MLCC_STAR_SUMS_FMM, fmm_order=order).cpu().numpy()
+        errs[order] = np.abs(got[:, 2:4] - ref[:, 2:4]).max()   # S2: the sum that carries F
+    rho = (0.5 ** 0.5) / 2.5
+    total = float((m[None, :] / 1.0).sum())                     # crude constant: sum m_i / s^2 with s >= 1
+    for order, e in errs.items():
+        assert e < max(total * (order + 1) * rho ** (order + 1), 1e-11), (order, e)
+    assert errs[15] < 1e-3 * errs[7] and (errs[23] < 1e-2 * errs[15] or errs[23] < 1e-11)
+    assert errs[31] < 1e-11
+    for spn in (1, 2, 16, 64, 100000):
+        got = api.star_sums(dev(xy), dev(m), dev(pts), mode=api.MLCC_STAR_SUMS_FMM, fmm_stars_per_node=spn).cpu().numpy()
+        assert np.abs(got - ref).max() < 1e-9 * (1 + np.abs(ref).max())
+
+
+@pytest.mark.parametrize("name,num_phi", [("cfg1", 1000), ("cfg2", 4000), ("cfg3", 64)])
+def test_fmm_mode_gives_the_same_root_sets_and_caustics(api, orc, name, num_phi):
+    cfg = CONFIGS[name]
+    xy, m, R = field(orc, cfg)
+    rows = np.arange(num_phi) if cfg.N <= 200 else np.array([0, 1, num_phi // 2, num_phi - 1])
+    ref, _, un = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, num_phi, rows, cfg.tol, cfg.max_iter)
+    assert un.sum() == 0
+    w_ref = orc.caustics(xy, m, cfg.kappa_s, cfg.gamma, ref)
+    for prec in (32, 64):
+        opt = api.options(star_sum_mode=api.MLCC_STAR_SUMS_FMM, aberth_sum_precision=prec)
+        roots, caus, iters, unconv, st = api.curves_and_caustics(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, num_phi,
+                                                                 cfg.tol, cfg.max_iter, opt=opt)
+        assert int(unconv.sum()) == 0 and st.degenerate_roots == 0
+        g, w = roots.cpu().numpy(), caus.cpu().numpy()
+        assert_rows_match(orc, g[rows], ref)
+        for i, j in enumerate(rows[::max(1, len(rows) // 50)]):
+            ii = i * max(1, len(rows) // 50)
+            assert_caustics_match(g[j], w[j], ref[ii], w_ref[ii])
+        # against the direct mode of the same library: far inside the parity tolerance
+        plain, _, _, _ = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, num_phi, cfg.tol,
+                                                cfg.max_iter, opt=api.options(aberth_sum_precision=prec))
+        err, bij = api.match_root_sets(roots, plain, 1e-12)
+        assert bool(bij.all())
+        # reproducible
+        r2, _, _, _, _ = api.curves_and_caustics(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, num_phi, cfg.tol,
+                                                 cfg.max_iter, opt=opt)
+        assert torch.equal(r2, roots)
+
+
+def test_fmm_mode_full_size_cfg4_sampled_rows(api, orc):
+    cfg = CONFIGS["cfg4"]
+    xy, m, R = field(orc, cfg)
+    num_phi = 512
+    opt = api.options(star_sum_mode=api.MLCC_STAR_SUMS_FMM)
+    roots, iters, unconv, st = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, num_phi, cfg.tol,
+                                                      cfg.max_iter, opt=opt)
+    assert int(unconv.sum()) == 0 and st.degenerate_roots == 0
+    e1, e2 = vieta_all_rows(roots, xy, m, cfg.kappa_s, cfg.gamma, num_phi)
+    assert e1 < 1e-12 and e2 < 1e-12, (e1, e2)
+    for j in (0, 255):
+        ref, _, un = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, num_phi, [j], cfg.tol, cfg.max_iter)
+        assert un.sum() == 0
+        assert_rows_match(orc, roots[j:j + 1].cpu().numpy(), ref)
+    check_row_invariants(orc, xy, m, cfg.kappa_s, cfg.gamma, 100, num_phi, cplx(roots[100].cpu().numpy()))

@@ -390,3 +390,45 @@ def test_star_field_mass_functions(orc):
     # explicit parameters == defaults
     xy2, m2, _ = orc.star_field(0, N, 0.2, 2, p)
     assert np.array_equal(m, m2) and np.array_equal(xy, xy2)
+
+
+def test_star_sums_regular_polygon_closed_form(orc):
+    """K equal stars of mass m on the circle |z| = a at the K-th roots of a^K (textbook partial fractions):
+    sum_j 1/(z - a w^j) = K z^(K-1)/(z^K - a^K) =: g(z), so S1 = g, Sm = m g, S2 = -m g', S3 = m g''/2.
+    Pins every sum the oracle's star loop forms (power, sign, mass factor), also for points inside the ring."""
+    K, a, mass = 7, 1.7, 0.6
+    zs = a * np.exp(2j * np.pi * np.arange(K) / K)
+    xy = np.stack([zs.real, zs.imag], axis=1)
+    m = np.full(K, mass)
+    pts = np.array([[0.3, -0.2], [2.5, 1.1], [-4.0, 0.7], [0.0, 3.3], [1.0, 1.0]])
+    z = pts[:, 0] + 1j * pts[:, 1]
+    q = z ** K - a ** K
+    g = K * z ** (K - 1) / q
+    g1 = K * (K - 1) * z ** (K - 2) / q - (K * z ** (K - 1)) ** 2 / q ** 2
+    g2 = (K * (K - 1) * (K - 2) * z ** (K - 3) / q - 3 * K * (K - 1) * z ** (K - 2) * K * z ** (K - 1) / q ** 2
+          + 2 * (K * z ** (K - 1)) ** 3 / q ** 3)
+    for ld in (False, True):
+        out = orc.star_sums(xy, m, pts, long_double=ld)
+        S1, S2, S3, Sm = (out[:, 0] + 1j * out[:, 1], out[:, 2] + 1j * out[:, 3], out[:, 4] + 1j * out[:, 5],
+                          out[:, 6] + 1j * out[:, 7])
+        assert np.abs(S1 - g).max() < 1e-13
+        assert np.abs(Sm - mass * g).max() < 1e-13
+        assert np.abs(S2 + mass * g1).max() < 1e-12
+        assert np.abs(S3 - mass * g2 / 2).max() < 1e-12
+
+
+def test_star_sums_consistent_with_residuals_and_caustics(orc):
+    """F = gamma + S2 - (1-kappa_s) e^{-i phi}, F' = -2 S3 (Eq. 15, 19) and w = (1-kappa_s) z + gamma conj z - conj Sm
+    (Eq. 12): the exported sums are the ones the solver and the caustic map use."""
+    xy, m, R = orc.star_field(3, 300, 0.3, 2)
+    pts = np.random.default_rng(0).normal(size=(50, 2)) * R * 0.6
+    ks, g = 0.15, 0.35
+    out = orc.star_sums(xy, m, pts)
+    res = orc.residuals(xy, m, ks, g, 7, 64, pts)
+    phi = 2 * np.pi * 7 / 64
+    F = g + (out[:, 2] + 1j * out[:, 3]) - (1 - ks) * np.exp(-1j * phi)
+    assert np.abs(F - res["F"]).max() < 1e-13 * (1 + np.abs(F).max())
+    assert np.abs(-2 * (out[:, 4] + 1j * out[:, 5]) - res["Fp"]).max() < 1e-13 * (1 + np.abs(res["Fp"]).max())
+    w = cplx(orc.caustics(xy, m, ks, g, pts, long_double=True))
+    z = pts[:, 0] + 1j * pts[:, 1]
+    assert np.abs((1 - ks) * z + g * np.conj(z) - np.conj(out[:, 6] + 1j * out[:, 7]) - w).max() < 1e-12
