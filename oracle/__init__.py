@@ -36,6 +36,9 @@ def lib():
         for f in (L.orc_star_sums, L.orc_star_sums_ld):
             f.argtypes = [_pd, _pd, C.c_int64, _pd, C.c_int64, _pd]
         L.orc_match_root_sets.argtypes = [_pd, _pd, C.c_int64, C.c_int64, C.c_double, _pd, _pi32]
+        L.orc_link_rows.argtypes = [_pd, C.c_int64, C.c_int64, _pi32, _pi32]
+        L.orc_crossing_map.argtypes = [_pd, C.c_void_p, C.c_int64, C.c_int64, C.c_double, C.c_double, C.c_double,
+                                       C.c_int32, C.c_int32, _pi32, C.c_void_p]
         L.orc_star_field.argtypes = [C.c_uint64, C.c_int64, C.c_double, C.c_int, C.c_void_p,
                                      _pd, _pd, C.POINTER(C.c_double)]
         L.orc_philox4x32_10.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32),
@@ -156,3 +159,29 @@ def match_root_sets(a, b, rel_tol):
     bij = np.empty(S, np.int32)
     _check(lib().orc_match_root_sets(a, b, S, n, float(rel_tol), err, bij), "match_root_sets")
     return err, bij
+
+
+def link_rows(rows):
+    """rows [S,n,2] -> (next [S,n] int32: column of row (s+1) % S that continues column i of row s, bijective [S])."""
+    rows = np.ascontiguousarray(rows, _d)
+    S, n, _ = rows.shape
+    nxt = np.empty((S, n), np.int32)
+    bij = np.empty(S, np.int32)
+    _check(lib().orc_link_rows(rows, S, n, nxt, bij), "link_rows")
+    return nxt, bij
+
+
+def crossing_map(caustics, nxt, x0, y0, pixel, nx, ny, want_ambiguous=False):
+    """caustics [S,n,2], nxt [S,n] int32 or None -> number of caustic crossings per pixel [ny,nx] int32
+    (and, if asked, the uint8 mask of pixels whose centre is within rounding of a segment)."""
+    caustics = np.ascontiguousarray(caustics, _d)
+    S, n, _ = caustics.shape
+    out = np.empty((ny, nx), np.int32)
+    amb = np.zeros((ny, nx), np.uint8) if want_ambiguous else None
+    if nxt is not None:
+        nxt = np.ascontiguousarray(nxt, np.int32)
+        assert nxt.shape == (S, n)
+    _check(lib().orc_crossing_map(caustics, None if nxt is None else nxt.ctypes.data, S, n, float(x0), float(y0),
+                                  float(pixel), int(nx), int(ny), out, None if amb is None else amb.ctypes.data),
+           "crossing_map")
+    return (out, amb) if want_ambiguous else out

@@ -217,6 +217,100 @@ int orc_match_root_sets(const double *a, const double *b, int64_t S, int64_t n, 
 }
 
 /* ------------------------------------------------------------------------------------------
+ * Chain joining (fn. 5 at :217): "the start of one chain is the end of another, with
+ * chains joining together until closed loops are formed".  Row s of `rows` holds the n roots of
+ * phase s in any column order; out_next[s][i] is the column of row (s+1) mod S whose root is nearest
+ * to root i of row s (brute force over all columns; the first index wins a tie).  Roots move
+ * continuously with phi, so for a fine enough grid that root continues the chain.
+ *   out_bijective[s] = 1 iff i -> out_next[s][i] is a bijection (every chain has one successor).
+ * ---------------------------------------------------------------------------------------- */
+int orc_link_rows(const double *rows, int64_t S, int64_t n, int32_t *out_next, int32_t *out_bijective)
+{
+    if (S < 1 || n < 1) return -2;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t s = 0; s < S; ++s) {
+        const double *as = rows + 2 * s * n, *bs = rows + 2 * ((s + 1) % S) * n;
+        int32_t *hits = (int32_t *)calloc((size_t)n, sizeof(int32_t));
+        int ok = 1;
+        for (int64_t i = 0; i < n; ++i) {
+            double best = INFINITY;
+            int64_t bj = -1;
+            for (int64_t j = 0; j < n; ++j) {
+                double dx = as[2 * i] - bs[2 * j], dy = as[2 * i + 1] - bs[2 * j + 1];
+                double d2 = dx * dx + dy * dy;
+                if (d2 < best) { best = d2; bj = j; }
+            }
+            out_next[s * n + i] = (int32_t)bj;
+            if (bj < 0) ok = 0; else hits[bj] += 1;
+        }
+        for (int64_t j = 0; j < n; ++j) if (hits[j] != 1) ok = 0;
+        out_bijective[s] = ok;
+        free(hits);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Number of caustic crossings per source pixel (Section 5.1): "Since the caustics
+ * are oriented curves, winding numbers provide the number of caustic crossings.  For every
+ * (pixelized) source location, we use ... Sunday's (2001) algorithm to calculate the winding number
+ * of the discretized caustic polygons around that point".  The polygons are the chains of caustic
+ * points joined by `next` (NULL = column i continues in column i), closed from row S-1 back to
+ * row 0.  The caustics are traced clockwise, so the count is MINUS the usual
+ * counter-clockwise winding number (reading R21).
+ * Written as the definition: for each pixel centre, a loop over every segment with Sunday's
+ * crossing rule (an upward edge with the point strictly on its left adds one, a downward edge
+ * with the point strictly on its right subtracts one).  Pixel (ix, iy) has its centre at
+ * (x0 + (ix + 1/2) pixel, y0 + (iy + 1/2) pixel); out_map is [ny][nx] row-major.
+ * out_ambiguous (may be NULL), [ny][nx]: 1 where the centre lies within 1e-9 pixel of a segment it
+ * could cross, so that rounding may decide the count there.
+ * ---------------------------------------------------------------------------------------- */
+int orc_crossing_map(const double *caustics, const int32_t *next, int64_t S, int64_t n,
+                     double x0, double y0, double pixel, int32_t nx, int32_t ny,
+                     int32_t *out_map, uint8_t *out_ambiguous)
+{
+    if (S < 1 || n < 1 || nx < 1 || ny < 1 || !(pixel > 0.0)) return -2;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t pix = 0; pix < (int64_t)nx * ny; ++pix) {
+        const int64_t iy = pix / nx, ix = pix % nx;
+        const long double px = (long double)x0 + ((long double)ix + 0.5L) * (long double)pixel;
+        const long double py = (long double)y0 + ((long double)iy + 0.5L) * (long double)pixel;
+        int32_t wn = 0;
+        int amb = 0;
+        for (int64_t s = 0; s < S; ++s) {
+            const double *a = caustics + 2 * s * n, *b = caustics + 2 * ((s + 1) % S) * n;
+            for (int64_t i = 0; i < n; ++i) {
+                const int64_t j = next ? next[s * n + i] : i;
+                if (j < 0) continue;
+                const long double ax = a[2 * i], ay = a[2 * i + 1], bx = b[2 * j], by = b[2 * j + 1];
+                if (!(ax == ax && ay == ay && bx == bx && by == by)) continue;   /* NaN point: no segment */
+                /* isLeft > 0: (px,py) left of the directed line a -> b */
+                const long double is_left = (bx - ax) * (py - ay) - (px - ax) * (by - ay);
+                if (ay <= py) {
+                    if (by > py && is_left > 0) ++wn;          /* upward crossing, point on the left  */
+                } else {
+                    if (by <= py && is_left < 0) --wn;         /* downward crossing, point on the right */
+                }
+                if (out_ambiguous) {
+                    const long double lo = ay < by ? ay : by, hi = ay < by ? by : ay;
+                    const long double len = sqrtl((bx - ax) * (bx - ax) + (by - ay) * (by - ay));
+                    const long double eps = 1e-9L * (long double)pixel;
+                    if (py >= lo - eps && py <= hi + eps && fabsl(is_left) <= eps * (len + eps)) amb = 1;
+                    if (fabsl(py - ay) <= eps || fabsl(py - by) <= eps) {
+                        /* the ray grazes an end point: which of the two segments there counts is a
+                           rounding decision if the point is also to the left of it */
+                        amb = amb || (px <= (ax > bx ? ax : bx) + eps);
+                    }
+                }
+            }
+        }
+        out_map[pix] = -wn;
+        if (out_ambiguous) out_ambiguous[pix] = (uint8_t)amb;
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
  * Star-field generator (recipe in DESIGN.md "Input recipe").
  * Counter-based Philox4x32-10 (Salmon, Moraes, Dror & Shaw 2011, "Parallel random numbers:
  * as easy as 1, 2, 3"), restated from the published algorithm.
