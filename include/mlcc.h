@@ -203,6 +203,35 @@ int mlcc_star_sums(const double *star_xy, const double *masses, int64_t N, const
 int mlcc_match_root_sets(const double *a, const double *b, int64_t S, int64_t n, double rel_tol,
                          double *out_max_err, int32_t *out_bijective, void *stream);
 
+/* (f) NEXT-4, as far as the crossing map needs it: chain joining (fn. 5 at :217: "the
+ * start of one chain is the end of another, with chains joining together until closed loops are
+ * formed").  Row s of `rows` holds n points in any column order (the root sets of consecutive
+ * phases: out_roots of the calls above, whose column order changes between sub-chains and at the
+ * wrap from the last row to row 0).  out_next[s][i] is the column of row (s+1) mod S holding the
+ * point nearest to point i of row s: roots move continuously with phi, so on a fine
+ * enough grid that point continues the chain.  Ties go to the lowest column.
+ *   rows [S][n][2]: device, read.  out_next [S][n]: device int32, written (-1 in a row with a
+ *   non-finite value).  out_bijective [S]: device int32, 1 iff i -> out_next[s][i] is a bijection.
+ * Asynchronous on `stream`.  Errors: INVALID_ARG, CUDA, NOMEM.                                    */
+int mlcc_link_rows(const double *rows, int64_t S, int64_t n, int32_t *out_next,
+                   int32_t *out_bijective, void *stream);
+
+/* (f) NEXT-2: number of caustic crossings per source pixel (Section 5.1): the
+ * winding number, by Sunday's crossing rule, of the oriented polygons whose vertices are the
+ * caustic points of consecutive phases: segment (s, i) runs from caustics[s][i] to
+ * caustics[s+1][next[s][i]] (next = NULL: column i continues in column i); with closed != 0 the
+ * last row joins row 0.  The caustics are traced clockwise as phi increases, so the
+ * count is MINUS the counter-clockwise winding number: 1 inside a simple caustic, 0 far away.
+ * Pixel (ix, iy) has its centre at (x0 + (ix + 1/2) pixel, y0 + (iy + 1/2) pixel).
+ *   caustics [S][n][2]: device, read (out_caustics of the calls above).  next [S][n]: device int32
+ *   or NULL (mlcc_link_rows of the ROOTS: the caustic points cross one another, the roots do not).
+ *   out_map [ny][nx]: device int32, written.  Segments with a non-finite end are skipped.
+ * A pixel whose centre lies on a segment to rounding may get either neighbour's count.
+ * Asynchronous on `stream`.  Errors: INVALID_ARG, CUDA, NOMEM.                                    */
+int mlcc_crossing_map(const double *caustics, const int32_t *next, int64_t S, int64_t n, int closed,
+                      double x0, double y0, double pixel, int32_t nx, int32_t ny, int32_t *out_map,
+                      void *stream);
+
 /* Host-only planning helper of the phase-continuation driver: splits rows
  * [0, num_phi) into `num_subchains` contiguous sub-chains and returns, per sub-chain c, its
  * first row, its centre row (cold-started) and one past its last row.  num_subchains = 0 asks

@@ -93,6 +93,8 @@ def lib() -> C.CDLL:
                                                C.POINTER(mlcc_stats), vp]
         L.mlcc_caustics.argtypes = [vp, vp, i64, dbl, dbl, vp, i64, vp, vp]
         L.mlcc_match_root_sets.argtypes = [vp, vp, i64, i64, dbl, vp, vp, vp]
+        L.mlcc_link_rows.argtypes = [vp, i64, i64, vp, vp, vp]
+        L.mlcc_crossing_map.argtypes = [vp, vp, i64, i64, C.c_int, dbl, dbl, dbl, i32, i32, vp, vp]
         L.mlcc_star_sums.argtypes = [vp, vp, i64, vp, i64, C.c_int, C.c_int, C.c_int, vp, vp]
         L.mlcc_plan_subchains.argtypes = [i64, i64, i32, i32, vp, vp, vp]
         L.mlcc_critical_curves_host.argtypes = [vp, vp, i64, dbl, dbl, i64, dbl, i32, vp]
@@ -246,6 +248,35 @@ def caustics(star_xy, masses, kappa_s, gamma, points, out=None):
     rc = lib().mlcc_caustics(_dev(star_xy, name="star_xy"), _dev(masses, name="masses"), N,
                              float(kappa_s), float(gamma), _dev(points, name="points"), P,
                              _dev(out, name="out"), _stream())
+    if rc != MLCC_OK:
+        _raise(rc)
+    return out
+
+
+def link_rows(rows):
+    """mlcc_link_rows: rows [S,n,2] -> (next [S,n] i32, bijective [S] i32)."""
+    if rows.dim() != 3 or rows.shape[2] != 2:
+        raise ValueError("rows must be [S, n, 2]")
+    S, n, _ = rows.shape
+    nxt = torch.empty((S, n), dtype=torch.int32, device=rows.device)
+    bij = torch.empty((S,), dtype=torch.int32, device=rows.device)
+    rc = lib().mlcc_link_rows(_dev(rows, name="rows"), S, n, nxt.data_ptr(), bij.data_ptr(), _stream())
+    if rc != MLCC_OK:
+        _raise(rc)
+    return nxt, bij
+
+
+def crossing_map(caustics, nxt, x0, y0, pixel, nx, ny, closed=True):
+    """mlcc_crossing_map: caustics [S,n,2], nxt [S,n] i32 or None -> number of caustic crossings [ny,nx] i32."""
+    if caustics.dim() != 3 or caustics.shape[2] != 2:
+        raise ValueError("caustics must be [S, n, 2]")
+    S, n, _ = caustics.shape
+    if nxt is not None and tuple(nxt.shape) != (S, n):
+        raise ValueError("nxt must be [S, n]")
+    out = torch.empty((ny, nx), dtype=torch.int32, device=caustics.device)
+    rc = lib().mlcc_crossing_map(_dev(caustics, name="caustics"), _dev(nxt, torch.int32, "nxt"), S, n,
+                                 1 if closed else 0, float(x0), float(y0), float(pixel), int(nx), int(ny),
+                                 out.data_ptr(), _stream())
     if rc != MLCC_OK:
         _raise(rc)
     return out

@@ -35,6 +35,9 @@ int critical_curves_impl(const double *, const double *, int64_t, double, double
 int caustics_impl(const double *, const double *, int64_t, double, double, const double *, int64_t, double *,
                   cudaStream_t);
 int star_field_impl(uint64_t, int64_t, double, int, const double *, double *, double *, double *, cudaStream_t);
+int link_rows_impl(const double *, int64_t, int64_t, int32_t *, int32_t *, cudaStream_t);
+int crossing_map_impl(const double *, const int32_t *, int64_t, int64_t, int, double, double, double, int32_t,
+                      int32_t, int32_t *, cudaStream_t);
 int star_sums_impl(const double *, const double *, int64_t, const double *, int64_t, int, int, int, double *,
                    cudaStream_t);
 int match_root_sets_impl(const double *, const double *, int64_t, int64_t, double, double *, int32_t *,
@@ -188,6 +191,19 @@ int mlcc_caustics(const double *star_xy, const double *masses, int64_t N, double
 {
     return caustics_impl(star_xy, masses, N, kappa_s, gamma, points, P, out_caustics,
                          static_cast<cudaStream_t>(stream));
+}
+
+int mlcc_link_rows(const double *rows, int64_t S, int64_t n, int32_t *out_next, int32_t *out_bijective,
+                   void *stream)
+{
+    return link_rows_impl(rows, S, n, out_next, out_bijective, static_cast<cudaStream_t>(stream));
+}
+
+int mlcc_crossing_map(const double *caustics, const int32_t *next, int64_t S, int64_t n, int closed, double x0,
+                      double y0, double pixel, int32_t nx, int32_t ny, int32_t *out_map, void *stream)
+{
+    return crossing_map_impl(caustics, next, S, n, closed, x0, y0, pixel, nx, ny, out_map,
+                             static_cast<cudaStream_t>(stream));
 }
 
 int mlcc_star_sums(const double *star_xy, const double *masses, int64_t N, const double *points, int64_t P,

@@ -40,7 +40,8 @@ __device__ __forceinline__ int cell_coord(double v, double lo, double inv_h, int
 __global__ void __launch_bounds__(BLOCK) k_match(const double2 *__restrict__ a, const double2 *__restrict__ b,
                                                  long long S, int n, double rel_tol, int G,
                                                  int *scratch, long long scratch_stride,
-                                                 double *out_max_err, int *out_bijective)
+                                                 double *out_max_err, int *out_bijective,
+                                                 long long b_shift, int *out_index)
 {
     __shared__ double s_buf[BLOCK];
     __shared__ int s_scan[BLOCK];
@@ -53,7 +54,8 @@ __global__ void __launch_bounds__(BLOCK) k_match(const double2 *__restrict__ a, 
     int *hits = sorted + n;                                              // [n]
 
     for (long long s = blockIdx.x; s < S; s += gridDim.x) {
-        const double2 *as = a + s * n, *bs = b + s * n;
+        // b_shift = 0: set s of a against set s of b.  b_shift = 1 (chain joining): row s against row (s+1) mod S
+        const double2 *as = a + s * n, *bs = b + ((s + b_shift) % S) * n;
         // ---- bounding box of b, finiteness of a and b ----
         double xmin = 1e308, xmax = -1e308, ymin = 1e308, ymax = -1e308, bad = 0.0;
         for (int j = tid; j < n; j += BLOCK) {
@@ -66,7 +68,8 @@ __global__ void __launch_bounds__(BLOCK) k_match(const double2 *__restrict__ a, 
         ymin = block_reduce(ymin, false, s_buf); ymax = block_reduce(ymax, true, s_buf);
         bad = block_reduce(bad, true, s_buf);
         if (bad > 0.0) {
-            if (tid == 0) { out_max_err[s] = INFINITY; out_bijective[s] = 0; }
+            if (tid == 0) { if (out_max_err) out_max_err[s] = INFINITY; out_bijective[s] = 0; }
+            if (out_index) for (int i = tid; i < n; i += BLOCK) out_index[s * n + i] = -1;
             continue;
         }
         const double wx = xmax - xmin, wy = ymax - ymin;
@@ -149,6 +152,7 @@ __global__ void __launch_bounds__(BLOCK) k_match(const double2 *__restrict__ a, 
                 }
             }
             max_d2 = fmax(max_d2, best);
+            if (out_index) out_index[s * n + i] = bj;
             if (bj >= 0) {
                 atomicAdd(&hits[bj], 1);
                 const double2 q = bs[bj];
@@ -165,12 +169,16 @@ __global__ void __launch_bounds__(BLOCK) k_match(const double2 *__restrict__ a, 
         __syncthreads();
         for (int j = tid; j < n; j += BLOCK) if (hits[j] != 1) s_flag = 0;
         __syncthreads();
-        if (tid == 0) { out_max_err[s] = sqrt(max_d2); out_bijective[s] = s_flag; }
+        if (tid == 0) { if (out_max_err) out_max_err[s] = sqrt(max_d2); out_bijective[s] = s_flag; }
         __syncthreads();
     }
 }
 
 }  // namespace
+
+static int match_launch(const double *a, const double *b, int64_t S, int64_t n, double rel_tol,
+                        double *out_max_err, int32_t *out_bijective, long long b_shift, int32_t *out_index,
+                        cudaStream_t stream);
 
 int match_root_sets_impl(const double *a, const double *b, int64_t S, int64_t n, double rel_tol,
                          double *out_max_err, int32_t *out_bijective, cudaStream_t stream)
@@ -180,6 +188,25 @@ int match_root_sets_impl(const double *a, const double *b, int64_t S, int64_t n,
     if (!(rel_tol >= 0.0)) return invalid("rel_tol must be >= 0");
     if (S == 0) return MLCC_OK;
     if (!a || !b || !out_max_err || !out_bijective) return invalid("null pointer");
+    return match_launch(a, b, S, n, rel_tol, out_max_err, out_bijective, 0, nullptr, stream);
+}
+
+// Chain joining (fn. 5 at :217): the successor of every root of row s in row (s+1) mod S.
+int link_rows_impl(const double *rows, int64_t S, int64_t n, int32_t *out_next, int32_t *out_bijective,
+                   cudaStream_t stream)
+{
+    if (S < 0) return invalid("S < 0");
+    if (n < 1 || n > (1 << 30)) return invalid("n out of range");
+    if (S == 0) return MLCC_OK;
+    if (!rows || !out_next || !out_bijective) return invalid("null pointer");
+    // no distance limit: the flag says only whether every chain has exactly one successor
+    return match_launch(rows, rows, S, n, 1.79769313486231570e308, nullptr, out_bijective, 1, out_next, stream);
+}
+
+static int match_launch(const double *a, const double *b, int64_t S, int64_t n, double rel_tol,
+                        double *out_max_err, int32_t *out_bijective, long long b_shift, int32_t *out_index,
+                        cudaStream_t stream)
+{
     int G = (int)ceil(sqrt((double)n));
     if (G < 1) G = 1;
     if (G > 2048) G = 2048;
@@ -199,7 +226,7 @@ int match_root_sets_impl(const double *a, const double *b, int64_t S, int64_t n,
     MLCC_CUDA(e);
     k_match<<<(int)grid, BLOCK, 0, stream>>>(reinterpret_cast<const double2 *>(a),
                                             reinterpret_cast<const double2 *>(b), (long long)S, (int)n,
-                                            rel_tol, G, scratch, stride, out_max_err, out_bijective);
+                                            rel_tol, G, scratch, stride, out_max_err, out_bijective, b_shift, out_index);
     MLCC_CUDA(cudaGetLastError());
     return MLCC_OK;
 }

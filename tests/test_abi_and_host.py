@@ -113,6 +113,13 @@ def test_invalid_arguments_fail_before_any_cuda_call(lib):
     assert L.mlcc_star_sums(one, one, 3, one, 5, 2, 0, 0, one, None) == api.MLCC_ERR_INVALID_ARG   # unknown mode
     assert L.mlcc_star_sums(one, one, 3, one, -1, 0, 0, 0, one, None) == api.MLCC_ERR_INVALID_ARG
     assert L.mlcc_star_sums(one, one, 3, None, 0, 1, 0, 0, None, None) == api.MLCC_OK              # P = 0
+    assert L.mlcc_link_rows(None, 3, 5, one, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_link_rows(one, 3, 0, one, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_link_rows(None, 0, 5, None, None, None) == api.MLCC_OK                           # S = 0
+    assert L.mlcc_crossing_map(None, None, 3, 5, 1, 0.0, 0.0, 0.1, 8, 8, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_crossing_map(one, None, 3, 5, 1, 0.0, 0.0, 0.0, 8, 8, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_crossing_map(one, None, 3, 5, 1, 0.0, 0.0, 0.1, 0, 8, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_crossing_map(one, None, 0, 5, 1, 0.0, 0.0, 0.1, 8, 8, one, None) == api.MLCC_ERR_INVALID_ARG
     o = api.mlcc_options()
     L.mlcc_options_default(C.byref(o))
     assert o.struct_size == C.sizeof(api.mlcc_options) and o.star_sum_mode == api.MLCC_STAR_SUMS_DIRECT

@@ -483,3 +483,85 @@ def test_fmm_mode_full_size_cfg4_sampled_rows(api, orc):
         assert un.sum() == 0
         assert_rows_match(orc, roots[j:j + 1].cpu().numpy(), ref)
     check_row_invariants(orc, xy, m, cfg.kappa_s, cfg.gamma, 100, num_phi, cplx(roots[100].cpu().numpy()))
+
+
+# ---------------------------------------------------------------------------------------------
+# chain joining and the caustic-crossing map
+# ---------------------------------------------------------------------------------------------
+def _map_window(caus, n_pix, margin=0.05):
+    lo, hi = caus.reshape(-1, 2).min(0), caus.reshape(-1, 2).max(0)
+    side = float((hi - lo).max()) * (1 + 2 * margin)
+    c = 0.5 * (lo + hi)
+    return float(c[0] - side / 2), float(c[1] - side / 2), side / n_pix
+
+
+@pytest.mark.parametrize("name,num_phi,n_pix", [("cfg1", 1000, 257), ("cfg2", 600, 96)])
+def test_link_rows_and_crossing_map_against_oracle(api, orc, name, num_phi, n_pix):
+    """GPU roots and caustics -> GPU joining -> GPU map, against the oracle's joining and its per-pixel winding
+    numbers of the same points.  Integer outputs: exact, except pixels whose centre the oracle flags as lying on a
+    segment to rounding (either neighbour's count is right there)."""
+    cfg = CONFIGS[name]
+    xy, m, R = field(orc, cfg)
+    roots, caus, iters, unconv, st = api.curves_and_caustics(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, num_phi,
+                                                             cfg.tol, cfg.max_iter)
+    assert st.subchains > 1                       # the column order really changes between rows
+    nxt, bij = api.link_rows(roots)
+    g_roots, g_caus = roots.cpu().numpy(), caus.cpu().numpy()
+    o_nxt, o_bij = orc.link_rows(g_roots)
+    assert o_bij.all() and bool(bij.all())
+    assert np.array_equal(nxt.cpu().numpy(), o_nxt)
+    assert (o_nxt != np.arange(o_nxt.shape[1])[None, :]).any()
+    x0, y0, pixel = _map_window(g_caus, n_pix)
+    got = api.crossing_map(caus, nxt, x0, y0, pixel, n_pix, n_pix).cpu().numpy()
+    ref, amb = orc.crossing_map(g_caus, o_nxt, x0, y0, pixel, n_pix, n_pix, want_ambiguous=True)
+    assert amb.mean() < 0.01
+    assert np.array_equal(got[amb == 0], ref[amb == 0])
+    assert ref.min() >= 0 and ref.max() >= 2 and ref[0, 0] == 0      # crossings are counted, never negative
+    # a window that cuts the caustics, non-square, off-centre
+    got2 = api.crossing_map(caus, nxt, x0 + 0.31 * n_pix * pixel, y0 + 0.4 * n_pix * pixel, pixel * 0.37, 75, 41).cpu().numpy()
+    ref2, amb2 = orc.crossing_map(g_caus, o_nxt, x0 + 0.31 * n_pix * pixel, y0 + 0.4 * n_pix * pixel, pixel * 0.37,
+                                  75, 41, want_ambiguous=True)
+    assert np.array_equal(got2[amb2 == 0], ref2[amb2 == 0])
+    # reproducible to the bit
+    assert np.array_equal(api.crossing_map(caus, nxt, x0, y0, pixel, n_pix, n_pix).cpu().numpy(), got)
+
+
+def test_crossing_map_on_oracle_points_and_open_chains(api, orc):
+    """Same points on both sides (oracle roots/caustics uploaded): identity columns, then an open set of rows."""
+    cfg = CONFIGS["cfg1"]
+    xy, m, R = field(orc, cfg)
+    num_phi = 360
+    roots, _, _ = orc.critical_curves(xy, m, cfg.kappa_s, cfg.gamma, num_phi)
+    caus = orc.caustics(xy, m, cfg.kappa_s, cfg.gamma, roots)
+    o_nxt, o_bij = orc.link_rows(roots)
+    assert o_bij.all()
+    nxt, bij = api.link_rows(dev(roots))
+    assert np.array_equal(nxt.cpu().numpy(), o_nxt) and bool(bij.all())
+    x0, y0, pixel = _map_window(caus, 128)
+    ref, amb = orc.crossing_map(caus, o_nxt, x0, y0, pixel, 128, 128, want_ambiguous=True)
+    got = api.crossing_map(dev(caus), nxt, x0, y0, pixel, 128, 128).cpu().numpy()
+    assert np.array_equal(got[amb == 0], ref[amb == 0])
+    # the oracle's rows are one chain per column except at the wrap: next = None is wrong only there
+    got_id = api.crossing_map(dev(caus), None, x0, y0, pixel, 128, 128).cpu().numpy()
+    ref_id = orc.crossing_map(caus, None, x0, y0, pixel, 128, 128)
+    assert (got_id != ref_id).mean() < 0.01
+    # open chains (closed = 0): with row 0 appended as an extra last row the open polygons are the closed ones
+    ext = np.concatenate([caus, caus[:1]])
+    ext_nxt = np.concatenate([o_nxt, np.arange(o_nxt.shape[1], dtype=np.int32)[None, :]])
+    open_map = api.crossing_map(dev(ext), dev(ext_nxt, torch.int32), x0, y0, pixel, 128, 128, closed=False).cpu().numpy()
+    assert np.array_equal(open_map, got)
+
+def test_link_rows_edge_cases(api, orc):
+    rng = np.random.default_rng(8)
+    for S, n in ((1, 1), (1, 7), (2, 1), (5, 300), (3, 2500)):
+        rows = rng.normal(size=(S, n, 2)) * 20
+        nxt, bij = api.link_rows(dev(rows))
+        o_nxt, o_bij = orc.link_rows(rows)
+        assert np.array_equal(nxt.cpu().numpy(), o_nxt) and bij.cpu().numpy().tolist() == o_bij.tolist()
+    rows[1, 3, 0] = np.nan
+    nxt, bij = api.link_rows(dev(rows))
+    b = bij.cpu().numpy()
+    assert b[1] == 0 and b[0] == 0 and (nxt.cpu().numpy()[1] == -1).all()     # rows 0 -> 1 and 1 -> 2 involve the NaN row
+    empty = torch.empty((0, 4, 2), dtype=torch.float64, device="cuda")
+    n0, b0 = api.link_rows(empty)
+    assert n0.shape == (0, 4) and b0.shape == (0,)
