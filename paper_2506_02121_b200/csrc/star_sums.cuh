@@ -77,8 +77,9 @@ __device__ __forceinline__ void horner3(const double2 *__restrict__ a, int n, do
                                         double2 &p0, double2 &p1, double2 &p2)
 {
     double b0x = 0, b0y = 0, b1x = 0, b1y = 0, b2x = 0, b2y = 0;
+#pragma unroll 8
     for (int l = n - 1; l >= 0; --l) {
-        const double2 c = a[l];
+        const double2 c = __ldg(&a[l]);
         double tx = fma(b2x, ux, fma(-b2y, uy, b1x));   // b2 = b2 u + b1
         double ty = fma(b2x, uy, fma(b2y, ux, b1y));
         b2x = tx; b2y = ty;
@@ -96,8 +97,9 @@ __device__ __forceinline__ void horner3(const double2 *__restrict__ a, int n, do
 __device__ __forceinline__ double2 horner1(const double2 *__restrict__ a, int n, double ux, double uy)
 {
     double bx = 0, by = 0;
+#pragma unroll 8
     for (int l = n - 1; l >= 0; --l) {
-        const double2 c = a[l];
+        const double2 c = __ldg(&a[l]);
         const double tx = fma(bx, ux, fma(-by, uy, c.x));
         const double ty = fma(bx, uy, fma(by, ux, c.y));
         bx = tx; by = ty;
@@ -118,9 +120,25 @@ __device__ __forceinline__ bool fmm_star_sums(const FmmGrid &g, double zx, doubl
     if (!inside) return false;
     const int ix = (int)fx, iy = (int)fy;
     const int xa = max(ix - g.h, 0), xb = min(ix + g.h, g.G - 1);
+    // The near stars of one node row are one contiguous range of the sorted arrays.  Four stars are loaded
+    // before any is used (a star past the range is replaced by a massless one far away), so a thread that
+    // runs alone -- the last unfrozen roots of a row -- waits for memory once per four pairs, not per pair.
     for (int cy = max(iy - g.h, 0); cy <= min(iy + g.h, g.G - 1); ++cy) {
-        const int i0 = g.cell_start[cy * g.G + xa], i1 = g.cell_start[cy * g.G + xb + 1];
-        for (int i = i0; i < i1; ++i) pair_star<true>(zx, zy, g.sxy[i], g.sm[i], a);
+        const int i0 = __ldg(&g.cell_start[cy * g.G + xa]), i1 = __ldg(&g.cell_start[cy * g.G + xb + 1]);
+        for (int i = i0; i < i1; i += 4) {
+            double2 s[4];
+            double m[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const bool in = i + u < i1;
+                const int q = in ? i + u : i;
+                s[u] = __ldg(&g.sxy[q]);
+                m[u] = in ? __ldg(&g.sm[q]) : 0.0;
+                if (!in) s[u] = make_double2(1e150, 1e150);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) pair_star<true>(zx, zy, s[u], m[u], a);
+        }
     }
     const double ux = fx - ((double)ix + 0.5), uy = fy - ((double)iy + 0.5);   // (z - c)/s
     const size_t node = (size_t)(iy * g.G + ix) * g.P1;
