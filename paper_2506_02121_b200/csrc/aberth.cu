@@ -725,9 +725,41 @@ __global__ void __launch_bounds__(APPLY_THREADS) k_apply(Params p)
 }
 
 // ------------------------------------------------------------------------------------------------
-// finalize kernel (one thread): advances the state machine
+// state machine (k_init, k_finalize): one CTA of FIN threads, thread s looks after slot s
+// (MAX_SLOTS = FIN), sums and prefix sums over the slots by block-wide scans
 // ------------------------------------------------------------------------------------------------
-// One thread: the tile table of the next compute launch for the counts in n_active[cur].
+constexpr int FIN = MAX_SLOTS;
+
+// exclusive prefix sum of v over the CTA's threads; *total = the sum (the same value in every thread)
+__device__ __forceinline__ long long block_scan(long long v, long long *total, long long *s_buf /*[33]*/)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    long long incl = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const long long t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    __syncthreads();   // s_buf may still be read from the previous call
+    if (lane == 31) s_buf[warp] = incl;
+    __syncthreads();
+    if (warp == 0) {
+        const long long w = s_buf[lane];
+        long long wi = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const long long t = __shfl_up_sync(0xffffffffu, wi, o);
+            if (lane >= o) wi += t;
+        }
+        s_buf[lane] = wi - w;
+        if (lane == 31) s_buf[32] = wi;
+    }
+    __syncthreads();
+    *total = s_buf[32];
+    return s_buf[warp] + incl - v;
+}
+
+// The tile table of the next compute launch for the counts in n_active[cur].
 // All grid_ctas CTAs are resident and pull tiles from one atomic counter, and tiles of one kind take the
 // same time, so a launch lasts ceil(tiles / grid_ctas) tile-times: with a handful of tiles per CTA
 // the last, partial round costs up to a whole round.  Hence two kinds of tile:
@@ -735,11 +767,13 @@ __global__ void __launch_bounds__(APPLY_THREADS) k_apply(Params p)
 //           least two rounds; only WHOLE rounds of them are handed out;
 //   fine:   Tf = MLCC_FINE_FACTOR T threads per root for what is left of every slot's list, so the
 //           partial round is quantised in units of 1 / MLCC_FINE_FACTOR of a coarse tile.
-__device__ void build_tiles(const Params &p, DevState &st)
+// Every thread returns with the same st.
+__device__ void build_tiles(const Params &p, DevState &st, long long *s_buf)
 {
-    const int *n_active = p.n_active + st.cur * MAX_SLOTS;
-    long long total = 0;
-    for (int s = 0; s < st.n_slots; ++s) total += n_active[s];
+    const int s = threadIdx.x;
+    const int n_act = s < st.n_slots ? p.n_active[st.cur * MAX_SLOTS + s] : 0;
+    long long total, W, tc_total, tf_total;
+    block_scan(n_act, &total, s_buf);
     st.total_active = (int)total;
     int T = 1;
     while (T < CTA && total * T / (p.R * CTA) < 2LL * p.grid_ctas) T <<= 1;
@@ -747,55 +781,61 @@ __device__ void build_tiles(const Params &p, DevState &st)
     int Tf = T * MLCC_FINE_FACTOR;
     if (Tf > CTA) Tf = CTA;
     const int tile_c = p.R * CTA / T, tile_f = p.R * CTA / Tf;
-    long long W = 0;   // coarse tiles if every slot were cut into coarse tiles only (whole tiles)
-    for (int s = 0; s < st.n_slots; ++s) W += n_active[s] / tile_c;
+    block_scan(n_act / tile_c, &W, s_buf);   // coarse tiles if every slot were cut into coarse tiles only
     const long long C = (W / p.grid_ctas) * p.grid_ctas;   // whole rounds
+    const int c_s = (W > 0 && Tf != T) ? (int)((long long)(n_act / tile_c) * C / W) : 0;
+    const int f_s = (n_act - c_s * tile_c + tile_f - 1) / tile_f;
+    const long long tc = block_scan(c_s, &tc_total, s_buf);
+    const long long tf = block_scan(f_s, &tf_total, s_buf);
     int *tab_c = p.tile_start, *tab_f = p.tile_start + MAX_SLOTS + 1;
-    int tc = 0, tf = 0;
-    for (int s = 0; s < st.n_slots; ++s) {
-        const int c_s = (W > 0 && Tf != T) ? (int)((long long)(n_active[s] / tile_c) * C / W) : 0;
-        tab_c[s] = tc;
-        tc += c_s;
+    if (s < st.n_slots) {
+        tab_c[s] = (int)tc;
+        tab_f[s] = (int)tf;
         p.coarse_roots[s] = c_s * tile_c;
-        tab_f[s] = tf;
-        tf += (n_active[s] - c_s * tile_c + tile_f - 1) / tile_f;
     }
-    tab_c[st.n_slots] = tc;
-    tab_f[st.n_slots] = tf;
+    if (s == 0) {
+        tab_c[st.n_slots] = (int)tc_total;
+        tab_f[st.n_slots] = (int)tf_total;
+    }
     st.T = T;
     st.Tf = Tf;
-    st.n_coarse = tc;
-    st.n_tiles = tc + tf;
+    st.n_coarse = (int)tc_total;
+    st.n_tiles = (int)(tc_total + tf_total);
     st.next_tile = 0;
 }
 
-// one thread: slots of step st.step
-__device__ void build_slots(const Params &p, DevState &st)
+// The slots of step st.step: thread c looks after sub-chain c (n_sub <= MAX_SLOTS / 2); the slots keep the
+// order (sub-chain, downward before upward).  Every thread returns with the same st.
+__device__ void build_slots(const Params &p, DevState &st, long long *s_buf)
 {
-    int n = 0;
-    if (st.step == 0) {
-        for (int c = 0; c < p.n_sub; ++c) {
-            p.slot_row[n] = p.sub_centre[c];
-            p.slot_sub[n] = c;
-            p.slot_dir[n] = 0;
-            ++n;
-        }
-    } else {
-        for (int c = 0; c < p.n_sub; ++c) {
-            const long long up = p.sub_centre[c] + st.step, dn = p.sub_centre[c] - st.step;
-            if (dn >= p.sub_first[c]) { p.slot_row[n] = dn; p.slot_sub[n] = c; p.slot_dir[n] = -1; ++n; }
-            if (up < p.sub_end[c])    { p.slot_row[n] = up; p.slot_sub[n] = c; p.slot_dir[n] = +1; ++n; }
+    const int c = threadIdx.x;
+    int has_dn = 0, has_up = 0;
+    long long row_dn = 0, row_up = 0;
+    if (c < p.n_sub) {
+        if (st.step == 0) {
+            has_dn = 1;                      // the centre row, direction 0
+            row_dn = p.sub_centre[c];
+        } else {
+            row_up = p.sub_centre[c] + st.step;
+            row_dn = p.sub_centre[c] - st.step;
+            has_dn = row_dn >= p.sub_first[c];
+            has_up = row_up < p.sub_end[c];
         }
     }
-    st.n_slots = n;
-    for (int s = 0; s < n; ++s) {
-        p.n_active[st.cur * MAX_SLOTS + s] = p.n_r;
-        p.n_active[(st.cur ^ 1) * MAX_SLOTS + s] = 0;
-        p.slot_iters[s] = 0;
+    long long n;
+    int at = (int)block_scan(has_dn + has_up, &n, s_buf);
+    if (has_dn) { p.slot_row[at] = row_dn; p.slot_sub[at] = c; p.slot_dir[at] = st.step == 0 ? 0 : -1; ++at; }
+    if (has_up) { p.slot_row[at] = row_up; p.slot_sub[at] = c; p.slot_dir[at] = +1; }
+    st.n_slots = (int)n;
+    if (threadIdx.x < st.n_slots) {
+        p.n_active[st.cur * MAX_SLOTS + threadIdx.x] = p.n_r;
+        p.n_active[(st.cur ^ 1) * MAX_SLOTS + threadIdx.x] = 0;
+        p.slot_iters[threadIdx.x] = 0;
     }
     st.iter = 0;
     st.need_seed = 1;
     if (n == 0) st.done = 1;
+    __syncthreads();   // the counts are read back by build_tiles
 }
 
 // input check: flags[0] = non-finite star coordinates / masses, flags[1] = pairs of coincident stars
@@ -824,23 +864,24 @@ __global__ void k_check_stars(const double2 *__restrict__ stars, const double *_
     if (same) atomicAdd(&flags[1], same);
 }
 
-__global__ void k_init(Params p)
+__global__ void __launch_bounds__(FIN) k_init(Params p)
 {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    __shared__ long long s_buf[33];
     DevState st;
     st.step = 0; st.iter = 0; st.n_slots = 0; st.done = 0; st.need_seed = 1; st.cur = 0;
     st.T = 1; st.Tf = 1; st.n_coarse = 0; st.n_tiles = 0; st.next_tile = 0; st.total_active = 0; st.total_iterations = 0;
     st.unconverged_rows = 0; st.degenerate = 0; st.n_outside = 0; st.root_iterations = 0; st.launches_used = 0;
-    build_slots(p, st);
-    build_tiles(p, st);
-    *p.state = st;
+    build_slots(p, st, s_buf);
+    build_tiles(p, st, s_buf);
+    if (threadIdx.x == 0) *p.state = st;
 }
 
-__global__ void k_finalize(Params p)
+__global__ void __launch_bounds__(FIN) k_finalize(Params p)
 {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    DevState st = *p.state;
+    __shared__ long long s_buf[33];
+    DevState st = *p.state;   // every thread carries the same copy and makes the same decisions
     if (st.done) return;
+    const int s = threadIdx.x;
     // the iteration that just ran
     st.iter += 1;
     st.total_iterations += 1;
@@ -848,31 +889,32 @@ __global__ void k_finalize(Params p)
     st.launches_used += 1;
     st.need_seed = 0;
     st.n_outside = 0;
-    int *cur = p.n_active + st.cur * MAX_SLOTS;
-    int *nxt = p.n_active + (st.cur ^ 1) * MAX_SLOTS;
-    int remaining = 0;
-    for (int s = 0; s < st.n_slots; ++s) {
-        if (cur[s] > 0) p.slot_iters[s] = st.iter;
-        remaining += nxt[s];
-        cur[s] = 0;   // becomes the "next" counter of the following iteration
+    int left = 0;
+    if (s < st.n_slots) {
+        if (p.n_active[st.cur * MAX_SLOTS + s] > 0) p.slot_iters[s] = st.iter;
+        left = p.n_active[(st.cur ^ 1) * MAX_SLOTS + s];
     }
+    long long remaining;
+    block_scan(left, &remaining, s_buf);
     st.cur ^= 1;
     const int cap = (st.step == 0) ? p.max_iter_cold : p.max_iter;
     if (remaining == 0 || st.iter >= cap) {
         // step finished: per-row diagnostics, then the next step's slots
-        for (int s = 0; s < st.n_slots; ++s) {
+        if (s < st.n_slots) {
             const long long row = p.slot_row[s];
-            const int left = p.n_active[st.cur * MAX_SLOTS + s];
             if (p.out_iters) p.out_iters[row] = p.slot_iters[s];
             if (p.out_unconverged) p.out_unconverged[row] = left;
-            if (left > 0) st.unconverged_rows += 1;
         }
+        long long unconverged;
+        block_scan(left > 0 ? 1 : 0, &unconverged, s_buf);
+        st.unconverged_rows += (int)unconverged;
         st.step += 1;
         if (st.step > p.max_steps) { st.done = 1; st.n_slots = 0; }
-        else build_slots(p, st);
+        else build_slots(p, st, s_buf);
     }
-    if (!st.done) build_tiles(p, st);
-    *p.state = st;
+    if (!st.done) build_tiles(p, st, s_buf);
+    __syncthreads();   // every thread has read *p.state
+    if (s == 0) *p.state = st;
 }
 
 // the kernels of one Aberth-sum mode / caustic fusion choice
@@ -1115,7 +1157,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     }
     const int grid_seed = sms * 4;
     ks.prepare<<<grid_seed, BLOCK, 0, stream>>>(p);
-    k_init<<<1, 32, 0, stream>>>(p);
+    k_init<<<1, FIN, 0, stream>>>(p);
     const int grid_apply = max_slots;
     const dim3 grid_star((unsigned)((n_r + BLOCK - 1) / BLOCK), (unsigned)max_slots);
     // Upper bound on iteration groups, so that a device-side fault cannot spin the host forever.
@@ -1134,7 +1176,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
             }
             ks.compute<<<grid_compute, CTA, 0, stream>>>(p);
             ks.apply<<<grid_apply, APPLY_THREADS, 0, stream>>>(p);
-            k_finalize<<<1, 32, 0, stream>>>(p);
+            k_finalize<<<1, FIN, 0, stream>>>(p);
         }
         launches += (use_fmm ? 6 : 4) * chunk;
         groups += chunk;
