@@ -36,6 +36,14 @@ def lib():
         for f in (L.orc_star_sums, L.orc_star_sums_ld):
             f.argtypes = [_pd, _pd, C.c_int64, _pd, C.c_int64, _pd]
         L.orc_match_root_sets.argtypes = [_pd, _pd, C.c_int64, C.c_int64, C.c_double, _pd, _pi32]
+        L.orc_rect_sheet.argtypes = [C.c_double, C.c_double, C.c_double, C.c_int, _pd, C.c_int64, C.c_void_p,
+                                     C.c_void_p, C.c_void_p]
+        L.orc_rect_truncation.argtypes = [C.c_double, C.c_double, C.c_double, C.c_double, C.c_double]
+        L.orc_rect_critical_curve_rows.argtypes = [_pd, _pd, C.c_int64, C.c_double, C.c_double, C.c_double, C.c_double,
+                                                   C.c_double, C.c_int, C.c_double, C.c_int64, _pi64, C.c_int64,
+                                                   C.c_double, C.c_int, C.c_void_p, _pd, _pi32, _pi32]
+        L.orc_rect_caustics.argtypes = [_pd, _pd, C.c_int64, C.c_double, C.c_double, C.c_double, C.c_double,
+                                        C.c_double, C.c_int, _pd, C.c_int64, _pd]
         L.orc_link_rows.argtypes = [_pd, C.c_int64, C.c_int64, _pi32, _pi32]
         L.orc_crossing_map.argtypes = [_pd, C.c_void_p, C.c_int64, C.c_int64, C.c_double, C.c_double, C.c_double,
                                        C.c_int32, C.c_int32, _pi32, C.c_void_p]
@@ -185,3 +193,50 @@ def crossing_map(caustics, nxt, x0, y0, pixel, nx, ny, want_ambiguous=False):
                                   float(pixel), int(nx), int(ny), out, None if amb is None else amb.ctypes.data),
            "crossing_map")
     return (out, amb) if want_ambiguous else out
+
+
+def rect_sheet(kappa_star, c1, c2, t, points):
+    """Eq. B2, B7, B9 as printed -> (alpha_s, d alpha_s/d zbar, d2 alpha_s/d zbar2) as complex arrays."""
+    flat = np.ascontiguousarray(points, _d).reshape(-1, 2)
+    a, b, d = (np.empty_like(flat) for _ in range(3))
+    _check(lib().orc_rect_sheet(float(kappa_star), float(c1), float(c2), int(t), flat, flat.shape[0],
+                                a.ctypes.data, b.ctypes.data, d.ctypes.data), "rect_sheet")
+    return a[:, 0] + 1j * a[:, 1], b[:, 0] + 1j * b[:, 1], d[:, 0] + 1j * d[:, 1]
+
+
+def rect_truncation(kappa_star, c1, c2, s=1.5, eps=1e-9):
+    t = lib().orc_rect_truncation(float(kappa_star), float(c1), float(c2), float(s), float(eps))
+    if t < 0:
+        raise RuntimeError("oracle rect_truncation failed")
+    return t
+
+
+def rect_critical_curve_rows(star_xy, masses, kappa_s, gamma, kappa_star, c1, c2, t, seed_radius, num_phi_total,
+                             rows, tol=1e-12, max_iter=50, init_roots=None):
+    """-> (roots [len(rows), 2N + t - 1, 2], iters, unconverged) for the rectangular sheet."""
+    xy, m, N = _stars(star_xy, masses)
+    rows = np.ascontiguousarray(rows, np.int64)
+    n_r = 2 * N + t - 1
+    out = np.empty((len(rows), n_r, 2), _d)
+    it = np.empty(len(rows), np.int32)
+    un = np.empty(len(rows), np.int32)
+    init = None
+    if init_roots is not None:
+        init = np.ascontiguousarray(init_roots, _d)
+        assert init.shape == (n_r, 2)
+    _check(lib().orc_rect_critical_curve_rows(xy, m, N, float(kappa_s), float(gamma), float(kappa_star), float(c1),
+                                              float(c2), int(t), float(seed_radius), int(num_phi_total), rows,
+                                              len(rows), float(tol), int(max_iter),
+                                              None if init is None else init.ctypes.data, out, it, un),
+           "rect_critical_curve_rows")
+    return out, it, un
+
+
+def rect_caustics(star_xy, masses, kappa_s, gamma, kappa_star, c1, c2, t, points):
+    xy, m, N = _stars(star_xy, masses)
+    pts = np.ascontiguousarray(points, _d)
+    flat = pts.reshape(-1, 2)
+    out = np.empty_like(flat)
+    _check(lib().orc_rect_caustics(xy, m, N, float(kappa_s), float(gamma), float(kappa_star), float(c1), float(c2),
+                                   int(t), flat, flat.shape[0], out), "rect_caustics")
+    return out.reshape(pts.shape)

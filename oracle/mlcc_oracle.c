@@ -217,6 +217,211 @@ int orc_match_root_sets(const double *a, const double *b, int64_t S, int64_t n, 
 }
 
 /* ------------------------------------------------------------------------------------------
+ * Rectangular field of microlenses (Section 4.2, Appendix A at :386-401 and
+ * Appendix B at :405-457).  The smooth term alpha_s(z) of a rectangular sheet with corner
+ * c = c1 + i c2, its logarithms Taylor-expanded about the origin and truncated at power t
+ * (Eq. B1-B2), the finite sheet extended to an infinite one.  Written as printed,
+ * with the four corners c, conj c, -c, -conj c, their signs +,-,+,-, and principal logarithms:
+ *   B2: alpha_s = -kappa_star i/pi [ sum_k sg_k (c_k - zb)(log c_k - sum_{j=1}^t (zb/c_k)^j / j) ]
+ *                 - kappa_star (c + conj c + zb + z),                                 zb = conj z
+ *   B7: d alpha_s/d zb = -kappa_star i/pi [ zb^t (1+(-1)^t)(1/c^t - 1/cb^t)
+ *                 + sum_{j=1}^t zb^j (1+(-1)^j)(1/c^j - 1/cb^j)/j ] + kappa_star - 4 kappa_star atan(c2/c1)/pi
+ *   B9: d2 alpha_s/d zb2 = -kappa_star i/(pi zb) [ t (zb/c)^t (1+(-1)^t)(1 - e^{2 i t Arg c})
+ *                 + sum_{j=1}^t (zb/c)^j (1+(-1)^j)(1 - e^{2 i j Arg c}) ]
+ *   B6: d alpha_s/d z = -kappa_star.
+ * Then Eq. 15: F = gamma + S2 - conj(d alpha_s/d zb) - (1 - kappa - d alpha_s/d z) e^{-i phi},
+ * F' = -2 S3 - conj(d2 alpha_s/d zb2), and Eq. 12: w = (1-kappa) z + gamma zb - conj(Sm) - alpha_s.
+ * With t odd the polynomial has 2N + t - 1 roots.  double complex only.
+ * ---------------------------------------------------------------------------------------- */
+typedef double complex dcx;
+#ifndef M_PI
+#define M_PI 3.14159265358979323846264338327950288
+#endif
+
+static dcx rect_alpha_B2(double kappa_star, dcx c, int t, dcx z)
+{
+    const dcx zb = conj(z);
+    const dcx corner[4] = {c, conj(c), -c, -conj(c)};
+    const double sg[4] = {1.0, -1.0, 1.0, -1.0};
+    dcx sum = 0;
+    for (int k = 0; k < 4; ++k) {
+        dcx series = 0, q = 1;
+        for (int j = 1; j <= t; ++j) {
+            q *= zb / corner[k];
+            series += q / (double)j;
+        }
+        sum += sg[k] * (corner[k] - zb) * (clog(corner[k]) - series);
+    }
+    return -kappa_star * I / M_PI * sum - kappa_star * (c + conj(c) + zb + z);
+}
+
+static dcx rect_dalpha_dzbar_B7(double kappa_star, dcx c, int t, dcx z)
+{
+    const dcx zb = conj(z), cb = conj(c);
+    const double sign_t = (t % 2 == 0) ? 2.0 : 0.0;   /* 1 + (-1)^t */
+    dcx sum = cpow(zb, t) * sign_t * (1.0 / cpow(c, t) - 1.0 / cpow(cb, t));
+    dcx zp = 1, cp = 1, cbp = 1;
+    for (int j = 1; j <= t; ++j) {
+        zp *= zb; cp *= c; cbp *= cb;
+        const double sign_j = (j % 2 == 0) ? 2.0 : 0.0;
+        sum += zp * sign_j * (1.0 / cp - 1.0 / cbp) / (double)j;
+    }
+    return -kappa_star * I / M_PI * sum + kappa_star - 4.0 * kappa_star * atan(cimag(c) / creal(c)) / M_PI;
+}
+
+static dcx rect_d2alpha_dzbar2_B9(double kappa_star, dcx c, int t, dcx z)
+{
+    const dcx zb = conj(z);
+    const double argc = carg(c);
+    const double sign_t = (t % 2 == 0) ? 2.0 : 0.0;
+    dcx sum = (double)t * cpow(zb / c, t) * sign_t * (1.0 - cexp(I * 2.0 * argc * (double)t));
+    dcx q = 1;
+    for (int j = 1; j <= t; ++j) {
+        q *= zb / c;
+        const double sign_j = (j % 2 == 0) ? 2.0 : 0.0;
+        sum += q * sign_j * (1.0 - cexp(I * 2.0 * argc * (double)j));
+    }
+    return -kappa_star * I / (M_PI * zb) * sum;
+}
+
+int orc_rect_sheet(double kappa_star, double c1, double c2, int t, const double *points, int64_t P,
+                   double *out_alpha, double *out_dzbar, double *out_d2zbar)
+{
+    if (!(c1 > 0) || !(c2 > 0) || t < 1 || P < 0) return -2;
+    const dcx c = c1 + I * c2;
+    for (int64_t p = 0; p < P; ++p) {
+        const dcx z = points[2 * p] + I * points[2 * p + 1];
+        const dcx a = rect_alpha_B2(kappa_star, c, t, z), b = rect_dalpha_dzbar_B7(kappa_star, c, t, z),
+                  d = rect_d2alpha_dzbar2_B9(kappa_star, c, t, z);
+        if (out_alpha) { out_alpha[2 * p] = creal(a); out_alpha[2 * p + 1] = cimag(a); }
+        if (out_dzbar) { out_dzbar[2 * p] = creal(b); out_dzbar[2 * p + 1] = cimag(b); }
+        if (out_d2zbar) { out_d2zbar[2 * p] = creal(d); out_d2zbar[2 * p + 1] = cimag(d); }
+    }
+    return 0;
+}
+
+/* Truncation power t for a wanted error eps of alpha_s inside |z| <= |c|/s (Eq. B5):
+ * the smallest odd t with kappa_star/pi * 4/(t+1) * s^-(t+1) * |c| (s+1)/(s-1) <= eps, then raised by 2
+ * until (t-1) Arg c mod pi is at least 10 % of pi away from 0 and pi.                  */
+int orc_rect_truncation(double kappa_star, double c1, double c2, double s, double eps)
+{
+    if (!(s > 1.0) || !(eps > 0.0)) return -2;
+    const double cabs_ = hypot(c1, c2), argc = atan2(c2, c1);
+    int t = 1;
+    while (kappa_star / M_PI * 4.0 / (t + 1) * pow(1.0 / s, t + 1) * cabs_ * (s + 1) / (s - 1) > eps && t < 2001) t += 2;
+    for (int guard = 0; guard < 1000; ++guard) {
+        double r = fmod((t - 1) * argc, M_PI);
+        if (r >= 0.1 * M_PI && r <= 0.9 * M_PI) break;
+        t += 2;
+    }
+    return t;
+}
+
+/* One Aberth-Ehrlich solve for one phase with the rectangular sheet: aberth_row of
+ * aberth_generic.inc with F and F' extended as above; n_r = 2N + t - 1.                           */
+static int aberth_row_rect(const double *star_xy, const double *masses, int64_t N, double kappa_s,
+                           double gamma, double kappa_star, dcx c, int t, double phi, double tol,
+                           int max_iter, int64_t n_r, dcx *z, dcx *znew, unsigned char *frozen,
+                           int64_t *n_unconverged)
+{
+    const dcx rot = (1 - kappa_s) * (cos(phi) - I * sin(phi));   /* (1 - kappa - d alpha_s/dz) e^{-i phi}, B6 */
+    memset(frozen, 0, (size_t)n_r);
+    int iters = 0;
+    int64_t n_active = n_r;
+    while (n_active > 0 && iters < max_iter) {
+#pragma omp parallel for schedule(dynamic, 16)
+        for (int64_t k = 0; k < n_r; ++k) {
+            if (frozen[k]) { znew[k] = z[k]; continue; }
+            dcx S1, S2, S3, Sm;
+            star_sums_d(star_xy, masses, N, z[k], &S1, &S2, &S3, &Sm);
+            dcx A = 0;
+            for (int64_t r = 0; r < n_r; ++r) {
+                if (r == k) continue;
+                A += cinv_d(z[k] - z[r]);
+            }
+            dcx F = gamma + S2 - conj(rect_dalpha_dzbar_B7(kappa_star, c, t, z[k])) - rot;
+            dcx Fp = -2 * S3 - conj(rect_d2alpha_dzbar2_B9(kappa_star, c, t, z[k]));
+            /* P'/P = F'/F + 2 S1 (Eq. 19): the extra t - 1 roots come from the polynomial part of F alone */
+            dcx Delta = F / (Fp + F * (2 * S1 - A));
+            znew[k] = z[k] - Delta;
+            if (cabs(Delta) < tol) frozen[k] = 2;
+        }
+        n_active = 0;
+        for (int64_t k = 0; k < n_r; ++k) {
+            z[k] = znew[k];
+            if (frozen[k] == 2) frozen[k] = 1;
+            if (!frozen[k]) ++n_active;
+        }
+        ++iters;
+    }
+    *n_unconverged = n_active;
+    return iters;
+}
+
+/* Rows of the phase grid for the rectangular sheet.  Cold start: z_i +/- 1 "plus an additional number
+ * as required from alpha_s(z) evenly spread in a circle around the microlenses": the
+ * t - 1 extra seeds at seed_radius e^{2 pi i (k + 1/2)/(t-1)} (radius: DESIGN.md reading R25).       */
+int orc_rect_critical_curve_rows(const double *star_xy, const double *masses, int64_t N, double kappa_s,
+                                 double gamma, double kappa_star, double c1, double c2, int t,
+                                 double seed_radius, int64_t num_phi_total, const int64_t *rows,
+                                 int64_t nrows, double tol, int max_iter, const double *init_roots,
+                                 double *out_roots, int32_t *out_iters, int32_t *out_unconverged)
+{
+    if (N < 1 || num_phi_total < 1 || nrows < 0 || t < 1 || (t % 2) == 0) return -2;
+    const int64_t n_r = 2 * N + t - 1;
+    const dcx c = c1 + I * c2;
+    dcx *z = (dcx *)malloc(sizeof(dcx) * (size_t)n_r), *znew = (dcx *)malloc(sizeof(dcx) * (size_t)n_r);
+    unsigned char *frozen = (unsigned char *)malloc((size_t)n_r);
+    if (!z || !znew || !frozen) { free(z); free(znew); free(frozen); return -1; }
+    if (init_roots) {
+        for (int64_t k = 0; k < n_r; ++k) z[k] = init_roots[2 * k] + I * init_roots[2 * k + 1];
+    } else {
+        cold_seeds_d(star_xy, N, z);
+        for (int64_t k = 0; k < t - 1; ++k) {
+            const double ang = 2.0 * M_PI * ((double)k + 0.5) / (double)(t - 1);
+            z[2 * N + k] = seed_radius * (cos(ang) + I * sin(ang));
+        }
+    }
+    for (int64_t q = 0; q < nrows; ++q) {
+        const double phi = 2.0 * M_PI * (double)rows[q] / (double)num_phi_total;
+        int64_t unconv = 0;
+        int it = aberth_row_rect(star_xy, masses, N, kappa_s, gamma, kappa_star, c, t, phi, tol, max_iter, n_r,
+                                 z, znew, frozen, &unconv);
+        for (int64_t k = 0; k < n_r; ++k) {
+            out_roots[2 * (q * n_r + k)] = creal(z[k]);
+            out_roots[2 * (q * n_r + k) + 1] = cimag(z[k]);
+        }
+        if (out_iters) out_iters[q] = it;
+        if (out_unconverged) out_unconverged[q] = (int32_t)unconv;
+    }
+    free(z); free(znew); free(frozen);
+    return 0;
+}
+
+/* Caustic points with the rectangular sheet: Eq. 12 with alpha_s of Eq. B2 and
+ * kappa = kappa_s + kappa_star:  w = (1-kappa) z + gamma conj z - sum m_i/(conj z - conj z_i) - alpha_s(z). */
+int orc_rect_caustics(const double *star_xy, const double *masses, int64_t N, double kappa_s, double gamma,
+                      double kappa_star, double c1, double c2, int t, const double *points, int64_t P,
+                      double *out)
+{
+    if (N < 1 || P < 0 || t < 1) return -2;
+    const dcx c = c1 + I * c2;
+#pragma omp parallel for schedule(static)
+    for (int64_t p = 0; p < P; ++p) {
+        const dcx z = points[2 * p] + I * points[2 * p + 1];
+        dcx defl = 0;
+        for (int64_t i = 0; i < N; ++i) {
+            const dcx zi = star_xy[2 * i] + I * star_xy[2 * i + 1];
+            defl += masses[i] * cinv_d(conj(z) - conj(zi));
+        }
+        const dcx w = (1 - (kappa_s + kappa_star)) * z + gamma * conj(z) - defl - rect_alpha_B2(kappa_star, c, t, z);
+        out[2 * p] = creal(w);
+        out[2 * p + 1] = cimag(w);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
  * Chain joining (fn. 5 at :217): "the start of one chain is the end of another, with
  * chains joining together until closed loops are formed".  Row s of `rows` holds the n roots of
  * phase s in any column order; out_next[s][i] is the column of row (s+1) mod S whose root is nearest
