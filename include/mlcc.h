@@ -89,6 +89,18 @@ typedef struct mlcc_options {
     int32_t fmm_stars_per_node; /* mean stars per grid node (the grid has ~N / this many nodes);
                                    0 = 4                                                             */
     int32_t reserved_;        /* 0                                                                   */
+    /* Smooth-sheet polynomial (rectangular microlens field, PAPER.md:197-205 and Appendix B).  With
+       H(u) = sum_{n=0}^{d} sheet_poly[n] u^n (REAL coefficients) the lens equation becomes
+         w = (1-kappa_s) z + gamma conj(z) - conj( sum_i m_i/(z - z_i) + H(z) ),
+       so F = gamma + S2 - H'(z) - (1-kappa_s) e^{-i phi}, F' = -2 S3 - H''(z), and every row has
+       2N + d - 1 roots (d >= 2).  mlcc_rect_sheet fills the coefficients from
+       Eq. B2; the caller adds its gamma_shift to gamma.  NULL / 0 = the infinite sheet of a disc. */
+    const double *sheet_poly; /* HOST pointer, [sheet_poly_n]; the last coefficient must be non-zero  */
+    int32_t sheet_poly_n;     /* d + 1, at most 512; 0 = none                                        */
+    int32_t reserved2_;       /* 0                                                                   */
+    double seed_radius;       /* the d - 1 extra cold seeds are spread evenly on the circle of this
+                                 radius about the origin; must be > 0 when d >= 2 and
+                                 init_roots is NULL                                                   */
 } mlcc_options;
 
 /* Counters of one mlcc_critical_curves_ex call (host struct, filled on return). */
@@ -135,7 +147,8 @@ int mlcc_star_field(uint64_t seed, int64_t N, double kappa_star, int mass_model,
  * one row seeding the next along each chain.
  *   star_xy [N][2], masses [N]: device, read.
  *   out_roots [num_phi][2N][2]: device, written.  Row j is the root SET of phi_j; the column
- *     order is continuous along a sub-chain but otherwise unspecified.
+ *     order is continuous along a sub-chain but otherwise unspecified.  (With a sheet polynomial,
+ *     mlcc_options.sheet_poly, every array documented as [..][2N] is [..][mlcc_num_roots()].)
  * Default options and the default stream; returns after the work has finished.
  * Errors: INVALID_ARG, CUDA, NOMEM, NOT_CONVERGED, DEGENERATE (outputs are written in the last two). */
 int mlcc_critical_curves(const double *star_xy, const double *masses, int64_t N,
@@ -231,6 +244,26 @@ int mlcc_link_rows(const double *rows, int64_t S, int64_t n, int32_t *out_next,
 int mlcc_crossing_map(const double *caustics, const int32_t *next, int64_t S, int64_t n, int closed,
                       double x0, double y0, double pixel, int32_t nx, int32_t ny, int32_t *out_map,
                       void *stream);
+
+/* (f) NEXT-3: the rectangular sheet of Appendix B as a polynomial (host-only, no CUDA call).
+ * For stars in the rectangle with corner c = c1 + i c2 and smooth compensation kappa_star, Eq. B2
+ * truncated at the odd power t and extended to an infinite sheet is
+ *   alpha_s(z) = -kappa_star z + kappa_star (1 - 4 theta/pi) conj(z) + H(conj z),  theta = Arg c,
+ *   H(u) = -(4 kappa_star/pi) sum_{n = 3,5,..,t} sin((n-1) theta) / (n (n-1)) u^n / |c|^(n-1)
+ * (the four logarithm series collected by powers; reading R24), so that Eq. 12 and Eq. 15
+ * take the form documented at mlcc_options.sheet_poly with gamma replaced by gamma + *out_gamma_shift,
+ * *out_gamma_shift = -kappa_star (1 - 4 theta/pi).
+ *   t_in > 0: that truncation power (made odd by adding 1).  t_in = 0: the smallest odd t whose error
+ *   bound Eq. B5 is below `eps` for |z| <= |c|/s  (s > 1).  In both cases t is then raised
+ *   by 2 until (t-1) theta mod pi is at least 0.1 pi away from 0 and pi, so that the
+ *   leading coefficient of H' does not vanish.
+ *   out_coef [capacity]: host, receives t + 1 coefficients (even powers and n = 1 are zero).
+ * Returns t (> 0), or a negative mlcc_status (bad arguments, capacity < t + 1).                     */
+int mlcc_rect_sheet(double kappa_star, double c1, double c2, double s, double eps, int32_t t_in,
+                    double *out_coef, int32_t capacity, double *out_gamma_shift);
+
+/* Roots per row for N stars and a sheet polynomial of sheet_poly_n coefficients (0 = none).       */
+int64_t mlcc_num_roots(int64_t N, int32_t sheet_poly_n);
 
 /* Host-only planning helper of the phase-continuation driver: splits rows
  * [0, num_phi) into `num_subchains` contiguous sub-chains and returns, per sub-chain c, its

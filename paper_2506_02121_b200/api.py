@@ -37,7 +37,9 @@ class mlcc_options(C.Structure):
                 ("phi_index_offset", C.c_int64), ("phi_index_total", C.c_int64),
                 ("min_lanes_per_root", C.c_int32), ("aberth_sum_precision", C.c_int32),
                 ("star_sum_mode", C.c_int32), ("fmm_order", C.c_int32),
-                ("fmm_stars_per_node", C.c_int32), ("reserved_", C.c_int32)]
+                ("fmm_stars_per_node", C.c_int32), ("reserved_", C.c_int32),
+                ("sheet_poly", C.c_void_p), ("sheet_poly_n", C.c_int32), ("reserved2_", C.c_int32),
+                ("seed_radius", C.c_double)]
 
 
 class mlcc_stats(C.Structure):
@@ -93,6 +95,9 @@ def lib() -> C.CDLL:
                                                C.POINTER(mlcc_stats), vp]
         L.mlcc_caustics.argtypes = [vp, vp, i64, dbl, dbl, vp, i64, vp, vp]
         L.mlcc_match_root_sets.argtypes = [vp, vp, i64, i64, dbl, vp, vp, vp]
+        L.mlcc_num_roots.restype = C.c_int64
+        L.mlcc_num_roots.argtypes = [i64, i32]
+        L.mlcc_rect_sheet.argtypes = [dbl, dbl, dbl, dbl, dbl, i32, vp, i32, C.POINTER(dbl)]
         L.mlcc_link_rows.argtypes = [vp, i64, i64, vp, vp, vp]
         L.mlcc_crossing_map.argtypes = [vp, vp, i64, i64, C.c_int, dbl, dbl, dbl, i32, i32, vp, vp]
         L.mlcc_star_sums.argtypes = [vp, vp, i64, vp, i64, C.c_int, C.c_int, C.c_int, vp, vp]
@@ -137,7 +142,7 @@ def last_error() -> str:
 
 def options(num_subchains=0, predictor_order=-1, max_iter_cold=0, phi_index_offset=0,
             phi_index_total=0, min_lanes_per_root=0, aberth_sum_precision=0, star_sum_mode=0, fmm_order=0,
-            fmm_stars_per_node=0) -> mlcc_options:
+            fmm_stars_per_node=0, sheet_poly=None, seed_radius=0.0) -> mlcc_options:
     o = mlcc_options()
     lib().mlcc_options_default(C.byref(o))
     o.num_subchains = num_subchains
@@ -150,7 +155,29 @@ def options(num_subchains=0, predictor_order=-1, max_iter_cold=0, phi_index_offs
     o.star_sum_mode = star_sum_mode
     o.fmm_order = fmm_order
     o.fmm_stars_per_node = fmm_stars_per_node
+    if sheet_poly is not None:
+        arr = np.ascontiguousarray(sheet_poly, np.float64)
+        o._keep = arr                       # the struct holds a raw host pointer: keep the array alive
+        o.sheet_poly = arr.ctypes.data
+        o.sheet_poly_n = int(arr.size)
+        o.seed_radius = float(seed_radius)
     return o
+
+
+def num_roots(N: int, opt=None) -> int:
+    """mlcc_num_roots: roots per row (2N, plus deg H' with a sheet polynomial)."""
+    return int(lib().mlcc_num_roots(int(N), int(opt.sheet_poly_n) if (opt is not None and opt.sheet_poly) else 0))
+
+
+def rect_sheet(kappa_star, c1, c2, s=1.5, eps=1e-9, t=0):
+    """mlcc_rect_sheet -> (coef [t+1] float64, gamma_shift, t)."""
+    coef = np.zeros(512, np.float64)
+    shift = C.c_double(0.0)
+    tt = lib().mlcc_rect_sheet(float(kappa_star), float(c1), float(c2), float(s), float(eps), int(t),
+                               coef.ctypes.data, 512, C.byref(shift))
+    if tt < 0:
+        _raise(-tt)
+    return coef[:tt + 1].copy(), shift.value, tt
 
 
 def star_field(seed: int, N: int, kappa_star: float, mass_model: int = 0, mass_params=None,
@@ -198,7 +225,7 @@ def critical_curves_ex(star_xy, masses, kappa_s, gamma, num_phi, tol=1e-12, max_
     N = masses.shape[0]
     dev = masses.device
     if out_roots is None:
-        out_roots = torch.empty((num_phi, 2 * N, 2), dtype=torch.float64, device=dev)
+        out_roots = torch.empty((num_phi, num_roots(N, opt), 2), dtype=torch.float64, device=dev)
     iters = unconv = None
     if want_diagnostics:
         iters = torch.zeros((num_phi,), dtype=torch.int32, device=dev)
@@ -220,9 +247,9 @@ def curves_and_caustics(star_xy, masses, kappa_s, gamma, num_phi, tol=1e-12, max
     N = masses.shape[0]
     dev = masses.device
     if out_roots is None:
-        out_roots = torch.empty((num_phi, 2 * N, 2), dtype=torch.float64, device=dev)
+        out_roots = torch.empty((num_phi, num_roots(N, opt), 2), dtype=torch.float64, device=dev)
     if out_caustics is None:
-        out_caustics = torch.empty((num_phi, 2 * N, 2), dtype=torch.float64, device=dev)
+        out_caustics = torch.empty((num_phi, num_roots(N, opt), 2), dtype=torch.float64, device=dev)
     iters = unconv = None
     if want_diagnostics:
         iters = torch.zeros((num_phi,), dtype=torch.int32, device=dev)
@@ -334,9 +361,9 @@ def curves_and_caustics_host(star_xy: np.ndarray, masses: np.ndarray, kappa_s, g
         return x.ctypes.data
     N = int(masses.shape[0])
     if out_roots is None:
-        out_roots = np.empty((num_phi, 2 * N, 2), np.float64)
+        out_roots = np.empty((num_phi, num_roots(N, opt), 2), np.float64)
     if want_caustics and out_caustics is None:
-        out_caustics = np.empty((num_phi, 2 * N, 2), np.float64)
+        out_caustics = np.empty((num_phi, num_roots(N, opt), 2), np.float64)
     st = mlcc_stats()
     rc = lib().mlcc_curves_and_caustics_host(hptr(star_xy), hptr(masses), N, float(kappa_s), float(gamma),
                                              int(num_phi), float(tol), int(max_iter),

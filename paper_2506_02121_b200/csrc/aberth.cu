@@ -134,6 +134,10 @@ struct Params {
     double2 *delta;           // [max_slots][n_r]
     int max_slots;            // slots that can be live at once (2 n_sub)
     int R;                    // roots per thread of the compute kernel in use
+    // smooth-sheet polynomial H(u) = sum poly[n] u^n (rectangular field, Appendix B); poly_n = 0: none
+    const double *poly;       // [poly_n] device
+    int poly_n;
+    double seed_radius;       // circle of the n_r - 2N extra cold seeds
     // far-field mode (MLCC_STAR_SUMS_FMM): star sums come from k_star_sums, the compute kernel sums root pairs only
     double *ssum;             // [max_slots][n_r][8] star sums of the unfrozen roots, by list position
     int2 *outside;            // [max_slots * n_r] (slot, position) of the roots outside the node grid
@@ -301,10 +305,14 @@ __global__ void k_seed(Params p)
         if (st.step == 0) {
             if (p.init_roots) {
                 z = p.init_roots[k];
-            } else {  // z_i + 1, z_i - 1
+            } else if (k < 2 * p.N) {  // z_i + 1, z_i - 1
                 const int i = (k < p.N) ? k : k - p.N;
                 z = p.stars[i];
                 z.x += (k < p.N) ? 1.0 : -1.0;
+            } else {  // "plus an additional number as required from alpha_s, evenly spread in a circle"
+                double sn, cs;
+                sincospi(2.0 * ((double)(k - 2 * p.N) + 0.5) / (double)(p.n_r - 2 * p.N), &sn, &cs);
+                z = make_double2(p.seed_radius * cs, p.seed_radius * sn);
             }
         } else {
             // extrapolate through the last (order+1) rows of this chain that exist:
@@ -347,6 +355,23 @@ __device__ __forceinline__ void aberth_step(const Params &p, int slot, long long
     const int k = list[pos];
     const double2 z = p.roots[row * p.n_r + k];
     const double2 rot = p.rot[row];
+    if (p.poly_n > 0) {
+        // sheet polynomial with real coefficients: Sm += H(z), S2 -= H'(z), S3 += H''(z)/2, so that
+        // F = gamma + S2 - (1-kappa_s) e^{-i phi}, F' = -2 S3 and the caustic expansion below hold as they are
+        double b0x = 0, b0y = 0, b1x = 0, b1y = 0, b2x = 0, b2y = 0;
+        for (int l = p.poly_n - 1; l >= 0; --l) {
+            const double c = __ldg(&p.poly[l]);
+            double tx_ = fma(b2x, z.x, fma(-b2y, z.y, b1x)), ty_ = fma(b2x, z.y, fma(b2y, z.x, b1y));
+            b2x = tx_; b2y = ty_;
+            tx_ = fma(b1x, z.x, fma(-b1y, z.y, b0x)); ty_ = fma(b1x, z.y, fma(b1y, z.x, b0y));
+            b1x = tx_; b1y = ty_;
+            tx_ = fma(b0x, z.x, fma(-b0y, z.y, c)); ty_ = fma(b0x, z.y, b0y * z.x);
+            b0x = tx_; b0y = ty_;
+        }
+        smx += b0x; smy += b0y;
+        s2x -= b1x; s2h -= 0.5 * b1y;
+        s3x += b2x; s3y += b2y;
+    }
     const double s2y = 2.0 * s2h;
     const double fx_ = p.gamma + s2x - rot.x;   // F
     const double fy_ = s2y - rot.y;
@@ -1041,8 +1066,22 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
         if (b > max_steps) max_steps = (int)b;
     }
     const int max_slots = 2 * n_sub > 1 ? 2 * n_sub : 1;
-    const int n_r = (int)(2 * N);
-    const int N_pad = (int)((N + S_TILE - 1) / S_TILE) * S_TILE;
+    // sheet polynomial: n_extra = deg H' = poly_n - 2 more roots per row
+    const int poly_n = opt.sheet_poly ? opt.sheet_poly_n : 0;
+    if (poly_n < 0 || poly_n > 512) return invalid("sheet_poly_n out of range");
+    if (poly_n > 0) {
+        for (int q = 0; q < poly_n; ++q)
+            if (!isfinite(opt.sheet_poly[q])) return invalid("sheet_poly has a non-finite coefficient");
+        if (opt.sheet_poly[poly_n - 1] == 0.0) return invalid("the last sheet_poly coefficient is zero");
+    }
+    const int n_extra = poly_n >= 3 ? poly_n - 2 : 0;
+    if (n_extra > 0 && !init_roots && !(opt.seed_radius > 0.0 && isfinite(opt.seed_radius)))
+        return invalid("seed_radius must be positive when the sheet polynomial adds roots");
+    if (2 * N + n_extra > (1ll << 30)) return invalid("too many roots");
+    const int n_r = (int)(2 * N) + n_extra;
+    // a stage pairs 256 stars with 512 root entries: enough (massless, far away) padding stars for all roots
+    const long long n_half = (n_r + 1) / 2 > N ? (n_r + 1) / 2 : N;
+    const int N_pad = (int)((n_half + S_TILE - 1) / S_TILE) * S_TILE;
 
     Workspace ws(stream);
     Params p{};
@@ -1119,6 +1158,14 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     p.min_T = min_T;
     p.grid_ctas = grid_compute;
     p.R = ks.R;
+    p.poly_n = poly_n;
+    p.seed_radius = opt.seed_radius;
+    if (poly_n > 0) {
+        double *d_poly = nullptr;
+        MLCC_CUDA(ws.alloc(&d_poly, (size_t)poly_n));
+        MLCC_CUDA(cudaMemcpyAsync(d_poly, opt.sheet_poly, sizeof(double) * poly_n, cudaMemcpyHostToDevice, stream));
+        p.poly = d_poly;
+    }
     p.rot = d_rot;
     p.init_roots = reinterpret_cast<const double2 *>(init_roots);
     p.roots = reinterpret_cast<double2 *>(out_roots);
@@ -1212,7 +1259,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     if (out_stats) {
         out_stats->root_iterations = fin.root_iterations;
         out_stats->star_pairs = fin.root_iterations * N;
-        out_stats->root_pairs = fin.root_iterations * (2 * N - 1);
+        out_stats->root_pairs = fin.root_iterations * (n_r - 1);
         out_stats->kernel_launches = launches;
         out_stats->total_iterations = fin.total_iterations;
         out_stats->steps = max_steps + 1;

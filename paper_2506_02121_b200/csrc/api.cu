@@ -149,6 +149,10 @@ void mlcc_options_default(mlcc_options *opt)
     opt->fmm_order = 0;
     opt->fmm_stars_per_node = 0;
     opt->reserved_ = 0;
+    opt->sheet_poly = nullptr;
+    opt->sheet_poly_n = 0;
+    opt->reserved2_ = 0;
+    opt->seed_radius = 0.0;
 }
 
 int mlcc_star_field(uint64_t seed, int64_t N, double kappa_star, int mass_model, const double *mass_params,
@@ -193,6 +197,40 @@ int mlcc_caustics(const double *star_xy, const double *masses, int64_t N, double
                          static_cast<cudaStream_t>(stream));
 }
 
+int64_t mlcc_num_roots(int64_t N, int32_t sheet_poly_n)
+{
+    return 2 * N + (sheet_poly_n >= 3 ? sheet_poly_n - 2 : 0);
+}
+
+int mlcc_rect_sheet(double kappa_star, double c1, double c2, double s, double eps, int32_t t_in, double *out_coef,
+                    int32_t capacity, double *out_gamma_shift)
+{
+    if (!out_coef || !out_gamma_shift) return -invalid("null pointer");
+    if (!(kappa_star >= 0.0) || !(c1 > 0.0) || !(c2 > 0.0) || !isfinite(kappa_star + c1 + c2)) return -invalid("kappa_star, c1, c2");
+    const double pi = 3.14159265358979323846264338327950288;
+    const double cabs = hypot(c1, c2), theta = atan2(c2, c1);
+    int t = t_in;
+    if (t < 0) return -invalid("t_in < 0");
+    if (t == 0) {   // Eq. B5
+        if (!(s > 1.0) || !(eps > 0.0)) return -invalid("s must be > 1 and eps > 0");
+        t = 1;
+        while (kappa_star / pi * 4.0 / (t + 1) * pow(1.0 / s, t + 1) * cabs * (s + 1.0) / (s - 1.0) > eps && t < 2001) t += 2;
+    } else if (t % 2 == 0) {
+        t += 1;
+    }
+    for (int guard = 0; guard < 1000; ++guard) {   // keep (t-1) theta away from the multiples of pi
+        const double r = fmod((t - 1) * theta, pi);
+        if (r >= 0.1 * pi && r <= 0.9 * pi) break;
+        t += 2;
+    }
+    if (t + 1 > capacity || t + 1 > 512) return -invalid("capacity < t + 1 (or t > 511)");
+    for (int n = 0; n <= t; ++n) out_coef[n] = 0.0;
+    for (int n = 3; n <= t; n += 2)
+        out_coef[n] = -(4.0 * kappa_star / pi) * sin((n - 1) * theta) / ((double)n * (n - 1)) / pow(cabs, n - 1);
+    *out_gamma_shift = -kappa_star * (1.0 - 4.0 * theta / pi);
+    return t;
+}
+
 int mlcc_link_rows(const double *rows, int64_t S, int64_t n, int32_t *out_next, int32_t *out_bijective,
                    void *stream)
 {
@@ -235,7 +273,7 @@ int mlcc_curves_and_caustics_host(const double *star_xy, const double *masses, i
     if (!star_xy || !masses || !out_roots) return invalid("null pointer");
     if (N < 1 || N > (1 << 28)) return invalid("N out of range");
     if (num_phi < 1) return invalid("num_phi < 1");
-    const size_t n_pts = (size_t)num_phi * 2 * (size_t)N;
+    const size_t n_pts = (size_t)num_phi * (size_t)mlcc_num_roots(N, (opt && opt->sheet_poly) ? opt->sheet_poly_n : 0);
     DeviceBuffer d_xy, d_m, d_roots, d_caus;
     MLCC_CUDA(d_xy.alloc(sizeof(double) * 2 * (size_t)N));
     MLCC_CUDA(d_m.alloc(sizeof(double) * (size_t)N));

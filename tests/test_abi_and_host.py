@@ -44,7 +44,7 @@ def test_version_and_status_strings(lib):
 def test_options_default_and_struct_layout(lib):
     from paper_2506_02121_b200 import api
     o = api.options()
-    assert o.struct_size == C.sizeof(api.mlcc_options) == 56
+    assert o.struct_size == C.sizeof(api.mlcc_options) == 80
     assert o.predictor_order == -1 and o.num_subchains == 0 and o.phi_index_total == 0
     assert C.sizeof(api.mlcc_stats) == 64
 
@@ -136,3 +136,32 @@ def test_product_does_not_import_the_oracle():
                 assert "liboracle" not in text and "mlcc_oracle" not in text, f
     text = open(os.path.join(ROOT, "include", "mlcc.h")).read()
     assert "oracle" not in text.lower()
+
+
+def test_rect_sheet_polynomial_reproduces_eq_b2(lib, orc):
+    """mlcc_rect_sheet (host-only): its real-coefficient polynomial H and gamma shift against the oracle's literal
+    Eq. B2 / B7 (four corners, complex logarithms): alpha_s = -kappa_star z + kappa_star (1 - 4 theta/pi) conj z + H(conj z),
+    conj(d alpha_s/d zbar) = -gamma_shift + H'(z); t from Eq. B5 and the (t-1) Arg c rule as the oracle finds it."""
+    from paper_2506_02121_b200 import api
+    rng = np.random.default_rng(2)
+    for kstar, c1, c2 in ((0.4, 3.0, 2.0), (0.25, 2.0, 5.0), (0.6, 4.0, 4.0)):
+        coef, shift, t = api.rect_sheet(kstar, c1, c2, s=1.5, eps=1e-9)
+        assert t == orc.rect_truncation(kstar, c1, c2, 1.5, 1e-9) and t % 2 == 1 and len(coef) == t + 1
+        assert coef[t] != 0.0 and (coef[0::2] == 0).all() and coef[1] == 0
+        theta = np.arctan2(c2, c1)
+        assert abs(shift + kstar * (1 - 4 * theta / np.pi)) < 1e-15
+        pts = rng.uniform(-1, 1, size=(50, 2)) * [c1, c2] * 0.6
+        z = pts[:, 0] + 1j * pts[:, 1]
+        a, b7, b9 = orc.rect_sheet(kstar, c1, c2, t, pts)
+        H = np.polyval(coef[::-1], np.conj(z))
+        assert np.abs(-kstar * z - shift * np.conj(z) + H - a).max() < 1e-13
+        dH = np.polyval(np.polyder(coef[::-1]), z)
+        assert np.abs(-shift + dH - np.conj(b7)).max() < 1e-13
+        d2H = np.polyval(np.polyder(coef[::-1], 2), z)
+        assert np.abs(d2H - np.conj(b9)).max() < 1e-12
+    coef5, _, t5 = api.rect_sheet(0.4, 3.0, 2.0, t=4)          # even request -> odd
+    assert t5 % 2 == 1 and t5 >= 5
+    assert api.num_roots(7) == 14 and api.num_roots(7, api.options(sheet_poly=coef5, seed_radius=4.0)) == 14 + t5 - 1
+    L = lib
+    assert L.mlcc_rect_sheet(0.4, -1.0, 2.0, 1.5, 1e-9, 0, coef5.ctypes.data, 6, C.byref(C.c_double())) < 0
+    assert L.mlcc_rect_sheet(0.4, 3.0, 2.0, 1.5, 1e-9, 0, coef5.ctypes.data, 6, C.byref(C.c_double())) < 0   # capacity

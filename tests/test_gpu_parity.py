@@ -565,3 +565,62 @@ def test_link_rows_edge_cases(api, orc):
     empty = torch.empty((0, 4, 2), dtype=torch.float64, device="cuda")
     n0, b0 = api.link_rows(empty)
     assert n0.shape == (0, 4) and b0.shape == (0,)
+
+
+# ---------------------------------------------------------------------------------------------
+# rectangular microlens field (Appendix A-B)
+# ---------------------------------------------------------------------------------------------
+def _rect_field(N, kappa_star, aspect, seed):
+    """N equal-or-random-mass stars uniform in the rectangle of area pi N / kappa_star (Eq. 9 with sum m = N)."""
+    rng = np.random.default_rng(seed)
+    c2 = np.sqrt(np.pi * N / (4 * kappa_star * aspect))
+    c1 = aspect * c2
+    xy = rng.uniform(-1, 1, size=(N, 2)) * [c1, c2]
+    m = rng.uniform(0.3, 1.7, size=N)
+    m *= N / m.sum()
+    return xy, m, c1, c2
+
+
+@pytest.mark.parametrize("N,aspect,num_phi,t_req", [(12, 1.5, 96, 7), (150, 0.6, 48, 0), (600, 2.0, 10, 0)])
+def test_rectangular_field_roots_and_caustics_against_oracle(api, orc, N, aspect, num_phi, t_req):
+    """The CUDA path evaluates the sheet as the real-coefficient polynomial of mlcc_rect_sheet; the oracle evaluates
+    Eq. B2 / B7 / B9 as printed.  Same 2N + t - 1 roots per row (1e-10 (1 + |z|)), caustic points within 1e-9."""
+    kstar, ks, g = 0.4, 0.05, 0.2
+    xy, m, c1, c2 = _rect_field(N, kstar, aspect, 17 + N)
+    coef, shift, t = api.rect_sheet(kstar, c1, c2, s=1.5, eps=1e-9, t=t_req)
+    seed_r = 1.2 * np.hypot(c1, c2)
+    n_r = 2 * N + t - 1
+    rows = np.arange(num_phi) if N <= 150 else np.array([0, num_phi // 2, num_phi - 1])
+    ref, _, un = orc.rect_critical_curve_rows(xy, m, ks, g, kstar, c1, c2, t, seed_r, num_phi, rows)
+    assert un.sum() == 0 and ref.shape[1] == n_r
+    w_ref = orc.rect_caustics(xy, m, ks, g, kstar, c1, c2, t, ref)
+    for mode in (api.MLCC_STAR_SUMS_DIRECT, api.MLCC_STAR_SUMS_FMM):
+        opt = api.options(sheet_poly=coef, seed_radius=seed_r, star_sum_mode=mode)
+        roots, caus, iters, unconv, st = api.curves_and_caustics(dev(xy), dev(m), ks, g + shift, num_phi, opt=opt)
+        assert roots.shape == (num_phi, n_r, 2) and int(unconv.sum()) == 0 and st.degenerate_roots == 0
+        gr, gw = roots.cpu().numpy(), caus.cpu().numpy()
+        assert_rows_match(orc, gr[rows], ref)
+        for i, j in enumerate(rows):
+            assert_caustics_match(gr[j], gw[j], ref[i], w_ref[i])
+    # the extra roots exist and lie outside the rectangle (where the truncated series stops representing the sheet)
+    zr = cplx(ref[0])
+    outside = (np.abs(zr.real) > c1) | (np.abs(zr.imag) > c2)
+    assert outside.sum() >= t - 1
+    # without the polynomial the same stars have 2N roots: the option changes the problem, and is needed
+    plain, _, _, _ = api.critical_curves_ex(dev(xy), dev(m), ks, g + shift, num_phi)
+    assert plain.shape[1] == 2 * N
+
+
+def test_rectangular_field_argument_checks(api):
+    xy, m = dev(np.array([[0.1, 0.2], [-0.4, 0.3]])), dev(np.ones(2))
+    with pytest.raises(api.MlccError) as e:          # extra roots need a seed circle (or init_roots)
+        api.critical_curves_ex(xy, m, 0.0, 0.1, 4, opt=api.options(sheet_poly=[0, 0, 0, 0.01], seed_radius=0.0))
+    assert e.value.status == api.MLCC_ERR_INVALID_ARG
+    with pytest.raises(api.MlccError) as e:          # vanishing leading coefficient: the degree would drop
+        api.critical_curves_ex(xy, m, 0.0, 0.1, 4, opt=api.options(sheet_poly=[0, 0, 0, 0.0], seed_radius=2.0))
+    assert e.value.status == api.MLCC_ERR_INVALID_ARG
+    # degree 1 (H = h1 u) is a pure shear shift: no extra roots, same as gamma - h1
+    a, _, _, _ = api.critical_curves_ex(xy, m, 0.0, 0.1, 4, opt=api.options(sheet_poly=[0.0, 0.03]))
+    b, _, _, _ = api.critical_curves_ex(xy, m, 0.0, 0.07, 4)
+    err, bij = api.match_root_sets(a, b, 1e-12)
+    assert a.shape == b.shape and bool(bij.all())
