@@ -52,6 +52,8 @@ def parse():
     ap.add_argument("--star-sums", default="direct", choices=["direct", "fmm"],
                     help="direct: O(N) star sums as BASELINE.json fixes (headline); fmm: the paper's near/far split "
                          "(PAPER.md:188-195) -- the roofline object then counts the root pairs only")
+    ap.add_argument("--skip-aberth-below", type=float, default=0.0,
+                    help="mlcc_options.skip_aberth_sum_below (0 = library default, negative = never skip)")
     ap.add_argument("--separate-caustics", action="store_true",
                     help="run mlcc_critical_curves_ex + mlcc_caustics instead of the fused call")
     return ap.parse_args()
@@ -171,7 +173,7 @@ def main():
     phi_off, phi_total = sharding.phase_shard(rank, world, num_phi)
     opt = api.options(num_subchains=args.subchains, predictor_order=args.order, min_lanes_per_root=args.min_lanes,
                       phi_index_offset=phi_off, phi_index_total=phi_total,
-                      aberth_sum_precision=args.aberth_sum,
+                      aberth_sum_precision=args.aberth_sum, skip_aberth_sum_below=args.skip_aberth_below,
                       star_sum_mode=api.MLCC_STAR_SUMS_FMM if args.star_sums == "fmm" else api.MLCC_STAR_SUMS_DIRECT)
 
     roots = torch.empty((num_phi, n_r, 2), dtype=torch.float64, device="cuda")
@@ -210,6 +212,7 @@ def main():
     solve_ms = 0.0
     launches = 0
     alg_flop = 0.0
+    alg_flop_survey = 0.0
     compute_launches = 0
     barrier()
     ev0.record()
@@ -218,6 +221,7 @@ def main():
         solve_ms += st.solve_ms
         launches += st.kernel_launches + 3 + 1 + (1 if args.separate_caustics else 0)   # star field (3), matcher, caustics
         alg_flop += (0.0 if args.star_sums == "fmm" else FLOP_PER_STAR_PAIR * st.star_pairs) + FLOP_PER_ROOT_PAIR * st.root_pairs
+        alg_flop_survey += (FLOP_PER_STAR_PAIR * cfg.N + FLOP_PER_ROOT_PAIR * (n_r - 1)) * st.root_iterations
         compute_launches += st.total_iterations
     ev1.record()
     barrier()
@@ -241,10 +245,14 @@ def main():
                 "peak_source": "measured on this GPU by mlcc_fp64_peak (dependent-free DFMA loop); "
                                f"nominal {NOMINAL_FP64_TFLOPS:.1f} TFLOP/s = 148 SMs x 64 lanes x 2 x 1.965 GHz",
                 "frac_of_nominal": achieved / NOMINAL_FP64_TFLOPS,
+                "frac_with_survey_accounting": (alg_flop_survey / (solve_ms * 1e-3) / 1e12 / peak_measured
+                                                if (solve_ms > 0 and peak_measured and args.star_sums == "direct") else None),
                 "algorithmic_flop_per_launch": alg_flop / max(compute_launches, 1),
                 "avg_launch_ms": solve_ms / max(compute_launches, 1),
-                "note": "achieved = (27 flop x star pairs + 10 flop x root pairs of unfrozen roots) / device time of the "
-                        "whole solve (seed/apply/finalize launches included), CUDA events on the launch stream",
+                "note": "achieved = (27 flop x star pairs + 10 flop x root pairs EVALUATED) / device time of the whole solve "
+                        "(seed/apply/finalize launches included), CUDA events on the launch stream. Confirming iterations "
+                        "of nearly converged roots leave the Aberth sum out (DESIGN.md R27) and their root pairs are not "
+                        "counted; frac_with_survey_accounting counts 47N flop for every root-iteration as SURVEY.md 8(d) does",
                 "traffic": None}
 
     # ---- measured issue model behind the roofline ----
@@ -262,7 +270,7 @@ def main():
     if world == 1 and args.star_sums == "direct" and not args.no_e2e:
         fopt = api.options(num_subchains=args.subchains, predictor_order=args.order, min_lanes_per_root=args.min_lanes,
                            phi_index_offset=phi_off, phi_index_total=phi_total, aberth_sum_precision=args.aberth_sum,
-                           star_sum_mode=api.MLCC_STAR_SUMS_FMM)
+                           skip_aberth_sum_below=args.skip_aberth_below, star_sum_mode=api.MLCC_STAR_SUMS_FMM)
         fxy, fm, _ = api.star_field(cfg.seed, cfg.N, cfg.kappa_star, cfg.mass_model, cfg.mass_params)
         best = None
         for _ in range(2):

@@ -101,13 +101,21 @@ typedef struct mlcc_options {
     double seed_radius;       /* the d - 1 extra cold seeds are spread evenly on the circle of this
                                  radius about the origin; must be > 0 when d >= 2 and
                                  init_roots is NULL                                                   */
+    double skip_aberth_sum_below; /* A root whose step |dz| was below this (but not below tol) is iterated
+                                 the next time without the Aberth sum A (Eq. 17): that iteration only
+                                 confirms |dz| < tol, and A, which multiplies F ~ F' dz in the
+                                 denominator, cannot move the step by more than |dz|^2 |A| (DESIGN.md
+                                 reading R27).  The first iteration of every row always has A, and so
+                                 has every root whose last step was larger.  0 = library default
+                                 (1e-8); negative = never skip.                                       */
 } mlcc_options;
 
 /* Counters of one mlcc_critical_curves_ex call (host struct, filled on return). */
 typedef struct mlcc_stats {
     int64_t root_iterations;   /* sum over all Aberth iterations of the number of unfrozen roots updated */
     int64_t star_pairs;        /* (root, star) pair evaluations  = root_iterations * N                  */
-    int64_t root_pairs;        /* (root, root) pair evaluations  = root_iterations * (2N - 1)           */
+    int64_t root_pairs;        /* (root, root) pair evaluations: (2N - 1) per root-iteration that had the
+                                  Aberth sum (see mlcc_options.skip_aberth_sum_below)                    */
     int64_t kernel_launches;   /* kernels launched by the call                                          */
     int32_t total_iterations;  /* Aberth iterations summed over steps (one step = all chains advance 1 row) */
     int32_t steps;             /* steps taken (cold step included)                                      */

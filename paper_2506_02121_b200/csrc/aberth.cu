@@ -67,6 +67,16 @@ constexpr float PAD_ROOT_F = 1e18f; // padding root of the FP32 source copy: its
 constexpr int MODE_F32 = 0;       // Aberth sum in double-single FP32 (default)
 constexpr int MODE_F64 = 1;       // Aberth sum in FP64 with the 20-bit reciprocal seed
 
+// Tiles of one compute kernel.
+struct TileSet {
+    int T;                // threads per root in the coarse tiles
+    int Tf;               // threads per root in the fine tiles (the last, partial round of work)
+    int n_coarse;         // tiles [0, n_coarse) are coarse, [n_coarse, n_tiles) fine
+    int n_tiles;
+    int next_tile;        // tile counter of the running launch (atomic)
+    int total;            // roots in these tiles
+};
+
 struct DevState {
     int step;             // current step: 0 = cold centre rows, s >= 1 = rows centre +/- s
     int iter;             // iterations done in this step
@@ -74,16 +84,13 @@ struct DevState {
     int done;             // all steps finished
     int need_seed;        // the seed kernel must write starting values for this step
     int cur;              // which of the two active lists is current
-    int T;                // threads per root in the coarse tiles of the next compute launch
-    int Tf;               // threads per root in its fine tiles (the last, partial round of work)
-    int n_coarse;         // coarse tiles: tiles [0, n_coarse) are coarse, [n_coarse, n_tiles) fine
-    int n_tiles;          // CTA tiles of the next compute launch
-    int next_tile;        // tile counter of the running compute launch (atomic)
+    TileSet ts[2];        // tiles of the next compute launches: [0] full kernel, [1] the one without the Aberth sum
     int total_active;     // unfrozen roots over all slots
     int total_iterations;
     int unconverged_rows;
     int degenerate;
     int n_outside;        // far-field mode: roots of this iteration that lie outside the node grid (atomic)
+    long long root_iterations_noA;   // root-iterations done without the Aberth sum
     long long root_iterations;
     long long launches_used;  // compute launches that did work
 };
@@ -128,8 +135,10 @@ struct Params {
     int *slot_dir;            // [MAX_SLOTS] -1, +1 (0 = centre)
     int *slot_iters;          // [MAX_SLOTS] iteration at which the slot last had unfrozen roots
     int *n_active;            // [2][MAX_SLOTS]
-    int *tile_start;          // [2][MAX_SLOTS + 1] first coarse / first fine tile of each slot
-    int *coarse_roots;        // [MAX_SLOTS] unfrozen roots of the slot covered by its coarse tiles
+    int *tile_start;          // [2 kernels][2][MAX_SLOTS + 1] first coarse / first fine tile of each slot
+    int *coarse_roots;        // [2 kernels][MAX_SLOTS] roots of the slot covered by its coarse tiles
+    int *n_small;             // [2][MAX_SLOTS] of the unfrozen roots of a slot, how many took a step below the
+                              //   skip threshold last time: they sit at the END of the slot's list
     int *list;                // [2][max_slots][n_r]
     double2 *delta;           // [max_slots][n_r]
     int max_slots;            // slots that can be live at once (2 n_sub)
@@ -138,6 +147,7 @@ struct Params {
     const double *poly;       // [poly_n] device
     int poly_n;
     double seed_radius;       // circle of the n_r - 2N extra cold seeds
+    double skip_below2;       // a root whose last |Delta|^2 was below this is iterated without the Aberth sum; 0 = never
     // far-field mode (MLCC_STAR_SUMS_FMM): star sums come from k_star_sums, the compute kernel sums root pairs only
     double *ssum;             // [max_slots][n_r][8] star sums of the unfrozen roots, by list position
     int2 *outside;            // [max_slots * n_r] (slot, position) of the roots outside the node grid
@@ -463,20 +473,27 @@ __global__ void __launch_bounds__(BLOCK) k_star_sums_outside(Params p)
 // read costs the same wavefronts whatever T is, and each value read is used for R roots.
 // STARS = false (far-field mode): the stages carry root entries only and the star sums are read
 // from p.ssum; the loop body is then two packed FP32 root pairs per root, hence the larger R.
-template <int MODE, bool CAUS, bool STARS, int R>
+// ROOTS = false: the variant without the Aberth sum (A = 0).  It takes the unfrozen roots whose last step was below
+// the skip threshold (the tail [n_active - n_small, n_active) of every slot's list, tile set 1); the full kernel
+// takes the others (tile set 0).  DESIGN.md reading R27.
+template <int MODE, bool CAUS, bool STARS, bool ROOTS, int R>
 __global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Params p)
 {
     __shared__ Stage s_stage[2];
     __shared__ __align__(8) unsigned long long s_full[2];
     __shared__ int s_tile;
     constexpr int NV = STARS ? (CAUS ? 8 : 6) : 2;
-    constexpr unsigned STAGE_TX = STARS ? STAGE_BYTES : 2 * S_TILE * 16;
+    constexpr unsigned STAGE_TX = (STARS ? S_TILE * 24 : 0) + (ROOTS ? 2 * S_TILE * 16 : 0);
+    constexpr bool STAGES = STARS || ROOTS;
     static_assert(sizeof(Stage) * 2 >= (size_t)NV * R * CTA * sizeof(double), "reduction scratch aliases the stages");
 
     const DevState st = *p.state;
     if (st.done) return;
+    constexpr int K = ROOTS ? 0 : 1;
+    const TileSet ts = st.ts[K];
+    if (ts.n_tiles == 0) return;
     const int tid = threadIdx.x;
-    const int n_stage = p.N_pad / S_TILE;
+    const int n_stage = STAGES ? p.N_pad / S_TILE : 0;
     const int n_src = 2 * p.N_pad;
     const int *n_active = p.n_active + st.cur * MAX_SLOTS;
 
@@ -489,21 +506,21 @@ __global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Para
     unsigned g = 0;   // stages consumed by this CTA so far: buffer g & 1, parity (g >> 1) & 1
 
     for (;;) {
-        if (tid == 0) s_tile = atomicAdd(&p.state->next_tile, 1);
+        if (tid == 0) s_tile = atomicAdd(&p.state->ts[K].next_tile, 1);
         __syncthreads();
         const int tile = s_tile;
-        if (tile >= st.n_tiles) break;
+        if (tile >= ts.n_tiles) break;
         // coarse tiles first (whole rounds of the grid), then fine tiles (more threads per root, fewer
         // roots per tile) that even out the last, partial round
-        const bool fine = tile >= st.n_coarse;
-        const int T = fine ? st.Tf : st.T;   // threads per root (power of two, 1..CTA)
+        const bool fine = tile >= ts.n_coarse;
+        const int T = fine ? ts.Tf : ts.T;   // threads per root (power of two, 1..CTA)
         const int G = CTA / T;
         const int sub = tid / G;
         const int local = tid - sub * G;
         const int n_it = S_TILE / T;         // pair-loop iterations per stage (even, >= 2)
         const int tile_roots = R * G;
-        const int *tab = p.tile_start + (fine ? MAX_SLOTS + 1 : 0);
-        const int tt = fine ? tile - st.n_coarse : tile;
+        const int *tab = p.tile_start + (2 * K + (fine ? 1 : 0)) * (MAX_SLOTS + 1);
+        const int tt = fine ? tile - ts.n_coarse : tile;
         int lo = 0, hi = st.n_slots;         // slot of this tile: last slot with tab[slot] <= tt
         while (hi - lo > 1) {
             const int mid = (lo + hi) >> 1;
@@ -512,18 +529,21 @@ __global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Para
         const int slot = lo;
         const long long row = p.slot_row[slot];
         const float4 *slot_src = p.src + (size_t)slot * n_src;
-        if (tid == 0) {   // first stage of this tile
+        if (STAGES && tid == 0) {   // first stage of this tile
             const unsigned b = g & 1u;
             mbar_expect_tx(&s_full[b], STAGE_TX);
             if (STARS) {
                 tma_load(s_stage[b].sxy, p.stars_pad, S_TILE * 16, &s_full[b]);
                 tma_load(s_stage[b].sm, p.mass_pad, S_TILE * 8, &s_full[b]);
             }
-            tma_load(s_stage[b].rp, slot_src, 2 * S_TILE * 16, &s_full[b]);
+            if (ROOTS) tma_load(s_stage[b].rp, slot_src, 2 * S_TILE * 16, &s_full[b]);
         }
         const int *list = p.list + ((long long)st.cur * p.max_slots + slot) * p.n_r;
-        const int n_act = n_active[slot];
-        const int base = (fine ? p.coarse_roots[slot] : 0) + (tt - tab[slot]) * tile_roots;
+        // this kernel's share of the slot's list: positions [pos_lo, n_act)
+        const int n_all = n_active[slot], n_large = n_all - p.n_small[st.cur * MAX_SLOTS + slot];
+        const int pos_lo = ROOTS ? 0 : n_large;
+        const int n_act = ROOTS ? n_large : n_all;
+        const int base = pos_lo + (fine ? p.coarse_roots[K * MAX_SLOTS + slot] : 0) + (tt - tab[slot]) * tile_roots;
         const bool valid = base + local < n_act;   // this thread has at least its first root
         double zx[R], zy[R];
         float zxh[R], zxl[R], zyh[R], zyl[R];
@@ -558,7 +578,7 @@ __global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Para
                     tma_load(s_stage[nb].sxy, p.stars_pad + (size_t)(t + 1) * S_TILE, S_TILE * 16, &s_full[nb]);
                     tma_load(s_stage[nb].sm, p.mass_pad + (size_t)(t + 1) * S_TILE, S_TILE * 8, &s_full[nb]);
                 }
-                tma_load(s_stage[nb].rp, slot_src + (size_t)(t + 1) * 2 * S_TILE, 2 * S_TILE * 16, &s_full[nb]);
+                if (ROOTS) tma_load(s_stage[nb].rp, slot_src + (size_t)(t + 1) * 2 * S_TILE, 2 * S_TILE * 16, &s_full[nb]);
             }
             mbar_wait(&s_full[b], (g >> 1) & 1u);
             if (valid) {
@@ -575,7 +595,11 @@ __global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Para
                             sxy = sg.sxy[j];
                             sm = sg.sm[j];
                         }
-                        if (MODE == MODE_F64) {
+                        if (!ROOTS) {
+#pragma unroll
+                            for (int r = 0; r < R; ++r)
+                                if (STARS) pair_star<CAUS>(zx[r], zy[r], sxy, sm, acc[r]);
+                        } else if (MODE == MODE_F64) {
                             const double2 *rr = reinterpret_cast<const double2 *>(sg.rp);
                             const double2 ra = rr[2 * j], rb = rr[2 * j + 1];
 #pragma unroll
@@ -691,15 +715,36 @@ __global__ void __launch_bounds__(APPLY_THREADS) k_apply(Params p)
     const double2 *delta = p.delta + (long long)slot * p.n_r;
     double2 *row = p.roots + p.slot_row[slot] * p.n_r;
     float4 *slot_src = p.src + (size_t)slot * 2 * p.N_pad;
-    int base = 0;
+    // A survivor (|Delta|^2 >= tol^2) is "large" if |Delta|^2 >= skip_below2, else "small": the next list holds
+    // the large ones first, then the small ones, each group in the order of this list.
+    // pass 1: the number of large survivors = where the small ones start
+    int n_large = 0;
+    for (int pos = tid; pos < n_act; pos += APPLY_THREADS) {
+        const double2 d = delta[pos];
+        const double d2 = d.x * d.x + d.y * d.y;
+        if (d2 <= 1.79769313486231570e308 && !(d2 < p.tol2) && !(d2 < p.skip_below2)) ++n_large;
+    }
+    for (int o = 16; o > 0; o >>= 1) n_large += __shfl_xor_sync(0xffffffffu, n_large, o);
+    if (lane == 0) s_warp[warp] = n_large;
+    __syncthreads();
+    if (tid == 0) {
+        int t = 0;
+        for (int w = 0; w < APPLY_THREADS / 32; ++w) t += s_warp[w];
+        s_total = t;
+    }
+    __syncthreads();
+    n_large = s_total;
+    __syncthreads();
+    // pass 2: apply the steps, write both groups in order (counts packed: large in the low 16 bits, small above)
+    int base_l = 0, base_s = n_large;
     for (int c0 = 0; c0 < n_act; c0 += APPLY_THREADS * APPLY_ITEMS) {
         int ks[APPLY_ITEMS];
-        bool keep[APPLY_ITEMS];
+        int kind[APPLY_ITEMS];   // 0 frozen, 1 large, 2 small
         int cnt = 0;
 #pragma unroll
         for (int i = 0; i < APPLY_ITEMS; ++i) {
             const int pos = c0 + tid * APPLY_ITEMS + i;
-            keep[i] = false;
+            kind[i] = 0;
             ks[i] = 0;
             if (pos < n_act) {
                 const int k = list[pos];
@@ -711,12 +756,12 @@ __global__ void __launch_bounds__(APPLY_THREADS) k_apply(Params p)
                     z.y -= d.y;
                     row[k] = z;
                     store_src<MODE>(slot_src, k, z);
-                    keep[i] = !(d2 < p.tol2);
+                    if (!(d2 < p.tol2)) kind[i] = (d2 < p.skip_below2) ? 2 : 1;
                 } else {                                // NaN / Inf: freeze where it is, report
                     atomicAdd(&p.state->degenerate, 1);
                 }
                 ks[i] = k;
-                cnt += keep[i] ? 1 : 0;
+                cnt += kind[i] == 1 ? 1 : (kind[i] == 2 ? (1 << 16) : 0);
             }
         }
         int incl = cnt;   // inclusive scan over the warp, then over the warps
@@ -739,14 +784,21 @@ __global__ void __launch_bounds__(APPLY_THREADS) k_apply(Params p)
             if (lane == 31) s_total = wi;
         }
         __syncthreads();
-        int off = base + s_warp[warp] + incl - cnt;
+        const int excl = s_warp[warp] + incl - cnt;
+        int off_l = base_l + (excl & 0xffff), off_s = base_s + (excl >> 16);
 #pragma unroll
-        for (int i = 0; i < APPLY_ITEMS; ++i)
-            if (keep[i]) next[off++] = ks[i];
-        base += s_total;
+        for (int i = 0; i < APPLY_ITEMS; ++i) {
+            if (kind[i] == 1) next[off_l++] = ks[i];
+            else if (kind[i] == 2) next[off_s++] = ks[i];
+        }
+        base_l += s_total & 0xffff;
+        base_s += s_total >> 16;
         __syncthreads();
     }
-    if (tid == 0) p.n_active[(st.cur ^ 1) * MAX_SLOTS + slot] = base;
+    if (tid == 0) {
+        p.n_active[(st.cur ^ 1) * MAX_SLOTS + slot] = base_s;
+        p.n_small[(st.cur ^ 1) * MAX_SLOTS + slot] = base_s - n_large;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -793,40 +845,52 @@ __device__ __forceinline__ long long block_scan(long long v, long long *total, l
 //   fine:   Tf = MLCC_FINE_FACTOR T threads per root for what is left of every slot's list, so the
 //           partial round is quantised in units of 1 / MLCC_FINE_FACTOR of a coarse tile.
 // Every thread returns with the same st.
-__device__ void build_tiles(const Params &p, DevState &st, long long *s_buf)
+__device__ void build_tiles_of(const Params &p, DevState &st, int K, int count, long long *s_buf)
 {
+    // count = this slot's roots for kernel K (0 for the threads beyond n_slots)
     const int s = threadIdx.x;
-    const int n_act = s < st.n_slots ? p.n_active[st.cur * MAX_SLOTS + s] : 0;
     long long total, W, tc_total, tf_total;
-    block_scan(n_act, &total, s_buf);
-    st.total_active = (int)total;
+    block_scan(count, &total, s_buf);
     int T = 1;
     while (T < CTA && total * T / (p.R * CTA) < 2LL * p.grid_ctas) T <<= 1;
     if (T < p.min_T) T = p.min_T;
     int Tf = T * MLCC_FINE_FACTOR;
     if (Tf > CTA) Tf = CTA;
     const int tile_c = p.R * CTA / T, tile_f = p.R * CTA / Tf;
-    block_scan(n_act / tile_c, &W, s_buf);   // coarse tiles if every slot were cut into coarse tiles only
+    block_scan(count / tile_c, &W, s_buf);   // coarse tiles if every slot were cut into coarse tiles only
     const long long C = (W / p.grid_ctas) * p.grid_ctas;   // whole rounds
-    const int c_s = (W > 0 && Tf != T) ? (int)((long long)(n_act / tile_c) * C / W) : 0;
-    const int f_s = (n_act - c_s * tile_c + tile_f - 1) / tile_f;
+    const int c_s = (W > 0 && Tf != T) ? (int)((long long)(count / tile_c) * C / W) : 0;
+    const int f_s = (count - c_s * tile_c + tile_f - 1) / tile_f;
     const long long tc = block_scan(c_s, &tc_total, s_buf);
     const long long tf = block_scan(f_s, &tf_total, s_buf);
-    int *tab_c = p.tile_start, *tab_f = p.tile_start + MAX_SLOTS + 1;
+    int *tab_c = p.tile_start + (2 * K) * (MAX_SLOTS + 1), *tab_f = tab_c + MAX_SLOTS + 1;
     if (s < st.n_slots) {
         tab_c[s] = (int)tc;
         tab_f[s] = (int)tf;
-        p.coarse_roots[s] = c_s * tile_c;
+        p.coarse_roots[K * MAX_SLOTS + s] = c_s * tile_c;
     }
     if (s == 0) {
         tab_c[st.n_slots] = (int)tc_total;
         tab_f[st.n_slots] = (int)tf_total;
     }
-    st.T = T;
-    st.Tf = Tf;
-    st.n_coarse = (int)tc_total;
-    st.n_tiles = (int)(tc_total + tf_total);
-    st.next_tile = 0;
+    TileSet &ts = st.ts[K];
+    ts.T = T;
+    ts.Tf = Tf;
+    ts.n_coarse = (int)tc_total;
+    ts.n_tiles = (int)(tc_total + tf_total);
+    ts.next_tile = 0;
+    ts.total = (int)total;
+}
+
+// both kernels' tile sets for the counts in n_active[cur] / n_small[cur]
+__device__ void build_tiles(const Params &p, DevState &st, long long *s_buf)
+{
+    const int s = threadIdx.x;
+    const int n_act = s < st.n_slots ? p.n_active[st.cur * MAX_SLOTS + s] : 0;
+    const int n_sm = s < st.n_slots ? p.n_small[st.cur * MAX_SLOTS + s] : 0;
+    build_tiles_of(p, st, 0, n_act - n_sm, s_buf);
+    build_tiles_of(p, st, 1, n_sm, s_buf);
+    st.total_active = st.ts[0].total + st.ts[1].total;
 }
 
 // The slots of step st.step: thread c looks after sub-chain c (n_sub <= MAX_SLOTS / 2); the slots keep the
@@ -855,6 +919,8 @@ __device__ void build_slots(const Params &p, DevState &st, long long *s_buf)
     if (threadIdx.x < st.n_slots) {
         p.n_active[st.cur * MAX_SLOTS + threadIdx.x] = p.n_r;
         p.n_active[(st.cur ^ 1) * MAX_SLOTS + threadIdx.x] = 0;
+        p.n_small[st.cur * MAX_SLOTS + threadIdx.x] = 0;      // a new row: every root gets the Aberth sum
+        p.n_small[(st.cur ^ 1) * MAX_SLOTS + threadIdx.x] = 0;
         p.slot_iters[threadIdx.x] = 0;
     }
     st.iter = 0;
@@ -894,8 +960,9 @@ __global__ void __launch_bounds__(FIN) k_init(Params p)
     __shared__ long long s_buf[33];
     DevState st;
     st.step = 0; st.iter = 0; st.n_slots = 0; st.done = 0; st.need_seed = 1; st.cur = 0;
-    st.T = 1; st.Tf = 1; st.n_coarse = 0; st.n_tiles = 0; st.next_tile = 0; st.total_active = 0; st.total_iterations = 0;
-    st.unconverged_rows = 0; st.degenerate = 0; st.n_outside = 0; st.root_iterations = 0; st.launches_used = 0;
+    st.ts[0] = TileSet{1, 1, 0, 0, 0, 0}; st.ts[1] = TileSet{1, 1, 0, 0, 0, 0};
+    st.total_active = 0; st.total_iterations = 0;
+    st.unconverged_rows = 0; st.degenerate = 0; st.n_outside = 0; st.root_iterations_noA = 0; st.root_iterations = 0; st.launches_used = 0;
     build_slots(p, st, s_buf);
     build_tiles(p, st, s_buf);
     if (threadIdx.x == 0) *p.state = st;
@@ -911,6 +978,7 @@ __global__ void __launch_bounds__(FIN) k_finalize(Params p)
     st.iter += 1;
     st.total_iterations += 1;
     st.root_iterations += st.total_active;
+    st.root_iterations_noA += st.ts[1].total;
     st.launches_used += 1;
     st.need_seed = 0;
     st.n_outside = 0;
@@ -947,33 +1015,32 @@ struct KernelSet {
     void (*prepare)(Params);
     void (*seed)(Params);
     void (*compute)(Params);
+    void (*compute_noA)(Params);   // the variant without the Aberth sum, for the roots whose last step was small
     void (*apply)(Params);
     int R;   // roots per thread of `compute`
 };
 
-KernelSet kernel_set(int mode, bool caus, bool fmm)
+template <int MODE>
+KernelSet kernel_set_mode(bool caus, bool fmm)
 {
+    constexpr int RR = MODE == MODE_F64 ? R_ROOTS_F64 : R_ROOTS_F32;
     KernelSet k;
-    if (mode == MODE_F64) {
-        k.prepare = k_prepare<MODE_F64>; k.seed = k_seed<MODE_F64>; k.apply = k_apply<MODE_F64>;
-        if (fmm) {
-            k.compute = caus ? k_compute<MODE_F64, true, false, R_ROOTS_F64> : k_compute<MODE_F64, false, false, R_ROOTS_F64>;
-            k.R = R_ROOTS_F64;
-        } else {
-            k.compute = caus ? k_compute<MODE_F64, true, true, R_STARS> : k_compute<MODE_F64, false, true, R_STARS>;
-            k.R = R_STARS;
-        }
+    k.prepare = k_prepare<MODE>; k.seed = k_seed<MODE>; k.apply = k_apply<MODE>;
+    if (fmm) {
+        k.compute = caus ? k_compute<MODE, true, false, true, RR> : k_compute<MODE, false, false, true, RR>;
+        k.compute_noA = caus ? k_compute<MODE, true, false, false, RR> : k_compute<MODE, false, false, false, RR>;
+        k.R = RR;
     } else {
-        k.prepare = k_prepare<MODE_F32>; k.seed = k_seed<MODE_F32>; k.apply = k_apply<MODE_F32>;
-        if (fmm) {
-            k.compute = caus ? k_compute<MODE_F32, true, false, R_ROOTS_F32> : k_compute<MODE_F32, false, false, R_ROOTS_F32>;
-            k.R = R_ROOTS_F32;
-        } else {
-            k.compute = caus ? k_compute<MODE_F32, true, true, R_STARS> : k_compute<MODE_F32, false, true, R_STARS>;
-            k.R = R_STARS;
-        }
+        k.compute = caus ? k_compute<MODE, true, true, true, R_STARS> : k_compute<MODE, false, true, true, R_STARS>;
+        k.compute_noA = caus ? k_compute<MODE, true, true, false, R_STARS> : k_compute<MODE, false, true, false, R_STARS>;
+        k.R = R_STARS;
     }
     return k;
+}
+
+KernelSet kernel_set(int mode, bool caus, bool fmm)
+{
+    return mode == MODE_F64 ? kernel_set_mode<MODE_F64>(caus, fmm) : kernel_set_mode<MODE_F32>(caus, fmm);
 }
 
 }  // namespace
@@ -1037,6 +1104,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     if (opt.aberth_sum_precision != 0 && opt.aberth_sum_precision != 32 && opt.aberth_sum_precision != 64)
         return invalid("aberth_sum_precision must be 0, 32 or 64");
     const int mode = opt.aberth_sum_precision == 64 ? MODE_F64 : MODE_F32;
+    if (!isfinite(opt.skip_aberth_sum_below)) return invalid("skip_aberth_sum_below");
     if (opt.star_sum_mode != MLCC_STAR_SUMS_DIRECT && opt.star_sum_mode != MLCC_STAR_SUMS_FMM)
         return invalid("star_sum_mode");
 
@@ -1099,8 +1167,9 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
         (e = ws.alloc(&p.slot_dir, MAX_SLOTS)) != cudaSuccess ||
         (e = ws.alloc(&p.slot_iters, MAX_SLOTS)) != cudaSuccess ||
         (e = ws.alloc(&p.n_active, 2 * MAX_SLOTS)) != cudaSuccess ||
-        (e = ws.alloc(&p.tile_start, 2 * (MAX_SLOTS + 1))) != cudaSuccess ||
-        (e = ws.alloc(&p.coarse_roots, MAX_SLOTS)) != cudaSuccess ||
+        (e = ws.alloc(&p.tile_start, 4 * (MAX_SLOTS + 1))) != cudaSuccess ||
+        (e = ws.alloc(&p.coarse_roots, 2 * MAX_SLOTS)) != cudaSuccess ||
+        (e = ws.alloc(&p.n_small, 2 * MAX_SLOTS)) != cudaSuccess ||
         (e = ws.alloc(&p.list, (size_t)2 * max_slots * n_r)) != cudaSuccess ||
         (e = ws.alloc(&p.delta, (size_t)max_slots * n_r)) != cudaSuccess) {
         if (e == cudaErrorMemoryAllocation) {
@@ -1117,6 +1186,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     MLCC_CUDA(cudaMemcpyAsync(d_plan, plan.data(), sizeof(long long) * plan.size(),
                               cudaMemcpyHostToDevice, stream));
     MLCC_CUDA(cudaMemsetAsync(p.n_active, 0, sizeof(int) * 2 * MAX_SLOTS, stream));
+    MLCC_CUDA(cudaMemsetAsync(p.n_small, 0, sizeof(int) * 2 * MAX_SLOTS, stream));
 
     // input check (one small read-back before the solve)
     {
@@ -1158,6 +1228,9 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     p.min_T = min_T;
     p.grid_ctas = grid_compute;
     p.R = ks.R;
+    const double skip_below = opt.skip_aberth_sum_below == 0.0 ? 1e-8 : opt.skip_aberth_sum_below;
+    const bool skip_on = skip_below > 0.0;
+    p.skip_below2 = skip_on ? skip_below * skip_below : 0.0;
     p.poly_n = poly_n;
     p.seed_radius = opt.seed_radius;
     if (poly_n > 0) {
@@ -1222,10 +1295,11 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
                 k_star_sums_outside<<<sms, BLOCK, 0, stream>>>(p);
             }
             ks.compute<<<grid_compute, CTA, 0, stream>>>(p);
+            if (skip_on) ks.compute_noA<<<grid_compute, CTA, 0, stream>>>(p);
             ks.apply<<<grid_apply, APPLY_THREADS, 0, stream>>>(p);
             k_finalize<<<1, FIN, 0, stream>>>(p);
         }
-        launches += (use_fmm ? 6 : 4) * chunk;
+        launches += ((use_fmm ? 6 : 4) + (skip_on ? 1 : 0)) * chunk;
         groups += chunk;
         cudaMemcpyAsync(&h_state[which], p.state, sizeof(DevState), cudaMemcpyDeviceToHost, stream);
         cudaEventRecord(ev_poll[which], stream);
@@ -1259,7 +1333,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     if (out_stats) {
         out_stats->root_iterations = fin.root_iterations;
         out_stats->star_pairs = fin.root_iterations * N;
-        out_stats->root_pairs = fin.root_iterations * (n_r - 1);
+        out_stats->root_pairs = (fin.root_iterations - fin.root_iterations_noA) * (n_r - 1);
         out_stats->kernel_launches = launches;
         out_stats->total_iterations = fin.total_iterations;
         out_stats->steps = max_steps + 1;

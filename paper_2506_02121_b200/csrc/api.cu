@@ -153,6 +153,7 @@ void mlcc_options_default(mlcc_options *opt)
     opt->sheet_poly_n = 0;
     opt->reserved2_ = 0;
     opt->seed_radius = 0.0;
+    opt->skip_aberth_sum_below = 0.0;
 }
 
 int mlcc_star_field(uint64_t seed, int64_t N, double kappa_star, int mass_model, const double *mass_params,

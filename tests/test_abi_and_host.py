@@ -44,7 +44,7 @@ def test_version_and_status_strings(lib):
 def test_options_default_and_struct_layout(lib):
     from paper_2506_02121_b200 import api
     o = api.options()
-    assert o.struct_size == C.sizeof(api.mlcc_options) == 80
+    assert o.struct_size == C.sizeof(api.mlcc_options) == 88
     assert o.predictor_order == -1 and o.num_subchains == 0 and o.phi_index_total == 0
     assert C.sizeof(api.mlcc_stats) == 64
 

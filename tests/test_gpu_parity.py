@@ -624,3 +624,33 @@ def test_rectangular_field_argument_checks(api):
     b, _, _, _ = api.critical_curves_ex(xy, m, 0.0, 0.07, 4)
     err, bij = api.match_root_sets(a, b, 1e-12)
     assert a.shape == b.shape and bool(bij.all())
+
+
+def test_confirm_iterations_without_the_aberth_sum(api, orc):
+    """DESIGN.md reading R27: once every step of an iteration was below skip_aberth_sum_below, the next iteration of
+    the row leaves A out.  Same root sets (the fixed point F = 0 does not involve A), same iteration counts, fewer
+    (root, root) pairs; a negative threshold restores the Aberth sum in every iteration."""
+    cfg = CONFIGS["cfg3"]
+    xy, m, R = field(orc, cfg)
+    num_phi = 400
+    rows = np.array([0, 57, 200, 399])
+    ref, _, un = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, num_phi, rows, cfg.tol, cfg.max_iter)
+    assert un.sum() == 0
+    out = {}
+    for name, thr in (("default", 0.0), ("never", -1.0), ("loose", 1e-5)):
+        for mode in (api.MLCC_STAR_SUMS_DIRECT, api.MLCC_STAR_SUMS_FMM):
+            r, it, unc, st = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, num_phi, cfg.tol,
+                                                    cfg.max_iter, opt=api.options(skip_aberth_sum_below=thr,
+                                                                                  star_sum_mode=mode))
+            assert int(unc.sum()) == 0 and st.degenerate_roots == 0
+            assert_rows_match(orc, r.cpu().numpy()[rows], ref)
+            out[(name, mode)] = (r, it, st)
+    n_r = 2 * cfg.N
+    for mode in (api.MLCC_STAR_SUMS_DIRECT, api.MLCC_STAR_SUMS_FMM):
+        never, default, loose = (out[(k, mode)][2] for k in ("never", "default", "loose"))
+        assert never.root_pairs == never.root_iterations * (n_r - 1)
+        assert default.root_pairs < 0.95 * default.root_iterations * (n_r - 1)
+        assert loose.root_pairs <= default.root_pairs
+        assert abs(default.root_iterations - never.root_iterations) <= 0.01 * never.root_iterations
+        err, bij = api.match_root_sets(out[("default", mode)][0], out[("never", mode)][0], 1e-13)
+        assert bool(bij.all())

@@ -174,8 +174,16 @@ def check_row_invariants(orc, xy, m, kappa_s, gamma, row_index, num_phi, z, min_
     res = orc.residuals(xy, m, kappa_s, gamma, row_index, num_phi,
                         np.stack([z.real, z.imag], axis=1), long_double=True)
     ulp = np.spacing(np.abs(z))
-    # residual certificate: the long-double Newton step from the fp64 root is at rounding level
-    assert np.all(res["newton"] <= 4 * ulp + 1e-13), res["newton"].max()
+    # residual certificate: the long-double Newton step from the fp64 root is at rounding level.  "Rounding level" is
+    # the spacing of z, or -- for an ill-conditioned root (small |F'|) -- what the fp64 evaluation of F itself allows:
+    # F is a sum of N terms m_i/(z-z_i)^2, each term and each addition rounded, so |dF| ~ a few 2^-53 sum |terms| and
+    # the root cannot be placed better than |dF|/|F'| (reading R16; cfg4 has roots with |F'| ~ 1e-3).
+    plain = 4 * ulp + 1e-13
+    over = np.where(res["newton"] > plain)[0]          # only these need the conditioning term (few, if any)
+    for k in over:
+        floor = 8 * 2.0 ** -53 * (m / np.abs(z[k] - zs) ** 2).sum() / np.abs(res["Fp"][k])
+        assert res["newton"][k] <= plain[k] + floor, (k, res["newton"][k], plain[k], floor)
+    assert len(over) <= max(2, len(z) // 1000)
     # scaled det J bound (App. C linearised)
     bound = 1e-10 + 4 * (1 - kappa_s) * np.abs(res["Fp"]) * 2.0 ** -52 * (1 + np.abs(z))
     assert np.all(np.abs(res["inv_mu"]) <= bound), (np.abs(res["inv_mu"]) / bound).max()
