@@ -25,12 +25,17 @@ inline int invalid(const char *msg)
     return MLCC_ERR_INVALID_ARG;
 }
 
+// The stream-ordered allocator gives freed memory back to the driver at every synchronisation unless told
+// otherwise, and every call here would then pay for fresh device allocations (hundreds of ms for the GB-sized
+// scratch of the matcher): raise the device pool's release threshold once per device.
+void keep_pool_memory();
+
 // Stream-ordered workspace that frees itself (cudaFreeAsync) when it goes out of scope.
 struct Workspace {
     cudaStream_t stream;
     void *ptrs[48];
     int n = 0;
-    explicit Workspace(cudaStream_t s) : stream(s) {}
+    explicit Workspace(cudaStream_t s) : stream(s) { keep_pool_memory(); }
     ~Workspace()
     {
         for (int i = n - 1; i >= 0; --i) cudaFreeAsync(ptrs[i], stream);
