@@ -213,7 +213,10 @@ static int match_launch(const double *a, const double *b, int64_t S, int64_t n, 
     const long long ncell = (long long)G * G;
     const long long stride = (ncell + 1) + ncell + 2 * n;
     const int sms = device_sm_count();
-    long long grid = 2ll * sms;
+    // latency-bound CTAs (global-memory counting sort and ring search): as many as stay resident
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_match, BLOCK, 0) != cudaSuccess || per_sm < 1) per_sm = 2;
+    long long grid = (long long)per_sm * sms;
     if (grid > S) grid = S;
     Workspace ws(stream);
     int *scratch = nullptr;

@@ -654,3 +654,37 @@ def test_confirm_iterations_without_the_aberth_sum(api, orc):
         assert abs(default.root_iterations - never.root_iterations) <= 0.01 * never.root_iterations
         err, bij = api.match_root_sets(out[("default", mode)][0], out[("never", mode)][0], 1e-13)
         assert bool(bij.all())
+
+
+def test_crossing_map_full_size_cfg4_sampled_pixels(api, orc):
+    """cfg4 at its full size (10^4 phases x 2*10^4 roots = 2*10^8 caustic segments, far-field star sums for speed):
+    chains joined on the GPU, 2048^2 map, and a 4 x 4 sample of its pixels recomputed one by one by the oracle's
+    per-pixel winding sum over all segments of the GPU's own caustic points."""
+    cfg = CONFIGS["cfg4"]
+    xy, m, R = field(orc, cfg)
+    opt = api.options(star_sum_mode=api.MLCC_STAR_SUMS_FMM)
+    roots, caus, iters, unconv, st = api.curves_and_caustics(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, cfg.num_phi,
+                                                             cfg.tol, cfg.max_iter, opt=opt, want_diagnostics=False)
+    assert st.unconverged_rows == 0 and st.degenerate_roots == 0
+    nxt, bij = api.link_rows(roots)
+    n_bad = int((bij == 0).sum())
+    assert n_bad <= 5, n_bad                       # rows where two roots are closer than their step in phi (reported)
+    n_pix, half = 2048, 30.0
+    pixel = 2 * half / n_pix
+    cmap = api.crossing_map(caus, nxt, -half, -half, pixel, n_pix, n_pix)
+    assert int(cmap.min()) >= -1 and int(cmap.max()) >= 3
+    # sample: three pixels of every count 0..3, each recomputed by the oracle as a 1 x 1 map centred on that pixel
+    g_caus, g_nxt, g_map = caus.cpu().numpy(), nxt.cpu().numpy(), cmap.cpu().numpy()
+    rng = np.random.default_rng(6)
+    checked = 0
+    for value in range(4):
+        iy, ix = np.nonzero(g_map == value)
+        assert len(iy) > 0, value
+        for q in rng.choice(len(iy), size=3, replace=False):
+            x0s, y0s = -half + ix[q] * pixel, -half + iy[q] * pixel
+            ref, amb = orc.crossing_map(g_caus, g_nxt, x0s, y0s, pixel, 1, 1, want_ambiguous=True)
+            if amb[0, 0]:
+                continue
+            assert ref[0, 0] == value, (ix[q], iy[q], value, ref[0, 0])
+            checked += 1
+    assert checked >= 10
