@@ -47,6 +47,9 @@ def lib():
         L.orc_link_rows.argtypes = [_pd, C.c_int64, C.c_int64, _pi32, _pi32]
         L.orc_crossing_map.argtypes = [_pd, C.c_void_p, C.c_int64, C.c_int64, C.c_double, C.c_double, C.c_double,
                                        C.c_int32, C.c_int32, _pi32, C.c_void_p]
+        L.orc_closed_loops.argtypes = [_pi32, C.c_int64, C.c_int64, C.c_void_p, _pi32, _pi32, _pi32]
+        L.orc_distance_map.argtypes = [_pi32, C.c_int32, C.c_int32, C.c_double, _pd, _pi64]
+        L.orc_directional_distance_map.argtypes = [_pi32, C.c_int32, C.c_int32, C.c_double, C.c_int32, C.c_int32, _pd]
         L.orc_star_field.argtypes = [C.c_uint64, C.c_int64, C.c_double, C.c_int, C.c_void_p,
                                      _pd, _pd, C.POINTER(C.c_double)]
         L.orc_philox4x32_10.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32),
@@ -193,6 +196,39 @@ def crossing_map(caustics, nxt, x0, y0, pixel, nx, ny, want_ambiguous=False):
                                   float(pixel), int(nx), int(ny), out, None if amb is None else amb.ctypes.data),
            "crossing_map")
     return (out, amb) if want_ambiguous else out
+
+
+def closed_loops(nxt, want_chain_col=True):
+    """nxt [S,n] int32 (link_rows) -> dict(chain_col [S,n] or None, chain_end [n], loop_id [n], num_loops)."""
+    nxt = np.ascontiguousarray(nxt, np.int32)
+    S, n = nxt.shape
+    col = np.empty((S, n), np.int32) if want_chain_col else None
+    end = np.empty(n, np.int32)
+    lid = np.empty(n, np.int32)
+    cnt = np.zeros(1, np.int32)
+    _check(lib().orc_closed_loops(nxt, S, n, None if col is None else col.ctypes.data, end, lid, cnt), "closed_loops")
+    return {"chain_col": col, "chain_end": end, "loop_id": lid, "num_loops": int(cnt[0])}
+
+
+def distance_map(cmap, pixel):
+    """crossing map [ny,nx] int32 -> (distance to the nearest caustic pixel [ny,nx] f64, squared distance in pixels int64)."""
+    cmap = np.ascontiguousarray(cmap, np.int32)
+    ny, nx = cmap.shape
+    out = np.empty((ny, nx), _d)
+    d2 = np.empty((ny, nx), np.int64)
+    _check(lib().orc_distance_map(cmap, nx, ny, float(pixel), out, d2), "distance_map")
+    return out, d2
+
+
+def directional_distance_map(cmap, pixel, ux, uy):
+    """crossing map [ny,nx] int32, integer direction (ux, uy) -> signed distance along the ray [ny,nx] f64
+    (negative: the ray left the map first, |value| = distance to the exit point)."""
+    cmap = np.ascontiguousarray(cmap, np.int32)
+    ny, nx = cmap.shape
+    out = np.empty((ny, nx), _d)
+    _check(lib().orc_directional_distance_map(cmap, nx, ny, float(pixel), int(ux), int(uy), out),
+           "directional_distance_map")
+    return out
 
 
 def rect_sheet(kappa_star, c1, c2, t, points):

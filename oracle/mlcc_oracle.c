@@ -13,7 +13,9 @@
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): Einstein ring, Chang–Refsdal closed form and
  * cusp positions, equal-mass binary closed form, companion-matrix eigenvalues (N <= 6),
  * Vieta sums, det J, long-double residual certificates, continuity in phi, outer root pair,
- * Philox known-answer vectors, generator statistics.
+ * Philox known-answer vectors, generator statistics; closed loops by the binary-lens topologies and the
+ * Einstein ring / Chang-Refsdal chain structure; distance maps by scipy's Euclidean distance transform,
+ * a disc, and hand-worked rays (tests/test_oracle_loops_distance.py).
  * Parity unpinned: the mass functions and star positions "of the paper's fields" (the paper
  * publishes neither); both sides consume the same generated arrays.
  *
@@ -511,6 +513,179 @@ int orc_crossing_map(const double *caustics, const int32_t *next, int64_t S, int
         }
         out_map[pix] = -wn;
         if (out_ambiguous) out_ambiguous[pix] = (uint8_t)amb;
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Chains and closed loops ("Every one of the initial n_r roots begins and ends a
+ * 'chain' of values from 0 to 2 pi ... sometimes 2 or more chains are needed to fully create a closed
+ * critical curve"; fn. 5 at :217: "the start of one chain is the end of another, with chains joining
+ * together until closed loops are formed").  `next` is the successor table of orc_link_rows.
+ * Chain k is the one that starts in column k of row 0; written as the definition:
+ *   chain_col[0][k] = k,  chain_col[s+1][k] = next[s][chain_col[s][k]],
+ *   chain_end[k]    = next[S-1][chain_col[S-1][k]]   (the column of row 0 the chain arrives at after
+ *                     the whole turn of phi: the start of the chain that continues it),
+ *   loop_id[k]      = the smallest chain index met by walking k -> chain_end[k] -> ... back to k,
+ *   num_loops       = number of distinct loop_id values.
+ * A chain that meets an entry outside [0, n) gets -1 from there on, chain_end = -1 and loop_id = -1;
+ * so does a chain whose walk does not return to it within n steps (chain_end not a bijection).
+ * out_chain_col may be NULL.
+ * ---------------------------------------------------------------------------------------- */
+int orc_closed_loops(const int32_t *next, int64_t S, int64_t n, int32_t *out_chain_col,
+                     int32_t *out_chain_end, int32_t *out_loop_id, int32_t *out_num_loops)
+{
+    if (S < 1 || n < 1) return -2;
+    for (int64_t k = 0; k < n; ++k) {
+        int64_t c = k;
+        for (int64_t s = 0; s < S; ++s) {
+            if (out_chain_col) out_chain_col[s * n + k] = (int32_t)c;
+            if (c >= 0) {
+                c = next[s * n + c];
+                if (c < 0 || c >= n) c = -1;
+            }
+        }
+        out_chain_end[k] = (int32_t)c;
+    }
+    int32_t loops = 0;
+    for (int64_t k = 0; k < n; ++k) {
+        int64_t c = k, smallest = k, steps = 0;
+        int closed = 0;
+        while (steps < n) {
+            c = out_chain_end[c];
+            ++steps;
+            if (c < 0) break;
+            if (c == k) { closed = 1; break; }
+            if (c < smallest) smallest = c;
+        }
+        out_loop_id[k] = closed ? (int32_t)smallest : -1;
+        if (closed && smallest == k) ++loops;
+    }
+    *out_num_loops = loops;
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Distance to the nearest caustic for an expanding source (Section 5.2, Fig. 5 top):
+ * "the distance from each pixel to the nearest caustic ... calculated from the map of N_caustic
+ * crossings using a Euclidean distance transform".  Reading (R28): a pixel is a caustic
+ * pixel if one of its 4 neighbours inside the map holds a different count; the distance of pixel p is
+ * pixel * min over caustic pixels q of |p - q| (centre to centre, 0 on a caustic pixel), +inf if the map
+ * has no caustic pixel.  Brute force over all pairs, squared distances in integers.
+ * out_d2 (may be NULL): the squared distance in pixels as int64 (-1 for +inf).
+ * ---------------------------------------------------------------------------------------- */
+static int caustic_pixel(const int32_t *map, int64_t nx, int64_t ny, int64_t x, int64_t y)
+{
+    const int32_t v = map[y * nx + x];
+    if (x > 0 && map[y * nx + x - 1] != v) return 1;
+    if (x + 1 < nx && map[y * nx + x + 1] != v) return 1;
+    if (y > 0 && map[(y - 1) * nx + x] != v) return 1;
+    if (y + 1 < ny && map[(y + 1) * nx + x] != v) return 1;
+    return 0;
+}
+
+int orc_distance_map(const int32_t *map, int32_t nx, int32_t ny, double pixel, double *out, int64_t *out_d2)
+{
+    if (nx < 1 || ny < 1 || !(pixel > 0.0)) return -2;
+    const int64_t P = (int64_t)nx * ny;
+    uint8_t *edge = (uint8_t *)malloc((size_t)P);
+    for (int64_t y = 0; y < ny; ++y)
+        for (int64_t x = 0; x < nx; ++x) edge[y * nx + x] = (uint8_t)caustic_pixel(map, nx, ny, x, y);
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t p = 0; p < P; ++p) {
+        const int64_t py = p / nx, px = p % nx;
+        int64_t best = -1;
+        for (int64_t qy = 0; qy < ny; ++qy)
+            for (int64_t qx = 0; qx < nx; ++qx) {
+                if (!edge[qy * nx + qx]) continue;
+                const int64_t d2 = (px - qx) * (px - qx) + (py - qy) * (py - qy);
+                if (best < 0 || d2 < best) best = d2;
+            }
+        if (out_d2) out_d2[p] = best;
+        out[p] = best < 0 ? INFINITY : pixel * sqrt((double)best);
+    }
+    free(edge);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Distance to the nearest caustic for a source moving along a direction (Fig. 5
+ * bottom, Fig. 6-7).  Reading (R29): the direction is the integer vector u = (ux, uy); the ray
+ * starts at the centre of pixel p; the caustic is met where the ray first enters (the open interior
+ * of) a pixel whose count differs from that of p; the distance is from the centre of p to that entry
+ * point.  If the ray leaves the map first, the value is MINUS the distance to the exit point: a lower
+ * bound only ("the border of the map is a boundary that can be hit in the distance algorithms despite
+ * not being a caustic", Fig. 5 caption at PAPER.md:245).
+ * Written as the definition: for each pixel p a loop over every other pixel q with a different count,
+ * ray/square intersection by the slab rule in exact rational arithmetic (coordinates doubled so that
+ * centres are even and pixel borders odd integers), the smallest entry parameter wins.
+ * ---------------------------------------------------------------------------------------- */
+typedef struct { int64_t num, den; } orc_rat;            /* den > 0;  +-inf as (+-1, 0) */
+static int rat_lt(orc_rat a, orc_rat b)                   /* a < b */
+{
+    if (a.den == 0 && b.den == 0) return a.num < b.num;
+    if (a.den == 0) return a.num < 0;
+    if (b.den == 0) return b.num > 0;
+    return a.num * b.den < b.num * a.den;
+}
+static orc_rat rat_make(int64_t num, int64_t den)
+{
+    orc_rat r;
+    if (den < 0) { num = -num; den = -den; }
+    r.num = num; r.den = den;
+    return r;
+}
+/* parameter interval (lo, hi) of o + t u inside the open slab (a, b) along one axis; returns 0 if empty */
+static int slab(int64_t o, int64_t u, int64_t a, int64_t b, orc_rat *lo, orc_rat *hi)
+{
+    if (u == 0) {
+        if (!(a < o && o < b)) return 0;
+        *lo = rat_make(-1, 0); *hi = rat_make(1, 0);
+        return 1;
+    }
+    orc_rat ta = rat_make(a - o, u), tb = rat_make(b - o, u);
+    if (rat_lt(tb, ta)) { orc_rat t = ta; ta = tb; tb = t; }
+    *lo = ta; *hi = tb;
+    return 1;
+}
+
+int orc_directional_distance_map(const int32_t *map, int32_t nx, int32_t ny, double pixel, int32_t ux, int32_t uy,
+                                 double *out)
+{
+    if (nx < 1 || ny < 1 || !(pixel > 0.0) || (ux == 0 && uy == 0)) return -2;
+    const int64_t P = (int64_t)nx * ny;
+    const double ulen = sqrt((double)((int64_t)ux * ux + (int64_t)uy * uy));
+    const orc_rat zero = rat_make(0, 1);
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t p = 0; p < P; ++p) {
+        const int64_t py = p / nx, px = p % nx;
+        const int64_t ox = 2 * px, oy = 2 * py;
+        const int32_t v = map[p];
+        int found = 0;
+        orc_rat best = rat_make(1, 0);
+        for (int64_t qy = 0; qy < ny; ++qy)
+            for (int64_t qx = 0; qx < nx; ++qx) {
+                if (map[qy * nx + qx] == v) continue;
+                orc_rat xl, xh, yl, yh;
+                if (!slab(ox, ux, 2 * qx - 1, 2 * qx + 1, &xl, &xh)) continue;
+                if (!slab(oy, uy, 2 * qy - 1, 2 * qy + 1, &yl, &yh)) continue;
+                const orc_rat enter = rat_lt(xl, yl) ? yl : xl;      /* max of the lows  */
+                const orc_rat leave = rat_lt(xh, yh) ? xh : yh;      /* min of the highs */
+                if (!rat_lt(enter, leave)) continue;                   /* touches a corner or misses */
+                if (!rat_lt(zero, leave)) continue;                    /* behind the start */
+                if (!rat_lt(zero, enter)) continue;                    /* q == p cannot happen (same count) */
+                if (!found || rat_lt(enter, best)) { best = enter; found = 1; }
+            }
+        if (found) {
+            out[p] = pixel * 0.5 * ulen * ((double)best.num / (double)best.den);
+        } else {
+            /* exit point of the map rectangle (-1, 2 nx - 1) x (-1, 2 ny - 1) */
+            orc_rat xl, xh, yl, yh;
+            slab(ox, ux, -1, 2 * (int64_t)nx - 1, &xl, &xh);
+            slab(oy, uy, -1, 2 * (int64_t)ny - 1, &yl, &yh);
+            const orc_rat leave = rat_lt(xh, yh) ? xh : yh;
+            out[p] = -(pixel * 0.5 * ulen * ((double)leave.num / (double)leave.den));
+        }
     }
     return 0;
 }
