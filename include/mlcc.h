@@ -253,6 +253,58 @@ int mlcc_crossing_map(const double *caustics, const int32_t *next, int64_t S, in
                       double x0, double y0, double pixel, int32_t nx, int32_t ny, int32_t *out_map,
                       void *stream);
 
+/* (f) NEXT-4, second part: chains and closed loops ("Every one of the initial n_r roots
+ * begins and ends a 'chain' of values from 0 to 2 pi ... sometimes 2 or more chains are needed to fully
+ * create a closed critical curve"; fn. 5 at :217: "the start of one chain is the end of another, with
+ * chains joining together until closed loops are formed").  Chain k is the one that starts in column
+ * k of row 0:  chain_col[0][k] = k,  chain_col[s+1][k] = next[s][chain_col[s][k]].
+ *   next [S][n]: device int32, read: mlcc_link_rows of the roots (closed: row S-1 links to row 0).
+ *   out_chain_col [S][n]: device int32 or NULL, written: the column of row s that holds chain k.
+ *   out_chain_end [n]: device int32, written: next[S-1][chain_col[S-1][k]], the column of row 0 where
+ *     chain k arrives after the whole turn of phi, i.e. the chain that continues it.
+ *   out_loop_id [n]: device int32, written: the smallest chain index on the cycle of
+ *     k -> out_chain_end[k] through k; chains with equal ids form one closed critical curve.
+ *   out_num_loops [1]: device int32, written: the number of closed loops.
+ * A chain that meets an entry outside [0, n) (a row mlcc_link_rows marked -1) has -1 from there on,
+ * out_chain_end = -1 and out_loop_id = -1; so has every chain that does not lie on a cycle (possible
+ * only if some row of `next` is not a bijection).  Integer work: results are exact.
+ * Asynchronous on `stream`.  Errors: INVALID_ARG, CUDA, NOMEM.                                    */
+int mlcc_closed_loops(const int32_t *next, int64_t S, int64_t n, int32_t *out_chain_col,
+                      int32_t *out_chain_end, int32_t *out_loop_id, int32_t *out_num_loops,
+                      void *stream);
+
+/* Rows put into chain order (the paper's (m+1, n_r) matrix whose column is a chain):
+ * out[s][k] = points[s][chain_col[s][k]] (NaN where chain_col is outside [0, n)).  Use it on the roots
+ * and on the caustic points alike.  points, out [S][n][2]: device, must not overlap; chain_col [S][n]:
+ * device int32 (mlcc_closed_loops).  Asynchronous on `stream`.  Errors: INVALID_ARG, CUDA.         */
+int mlcc_order_by_chain(const double *points, const int32_t *chain_col, int64_t S, int64_t n,
+                        double *out, void *stream);
+
+/* (f) NEXT-4, third part: distance from every source pixel to the nearest caustic for an expanding
+ * source (Section 5.2, Fig. 5 top: "calculated from the map of N_caustic crossings
+ * using a Euclidean distance transform").  A pixel is a caustic pixel if one of its 4 neighbours
+ * inside the map holds a different count (reading R28);
+ *   out_distance[iy][ix] = pixel * min over caustic pixels q of |p - q|  (centre to centre; 0 on a
+ *   caustic pixel; +inf if the map has no caustic pixel).  The border of the map is not a caustic
+ *   (caption of Fig. 5): a value larger than the pixel's distance to the border is a lower bound only.
+ *   crossing_map [ny][nx]: device int32, read (out_map of mlcc_crossing_map, or any integer map).
+ *   out_distance [ny][nx]: device double, written.
+ *   out_d2 [ny][nx]: device int64 or NULL, written: the squared distance in pixels, exact (-1 for +inf).
+ * Asynchronous on `stream`.  Errors: INVALID_ARG, CUDA, NOMEM.                                    */
+int mlcc_distance_map(const int32_t *crossing_map, int32_t nx, int32_t ny, double pixel,
+                      double *out_distance, int64_t *out_d2, void *stream);
+
+/* The same for a source moving along a direction (Fig. 5 bottom, Fig. 6-7).  The
+ * direction is the integer vector (ux, uy), not both zero, |ux|, |uy| <= 2^20 (angle atan2(uy, ux)
+ * with the y_1 axis; reading R29).  The ray from the centre of pixel p is followed through
+ * the pixel grid exactly, to the point where it first enters the interior of a pixel whose count
+ * differs from that of p; out_distance is the distance from the centre of p to that point.  If the
+ * ray leaves the map first, out_distance is MINUS the distance to the exit point (a lower bound).
+ *   crossing_map [ny][nx]: device int32, read.  out_distance [ny][nx]: device double, written.
+ * Asynchronous on `stream`.  Errors: INVALID_ARG, CUDA.                                           */
+int mlcc_directional_distance_map(const int32_t *crossing_map, int32_t nx, int32_t ny, double pixel,
+                                  int32_t ux, int32_t uy, double *out_distance, void *stream);
+
 /* (f) NEXT-3: the rectangular sheet of Appendix B as a polynomial (host-only, no CUDA call).
  * For stars in the rectangle with corner c = c1 + i c2 and smooth compensation kappa_star, Eq. B2
  * truncated at the odd power t and extended to an infinite sheet is

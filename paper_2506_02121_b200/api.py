@@ -100,6 +100,10 @@ def lib() -> C.CDLL:
         L.mlcc_rect_sheet.argtypes = [dbl, dbl, dbl, dbl, dbl, i32, vp, i32, C.POINTER(dbl)]
         L.mlcc_link_rows.argtypes = [vp, i64, i64, vp, vp, vp]
         L.mlcc_crossing_map.argtypes = [vp, vp, i64, i64, C.c_int, dbl, dbl, dbl, i32, i32, vp, vp]
+        L.mlcc_closed_loops.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp]
+        L.mlcc_order_by_chain.argtypes = [vp, vp, i64, i64, vp, vp]
+        L.mlcc_distance_map.argtypes = [vp, i32, i32, dbl, vp, vp, vp]
+        L.mlcc_directional_distance_map.argtypes = [vp, i32, i32, dbl, i32, i32, vp, vp]
         L.mlcc_star_sums.argtypes = [vp, vp, i64, vp, i64, C.c_int, C.c_int, C.c_int, vp, vp]
         L.mlcc_plan_subchains.argtypes = [i64, i64, i32, i32, vp, vp, vp]
         L.mlcc_critical_curves_host.argtypes = [vp, vp, i64, dbl, dbl, i64, dbl, i32, vp]
@@ -305,6 +309,65 @@ def crossing_map(caustics, nxt, x0, y0, pixel, nx, ny, closed=True):
     rc = lib().mlcc_crossing_map(_dev(caustics, name="caustics"), _dev(nxt, torch.int32, "nxt"), S, n,
                                  1 if closed else 0, float(x0), float(y0), float(pixel), int(nx), int(ny),
                                  out.data_ptr(), _stream())
+    if rc != MLCC_OK:
+        _raise(rc)
+    return out
+
+
+def closed_loops(nxt, want_chain_col=True):
+    """mlcc_closed_loops: nxt [S,n] i32 -> (chain_col [S,n] i32 or None, chain_end [n] i32, loop_id [n] i32,
+    num_loops [1] i32), all on the device."""
+    if nxt.dim() != 2:
+        raise ValueError("nxt must be [S, n]")
+    S, n = nxt.shape
+    dev = nxt.device
+    col = torch.empty((S, n), dtype=torch.int32, device=dev) if want_chain_col else None
+    end = torch.empty((n,), dtype=torch.int32, device=dev)
+    lid = torch.empty((n,), dtype=torch.int32, device=dev)
+    cnt = torch.empty((1,), dtype=torch.int32, device=dev)
+    rc = lib().mlcc_closed_loops(_dev(nxt, torch.int32, "nxt"), S, n, None if col is None else col.data_ptr(),
+                                 end.data_ptr(), lid.data_ptr(), cnt.data_ptr(), _stream())
+    if rc != MLCC_OK:
+        _raise(rc)
+    return col, end, lid, cnt
+
+
+def order_by_chain(points, chain_col):
+    """mlcc_order_by_chain: points [S,n,2], chain_col [S,n] i32 -> [S,n,2] with column k = chain k."""
+    if points.dim() != 3 or points.shape[2] != 2 or tuple(chain_col.shape) != tuple(points.shape[:2]):
+        raise ValueError("points must be [S, n, 2] and chain_col [S, n]")
+    S, n, _ = points.shape
+    out = torch.empty_like(points)
+    rc = lib().mlcc_order_by_chain(_dev(points, name="points"), _dev(chain_col, torch.int32, "chain_col"), S, n,
+                                   out.data_ptr(), _stream())
+    if rc != MLCC_OK:
+        _raise(rc)
+    return out
+
+
+def distance_map(cmap, pixel, want_d2=False):
+    """mlcc_distance_map: crossing map [ny,nx] i32 -> distance to the nearest caustic pixel [ny,nx] f64
+    (and the exact squared distance in pixels, i64, if asked)."""
+    if cmap.dim() != 2:
+        raise ValueError("cmap must be [ny, nx]")
+    ny, nx = cmap.shape
+    out = torch.empty((ny, nx), dtype=torch.float64, device=cmap.device)
+    d2 = torch.empty((ny, nx), dtype=torch.int64, device=cmap.device) if want_d2 else None
+    rc = lib().mlcc_distance_map(_dev(cmap, torch.int32, "cmap"), nx, ny, float(pixel), out.data_ptr(),
+                                 None if d2 is None else d2.data_ptr(), _stream())
+    if rc != MLCC_OK:
+        _raise(rc)
+    return (out, d2) if want_d2 else out
+
+
+def directional_distance_map(cmap, pixel, ux, uy):
+    """mlcc_directional_distance_map: crossing map [ny,nx] i32, integer direction -> signed distance [ny,nx] f64."""
+    if cmap.dim() != 2:
+        raise ValueError("cmap must be [ny, nx]")
+    ny, nx = cmap.shape
+    out = torch.empty((ny, nx), dtype=torch.float64, device=cmap.device)
+    rc = lib().mlcc_directional_distance_map(_dev(cmap, torch.int32, "cmap"), nx, ny, float(pixel), int(ux), int(uy),
+                                             out.data_ptr(), _stream())
     if rc != MLCC_OK:
         _raise(rc)
     return out

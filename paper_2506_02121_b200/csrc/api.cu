@@ -54,6 +54,11 @@ int crossing_map_impl(const double *, const int32_t *, int64_t, int64_t, int, do
                       int32_t, int32_t *, cudaStream_t);
 int star_sums_impl(const double *, const double *, int64_t, const double *, int64_t, int, int, int, double *,
                    cudaStream_t);
+int closed_loops_impl(const int32_t *, int64_t, int64_t, int32_t *, int32_t *, int32_t *, int32_t *, cudaStream_t);
+int order_by_chain_impl(const double *, const int32_t *, int64_t, int64_t, double *, cudaStream_t);
+int distance_map_impl(const int32_t *, int32_t, int32_t, double, double *, int64_t *, cudaStream_t);
+int directional_distance_map_impl(const int32_t *, int32_t, int32_t, double, int32_t, int32_t, double *,
+                                  cudaStream_t);
 int match_root_sets_impl(const double *, const double *, int64_t, int64_t, double, double *, int32_t *,
                          cudaStream_t);
 
@@ -257,6 +262,32 @@ int mlcc_crossing_map(const double *caustics, const int32_t *next, int64_t S, in
 {
     return crossing_map_impl(caustics, next, S, n, closed, x0, y0, pixel, nx, ny, out_map,
                              static_cast<cudaStream_t>(stream));
+}
+
+int mlcc_closed_loops(const int32_t *next, int64_t S, int64_t n, int32_t *out_chain_col, int32_t *out_chain_end,
+                      int32_t *out_loop_id, int32_t *out_num_loops, void *stream)
+{
+    return closed_loops_impl(next, S, n, out_chain_col, out_chain_end, out_loop_id, out_num_loops,
+                             static_cast<cudaStream_t>(stream));
+}
+
+int mlcc_order_by_chain(const double *points, const int32_t *chain_col, int64_t S, int64_t n, double *out,
+                        void *stream)
+{
+    return order_by_chain_impl(points, chain_col, S, n, out, static_cast<cudaStream_t>(stream));
+}
+
+int mlcc_distance_map(const int32_t *crossing_map, int32_t nx, int32_t ny, double pixel, double *out_distance,
+                      int64_t *out_d2, void *stream)
+{
+    return distance_map_impl(crossing_map, nx, ny, pixel, out_distance, out_d2, static_cast<cudaStream_t>(stream));
+}
+
+int mlcc_directional_distance_map(const int32_t *crossing_map, int32_t nx, int32_t ny, double pixel, int32_t ux,
+                                  int32_t uy, double *out_distance, void *stream)
+{
+    return directional_distance_map_impl(crossing_map, nx, ny, pixel, ux, uy, out_distance,
+                                         static_cast<cudaStream_t>(stream));
 }
 
 int mlcc_star_sums(const double *star_xy, const double *masses, int64_t N, const double *points, int64_t P,

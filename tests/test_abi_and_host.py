@@ -120,6 +120,19 @@ def test_invalid_arguments_fail_before_any_cuda_call(lib):
     assert L.mlcc_crossing_map(one, None, 3, 5, 1, 0.0, 0.0, 0.0, 8, 8, one, None) == api.MLCC_ERR_INVALID_ARG
     assert L.mlcc_crossing_map(one, None, 3, 5, 1, 0.0, 0.0, 0.1, 0, 8, one, None) == api.MLCC_ERR_INVALID_ARG
     assert L.mlcc_crossing_map(one, None, 0, 5, 1, 0.0, 0.0, 0.1, 8, 8, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_closed_loops(None, 3, 5, None, one, one, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_closed_loops(one, 3, 5, None, None, one, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_closed_loops(one, 0, 5, None, one, one, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_closed_loops(one, 3, 0, None, one, one, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_order_by_chain(None, one, 3, 5, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_order_by_chain(one, one, 3, 5, one, None) == api.MLCC_ERR_INVALID_ARG            # aliasing
+    assert L.mlcc_order_by_chain(None, None, 0, 5, None, None) == api.MLCC_OK                      # S = 0
+    assert L.mlcc_distance_map(None, 8, 8, 0.1, one, None, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_distance_map(one, 0, 8, 0.1, one, None, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_distance_map(one, 8, 8, -0.1, one, None, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_directional_distance_map(one, 8, 8, 0.1, 0, 0, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_directional_distance_map(one, 8, 8, 0.1, 1 << 21, 1, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_directional_distance_map(one, 8, 8, 0.1, 1, 1, None, None) == api.MLCC_ERR_INVALID_ARG
     o = api.mlcc_options()
     L.mlcc_options_default(C.byref(o))
     assert o.struct_size == C.sizeof(api.mlcc_options) and o.star_sum_mode == api.MLCC_STAR_SUMS_DIRECT
