@@ -31,6 +31,7 @@ METRIC = "converged critical-curve roots/s"
 UNIT = "roots/s"
 FLOP_PER_STAR_PAIR = 27.0   # algorithmic flop per (root, star) pair, 1 reciprocal = 1 flop
 FLOP_PER_ROOT_PAIR = 10.0   # per (root, root) pair
+NCU_DRAM_BYTES_FULL_ITERATION = 11_930_880 + 6_912     # profiles/r01_k_compute_ncu.md C (launch 4: read + write)
 NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # SMs x FP64 lanes x 2 flop x max SM clock
 
 
@@ -253,7 +254,13 @@ def main():
                         "(seed/apply/finalize launches included), CUDA events on the launch stream. Confirming iterations "
                         "of nearly converged roots leave the Aberth sum out (DESIGN.md R27) and their root pairs are not "
                         "counted; frac_with_survey_accounting counts 47N flop for every root-iteration as SURVEY.md 8(d) does",
-                "traffic": None}
+                # dram__bytes_read.sum + dram__bytes_write.sum of one full-iteration launch of the cfg4 direct-sum kernel
+                # (16 rows x 20 000 roots, 1.504e11 algorithmic flop, 6.98 ms) from the ncu --set full capture summarised
+                # in profiles/r01_k_compute_ncu.md C: 11.93 MB read, < 0.01 MB written; not measured for other workloads
+                "traffic": (NCU_DRAM_BYTES_FULL_ITERATION if (args.workload == "cfg4" and args.star_sums == "direct")
+                            else None),
+                "traffic_note": "bytes of DRAM traffic per full-iteration launch (ncu capture, profiles/r01_k_compute_ncu.md): "
+                                "the working set is L2-resident, 12.6 kflop per DRAM byte; the bound is the ALU one"}
 
     # ---- measured issue model behind the roofline ----
     if rank == 0:
