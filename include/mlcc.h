@@ -148,6 +148,18 @@ int mlcc_star_field(uint64_t seed, int64_t N, double kappa_star, int mass_model,
                     const double *mass_params, double *star_xy, double *masses,
                     double *out_radius, void *stream);
 
+/* a0 for the rectangular field of Section 4.2 (Appendix A at :386: stars in the
+ * rectangle with corner c = c1 + i c2, sides 2 c1 x 2 c2).  Same masses and seed recipe as
+ * mlcc_star_field; Eq. 9 with A_star = 4 c1 c2 and sum m_i = N fixes
+ * c2 = sqrt(pi N / (4 kappa_star aspect)), c1 = aspect c2  (aspect = c1/c2 > 0).  Star i sits at
+ * (c1 x, c2 y) with x, y uniform in [-1, 1) from Philox counter (i, 0, 0).  Feed c1, c2 to
+ * mlcc_rect_sheet for the matching smooth sheet.
+ *   star_xy [N][2], masses [N]: device, written.  out_corner [2]: host, may be NULL, gets {c1, c2}.
+ * Synchronises `stream`.  Errors: INVALID_ARG (also aspect <= 0 or non-finite), CUDA.              */
+int mlcc_star_field_rect(uint64_t seed, int64_t N, double kappa_star, double aspect, int mass_model,
+                         const double *mass_params, double *star_xy, double *masses,
+                         double *out_corner, void *stream);
+
 /* a1-a6  Critical curves (PAPER.md:128 Eq. 15, :159 Eq. 17, :170 Eq. 19, :176-182, :211-213).
  * For each row j of the grid phi_j = 2 pi j / num_phi finds all 2N roots of F(z, phi_j) by the
  * Aberth–Ehrlich iteration evaluated from the rational form (O(N) star sums and an O(N) sum over

@@ -52,6 +52,8 @@ def lib():
         L.orc_directional_distance_map.argtypes = [_pi32, C.c_int32, C.c_int32, C.c_double, C.c_int32, C.c_int32, _pd]
         L.orc_star_field.argtypes = [C.c_uint64, C.c_int64, C.c_double, C.c_int, C.c_void_p,
                                      _pd, _pd, C.POINTER(C.c_double)]
+        L.orc_star_field_rect.argtypes = [C.c_uint64, C.c_int64, C.c_double, C.c_double, C.c_int, C.c_void_p,
+                                          _pd, _pd, _pd]
         L.orc_philox4x32_10.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32),
                                         C.POINTER(C.c_uint32)]
         L.orc_philox4x32_10.restype = None
@@ -89,6 +91,20 @@ def star_field(seed, N, kappa_star, mass_model=0, mass_params=None):
     _check(lib().orc_star_field(int(seed), int(N), float(kappa_star), int(mass_model), pp, xy, m,
                                 C.byref(R)), "star_field")
     return xy, m, R.value
+
+
+def star_field_rect(seed, N, kappa_star, aspect, mass_model=0, mass_params=None):
+    """-> (star_xy [N,2] f64, masses [N] f64, c1, c2): stars uniform in the rectangle with corner c1 + i c2."""
+    xy = np.empty((N, 2), _d)
+    m = np.empty(N, _d)
+    c = np.zeros(2, _d)
+    pp = None
+    if mass_params is not None:
+        arr = np.ascontiguousarray(mass_params, _d)
+        pp = arr.ctypes.data_as(C.c_void_p)
+    _check(lib().orc_star_field_rect(int(seed), int(N), float(kappa_star), float(aspect), int(mass_model), pp, xy, m, c),
+           "star_field_rect")
+    return xy, m, float(c[0]), float(c[1])
 
 
 def _stars(star_xy, masses):

@@ -740,8 +740,28 @@ static double powerlaw_icdf(double u, double lo, double hi, double alpha)
  * by rejection from the square: star i, attempt a uses Philox counter (i_lo, i_hi, a, 0) and key
  * (seed_lo, seed_hi); x = 2 u53(r0, r1) - 1, y = 2 u53(r2, r3) - 1, accepted iff x*x + y*y < 1.
  * The mass of star i uses counter (i_lo, i_hi, 0, 1) and u = u53(r0, r1).                       */
+static int star_field_any(uint64_t seed, int64_t N, double kappa_star, int mass_model, const double *mass_params,
+                          double aspect, double *star_xy, double *masses, double *out_radius, double *out_corner);
+
 int orc_star_field(uint64_t seed, int64_t N, double kappa_star, int mass_model,
                    const double *mass_params, double *star_xy, double *masses, double *out_radius)
+{
+    return star_field_any(seed, N, kappa_star, mass_model, mass_params, 0.0, star_xy, masses, out_radius, NULL);
+}
+
+/* Rectangular field (Section 4.2; Appendix A at :386: stars in the rectangle with corner
+ * c = c1 + i c2).  Same masses; Eq. 9 with A_star = 4 c1 c2 and sum m_i = N gives
+ * c2 = sqrt(pi N / (4 kappa_star aspect)), c1 = aspect c2.  Star i sits at (c1 x, c2 y) with the x, y of
+ * attempt 0 of the disk recipe (uniform in [-1,1)^2, no rejection).  out_corner = {c1, c2}.              */
+int orc_star_field_rect(uint64_t seed, int64_t N, double kappa_star, double aspect, int mass_model,
+                        const double *mass_params, double *star_xy, double *masses, double *out_corner)
+{
+    if (!(aspect > 0.0) || !(aspect < INFINITY)) return -2;
+    return star_field_any(seed, N, kappa_star, mass_model, mass_params, aspect, star_xy, masses, NULL, out_corner);
+}
+
+static int star_field_any(uint64_t seed, int64_t N, double kappa_star, int mass_model, const double *mass_params,
+                          double aspect, double *star_xy, double *masses, double *out_radius, double *out_corner)
 {
     if (N < 1 || !(kappa_star > 0.0) || mass_model < 0 || mass_model > 2) return -2;
     static const double salpeter[3] = {0.08, 1.0, 2.35};
@@ -791,6 +811,19 @@ int orc_star_field(uint64_t seed, int64_t N, double kappa_star, int mass_model,
     for (int64_t i = 0; i < N; ++i) masses[i] /= mean;
 
     /* positions */
+    if (aspect > 0.0) {
+        const double c2 = sqrt(3.14159265358979323846 * (double)N / (4.0 * kappa_star * aspect));
+        const double c1 = aspect * c2;
+        for (int64_t i = 0; i < N; ++i) {
+            uint32_t ctr[4] = {(uint32_t)((uint64_t)i & 0xFFFFFFFFu), (uint32_t)((uint64_t)i >> 32), 0u, 0u};
+            uint32_t r[4];
+            orc_philox4x32_10(ctr, key, r);
+            star_xy[2 * i] = c1 * (2.0 * u53(r[0], r[1]) - 1.0);
+            star_xy[2 * i + 1] = c2 * (2.0 * u53(r[2], r[3]) - 1.0);
+        }
+        if (out_corner) { out_corner[0] = c1; out_corner[1] = c2; }
+        return 0;
+    }
     const double R = sqrt((double)N / kappa_star);
     for (int64_t i = 0; i < N; ++i) {
         double x = 0.0, y = 0.0;

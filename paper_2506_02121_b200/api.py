@@ -86,6 +86,7 @@ def lib() -> C.CDLL:
         L.mlcc_options_default.argtypes = [C.POINTER(mlcc_options)]
         L.mlcc_options_default.restype = None
         L.mlcc_star_field.argtypes = [C.c_uint64, i64, dbl, C.c_int, vp, vp, vp, C.POINTER(dbl), vp]
+        L.mlcc_star_field_rect.argtypes = [C.c_uint64, i64, dbl, dbl, C.c_int, vp, vp, vp, vp, vp]
         L.mlcc_critical_curves.argtypes = [vp, vp, i64, dbl, dbl, i64, dbl, i32, vp]
         L.mlcc_critical_curves_ex.argtypes = [vp, vp, i64, dbl, dbl, i64, dbl, i32, vp,
                                               C.POINTER(mlcc_options), vp, vp, vp,
@@ -200,6 +201,23 @@ def star_field(seed: int, N: int, kappa_star: float, mass_model: int = 0, mass_p
     if rc != MLCC_OK:
         _raise(rc)
     return xy, m, R.value
+
+
+def star_field_rect(seed: int, N: int, kappa_star: float, aspect: float, mass_model: int = 0, mass_params=None,
+                    device="cuda"):
+    """mlcc_star_field_rect -> (star_xy [N,2], masses [N], c1, c2): stars uniform in the rectangle with corner c1 + i c2."""
+    xy = torch.empty((N, 2), dtype=torch.float64, device=device)
+    m = torch.empty((N,), dtype=torch.float64, device=device)
+    corner = np.zeros(2, np.float64)
+    pp = None
+    if mass_params is not None:
+        arr = np.ascontiguousarray(mass_params, np.float64)
+        pp = arr.ctypes.data_as(C.c_void_p)
+    rc = lib().mlcc_star_field_rect(int(seed), int(N), float(kappa_star), float(aspect), int(mass_model), pp,
+                                    xy.data_ptr(), m.data_ptr(), corner.ctypes.data, _stream())
+    if rc != MLCC_OK:
+        _raise(rc)
+    return xy, m, float(corner[0]), float(corner[1])
 
 
 def critical_curves(star_xy, masses, kappa_s, gamma, num_phi, tol=1e-12, max_iter=50):

@@ -48,7 +48,8 @@ int critical_curves_impl(const double *, const double *, int64_t, double, double
                          mlcc_stats *, cudaStream_t);
 int caustics_impl(const double *, const double *, int64_t, double, double, const double *, int64_t, double *,
                   cudaStream_t);
-int star_field_impl(uint64_t, int64_t, double, int, const double *, double *, double *, double *, cudaStream_t);
+int star_field_impl(uint64_t, int64_t, double, int, const double *, double, double *, double *, double *, double *,
+                    cudaStream_t);
 int link_rows_impl(const double *, int64_t, int64_t, int32_t *, int32_t *, cudaStream_t);
 int crossing_map_impl(const double *, const int32_t *, int64_t, int64_t, int, double, double, double, int32_t,
                       int32_t, int32_t *, cudaStream_t);
@@ -178,7 +179,18 @@ void mlcc_options_default(mlcc_options *opt)
 int mlcc_star_field(uint64_t seed, int64_t N, double kappa_star, int mass_model, const double *mass_params,
                     double *star_xy, double *masses, double *out_radius, void *stream)
 {
-    return star_field_impl(seed, N, kappa_star, mass_model, mass_params, star_xy, masses, out_radius,
+    return star_field_impl(seed, N, kappa_star, mass_model, mass_params, 0.0, star_xy, masses, out_radius, nullptr,
+                           static_cast<cudaStream_t>(stream));
+}
+
+int mlcc_star_field_rect(uint64_t seed, int64_t N, double kappa_star, double aspect, int mass_model,
+                         const double *mass_params, double *star_xy, double *masses, double *out_corner, void *stream)
+{
+    if (!(aspect > 0.0)) {
+        set_last_error("invalid argument: aspect must be positive");
+        return MLCC_ERR_INVALID_ARG;
+    }
+    return star_field_impl(seed, N, kappa_star, mass_model, mass_params, aspect, star_xy, masses, nullptr, out_corner,
                            static_cast<cudaStream_t>(stream));
 }
 

@@ -94,7 +94,8 @@ __global__ void k_mass_total(const double *partial, int n, double *total)
     }
 }
 
-__global__ void k_normalise_and_place(uint32_t k0, uint32_t k1, long long N, double R,
+// disk: sx = sy = R, rejection from the square.  rectangle: sx = c1, sy = c2, attempt 0 is the star.
+__global__ void k_normalise_and_place(uint32_t k0, uint32_t k1, long long N, double sx, double sy, int rect,
                                       const double *total, double *masses, double2 *xy, int *fail)
 {
     const double mean = *total / (double)N;
@@ -103,6 +104,13 @@ __global__ void k_normalise_and_place(uint32_t k0, uint32_t k1, long long N, dou
         masses[i] = masses[i] / mean;
         double x = 0.0, y = 0.0;
         bool ok = false;
+        if (rect) {
+            uint32_t r[4];
+            philox4x32_10((uint32_t)(i & 0xFFFFFFFFll), (uint32_t)((unsigned long long)i >> 32), 0u, 0u, k0, k1, r);
+            x = 2.0 * u53(r[0], r[1]) - 1.0;
+            y = 2.0 * u53(r[2], r[3]) - 1.0;
+            ok = true;
+        }
         for (uint32_t attempt = 0; attempt < 256u && !ok; ++attempt) {
             uint32_t r[4];
             philox4x32_10((uint32_t)(i & 0xFFFFFFFFll), (uint32_t)((unsigned long long)i >> 32), attempt, 0u, k0, k1, r);
@@ -111,16 +119,18 @@ __global__ void k_normalise_and_place(uint32_t k0, uint32_t k1, long long N, dou
             ok = __dadd_rn(__dmul_rn(x, x), __dmul_rn(y, y)) < 1.0;
         }
         if (!ok) atomicExch(fail, 1);
-        xy[i] = make_double2(__dmul_rn(R, x), __dmul_rn(R, y));
+        xy[i] = make_double2(__dmul_rn(sx, x), __dmul_rn(sy, y));
     }
 }
 
 }  // namespace
 
+// aspect = 0: the disk of mlcc_star_field; aspect > 0: the rectangle of mlcc_star_field_rect (out_corner = {c1, c2})
 int star_field_impl(uint64_t seed, int64_t N, double kappa_star, int mass_model,
-                    const double *mass_params, double *star_xy, double *masses, double *out_radius,
-                    cudaStream_t stream)
+                    const double *mass_params, double aspect, double *star_xy, double *masses, double *out_radius,
+                    double *out_corner, cudaStream_t stream)
 {
+    if (!(aspect >= 0.0) || !isfinite(aspect)) return invalid("aspect must be positive");
     if (!star_xy || !masses) return invalid("null pointer");
     if (N < 1 || N > (1ll << 29)) return invalid("N out of range");
     if (!(kappa_star > 0.0) || !isfinite(kappa_star)) return invalid("kappa_star must be positive");
@@ -156,6 +166,9 @@ int star_field_impl(uint64_t seed, int64_t N, double kappa_star, int mass_model,
         mm.cum[3] = 1.0;
     }
     const double R = sqrt((double)N / kappa_star);
+    // Eq. 9 with A_star = 4 c1 c2 and sum m_i = N
+    const double c2 = aspect > 0.0 ? sqrt(3.14159265358979323846 * (double)N / (4.0 * kappa_star * aspect)) : 0.0;
+    const double c1 = aspect * c2;
     const uint32_t k0 = (uint32_t)(seed & 0xFFFFFFFFull), k1 = (uint32_t)(seed >> 32);
 
     Workspace ws(stream);
@@ -169,7 +182,8 @@ int star_field_impl(uint64_t seed, int64_t N, double kappa_star, int mass_model,
     k_masses<<<nblk, BLOCK, 0, stream>>>(mm, k0, k1, (long long)N, masses, partial);
     k_mass_total<<<1, 32, 0, stream>>>(partial, nblk, total);
     const int grid = (int)((N + BLOCK - 1) / BLOCK < 2048 ? (N + BLOCK - 1) / BLOCK : 2048);
-    k_normalise_and_place<<<grid, BLOCK, 0, stream>>>(k0, k1, (long long)N, R, total, masses,
+    k_normalise_and_place<<<grid, BLOCK, 0, stream>>>(k0, k1, (long long)N, aspect > 0.0 ? c1 : R, aspect > 0.0 ? c2 : R,
+                                                     aspect > 0.0 ? 1 : 0, total, masses,
                                                      reinterpret_cast<double2 *>(star_xy), fail);
     MLCC_CUDA(cudaGetLastError());
     int h_fail = 0;
@@ -180,6 +194,7 @@ int star_field_impl(uint64_t seed, int64_t N, double kappa_star, int mass_model,
         return MLCC_ERR_CUDA;
     }
     if (out_radius) *out_radius = R;
+    if (out_corner && aspect > 0.0) { out_corner[0] = c1; out_corner[1] = c2; }
     return MLCC_OK;
 }
 

@@ -108,6 +108,12 @@ def test_invalid_arguments_fail_before_any_cuda_call(lib):
     assert L.mlcc_star_field(0, 0, 0.4, 0, None, one, one, None, None) == api.MLCC_ERR_INVALID_ARG
     assert L.mlcc_star_field(0, 5, -1.0, 0, None, one, one, None, None) == api.MLCC_ERR_INVALID_ARG
     assert L.mlcc_star_field(0, 5, 0.4, 7, None, one, one, None, None) == api.MLCC_ERR_INVALID_ARG
+    L.mlcc_star_field_rect.argtypes = [C.c_uint64, C.c_int64, C.c_double, C.c_double, C.c_int, C.c_void_p, C.c_void_p,
+                                       C.c_void_p, C.c_void_p, C.c_void_p]
+    assert L.mlcc_star_field_rect(0, 5, 0.4, 0.0, 0, None, one, one, None, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_star_field_rect(0, 5, 0.4, float("inf"), 0, None, one, one, None, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_star_field_rect(0, 0, 0.4, 1.0, 0, None, one, one, None, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_star_field_rect(0, 5, 0.4, 1.0, 0, None, None, one, None, None) == api.MLCC_ERR_INVALID_ARG
     assert L.mlcc_fp64_peak(50.0, None, None) == api.MLCC_ERR_INVALID_ARG
     assert L.mlcc_star_sums(None, one, 3, one, 5, 0, 0, 0, one, None) == api.MLCC_ERR_INVALID_ARG
     assert L.mlcc_star_sums(one, one, 3, one, 5, 2, 0, 0, one, None) == api.MLCC_ERR_INVALID_ARG   # unknown mode

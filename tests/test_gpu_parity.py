@@ -64,6 +64,19 @@ def test_star_field_matches_oracle_generator(api, orc, name):
     assert abs(float(m.sum()) - cfg.N) < 1e-9 * cfg.N
 
 
+@pytest.mark.parametrize("N,kstar,aspect,model", [(1, 0.4, 1.0, 0), (600, 0.4, 2.0, 1), (10000, 0.2, 0.5, 2),
+                                                  (50001, 0.6, 1.3, 0)])
+def test_rectangular_star_field_matches_oracle_generator(api, orc, N, kstar, aspect, model):
+    """mlcc_star_field_rect (Section 4.2's field): corner and positions bit-exact, masses to a few ulp."""
+    xy, m, c1, c2 = api.star_field_rect(7, N, kstar, aspect, model)
+    oxy, om, oc1, oc2 = orc.star_field_rect(7, N, kstar, aspect, model)
+    assert (c1, c2) == (oc1, oc2)
+    assert np.array_equal(xy.cpu().numpy(), oxy)
+    assert np.abs(m.cpu().numpy() / om - 1).max() < 1e-14
+    with pytest.raises(api.MlccError):
+        api.star_field_rect(7, N, kstar, -1.0, model)
+
+
 def test_star_field_seed_and_defaults(api, orc):
     a = api.star_field(5, 1000, 0.3, 2)
     b = api.star_field(5, 1000, 0.3, 2, (0.01, 0.08, 0.5, 1.5, 0.3, 1.3, 2.3))
@@ -609,6 +622,28 @@ def test_rectangular_field_roots_and_caustics_against_oracle(api, orc, N, aspect
     # without the polynomial the same stars have 2N roots: the option changes the problem, and is needed
     plain, _, _, _ = api.critical_curves_ex(dev(xy), dev(m), ks, g + shift, num_phi)
     assert plain.shape[1] == 2 * N
+
+
+def test_rectangular_field_from_the_seeded_generator(api, orc):
+    """The whole rectangular path on generated inputs: mlcc_star_field_rect -> mlcc_rect_sheet -> curves and caustics,
+    against the oracle on the oracle's own generated field (bit-identical positions)."""
+    N, kstar, aspect, ks, g, num_phi = 300, 0.4, 1.6, 0.05, 0.15, 12
+    xy, m, c1, c2 = api.star_field_rect(11, N, kstar, aspect, 1)
+    oxy, om, oc1, oc2 = orc.star_field_rect(11, N, kstar, aspect, 1)
+    assert (c1, c2) == (oc1, oc2) and np.array_equal(xy.cpu().numpy(), oxy)
+    coef, shift, t = api.rect_sheet(kstar, c1, c2, s=1.5, eps=1e-9)
+    seed_r = 1.2 * np.hypot(c1, c2)
+    rows = np.array([0, 5, 11])
+    ref, _, un = orc.rect_critical_curve_rows(oxy, om, ks, g, kstar, c1, c2, t, seed_r, num_phi, rows)
+    assert un.sum() == 0
+    w_ref = orc.rect_caustics(oxy, om, ks, g, kstar, c1, c2, t, ref)
+    opt = api.options(sheet_poly=coef, seed_radius=seed_r)
+    roots, caus, iters, unconv, st = api.curves_and_caustics(xy, m, ks, g + shift, num_phi, opt=opt)
+    assert int(unconv.sum()) == 0 and roots.shape[1] == 2 * N + t - 1
+    gr, gw = roots.cpu().numpy(), caus.cpu().numpy()
+    assert_rows_match(orc, gr[rows], ref)
+    for i, j in enumerate(rows):
+        assert_caustics_match(gr[j], gw[j], ref[i], w_ref[i])
 
 
 def test_rectangular_field_argument_checks(api):

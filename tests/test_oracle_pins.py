@@ -369,6 +369,33 @@ def _broken_power_law_cdf(mgrid, p):
     return np.interp(mgrid, xs, cum)
 
 
+def test_rectangular_star_field_geometry_and_stats(orc):
+    """Stars of Section 4.2's rectangular field: Eq. 9 with A_star = 4 c1 c2 and
+    sum m = N gives the corner; x/c1 and y/c2 are independent and uniform on [-1, 1); the stars the disk recipe
+    accepts at its first attempt are the same points of the unit square."""
+    from scipy import stats
+    N, kstar, aspect = 20000, 0.35, 1.7
+    xy, m, c1, c2 = orc.star_field_rect(3, N, kstar, aspect, 1)
+    assert abs(c1 / c2 - aspect) < 1e-14 and abs(np.pi * m.sum() / (4 * c1 * c2) - kstar) < 1e-12   # Eq. 9
+    assert abs(m.sum() - N) < 1e-9 * N
+    u, v = xy[:, 0] / c1, xy[:, 1] / c2
+    assert np.abs(u).max() < 1 and np.abs(v).max() < 1 and np.abs(u).max() > 0.999
+    assert stats.kstest((u + 1) / 2, "uniform").pvalue > 1e-3 and stats.kstest((v + 1) / 2, "uniform").pvalue > 1e-3
+    assert abs(np.corrcoef(u, v)[0, 1]) < 0.03
+    occupancy = np.histogram2d(u, v, bins=8, range=[[-1, 1], [-1, 1]])[0]
+    assert stats.chisquare(occupancy.ravel()).pvalue > 1e-3                       # uniform in area
+    # same seed -> same masses as the disk field; first-attempt stars of the disk are the same unit-square points
+    dxy, dm, R = orc.star_field(3, N, kstar, 1)
+    assert np.array_equal(dm, m)
+    first = u ** 2 + v ** 2 < 1 - 1e-12
+    assert 0.75 < first.mean() < 0.82                                             # pi/4
+    assert np.abs(dxy[first, 0] / R - u[first]).max() < 1e-15 and np.abs(dxy[first, 1] / R - v[first]).max() < 1e-15
+    xy2, _, _, _ = orc.star_field_rect(4, N, kstar, aspect, 1)
+    assert not np.array_equal(xy, xy2)
+    with pytest.raises(RuntimeError):
+        orc.star_field_rect(0, 10, 0.4, 0.0)
+
+
 def test_star_field_mass_functions(orc):
     from scipy import stats
     N = 40000
