@@ -45,6 +45,9 @@ def parse():
     ap.add_argument("--num-phi", type=int, default=0, help="override the number of phases (profiling runs)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--post", action="store_true",
+                    help="also time the post-processing calls on the step's outputs (chain joining, closed loops, "
+                         "crossing map, distance maps) and add them as `post_processing`; outside the timed region")
     ap.add_argument("--subchains", type=int, default=0)
     ap.add_argument("--order", type=int, default=-1)
     ap.add_argument("--min-lanes", type=int, default=0)
@@ -272,6 +275,44 @@ def main():
                                               "a 3-source DFMA takes 3 clk, and packed FP32 FMAs take operand slots away "
                                               "from the FP64 stream"}
 
+    # ---- post-processing of the timed step's outputs, outside the timed region ----
+    post = None
+    if args.post and world == 1:
+        def timed(f, reps=3):
+            f()
+            best, out = None, None
+            for _ in range(reps):
+                torch.cuda.synchronize()
+                p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                p0.record()
+                out = f()
+                p1.record()
+                torch.cuda.synchronize()
+                t_ms = p0.elapsed_time(p1)
+                best = t_ms if best is None or t_ms < best else best
+            return best, out
+
+        n_pix = 2048
+        half = 0.134 * (cfg.N / cfg.kappa_star) ** 0.5          # 60 theta_star wide at cfg4
+        pixel = 2 * half / n_pix
+        t_link, (nxt, lbij) = timed(lambda: api.link_rows(roots))
+        t_loops, (col, end, lid, cnt) = timed(lambda: api.closed_loops(nxt))
+        t_order, ordered = timed(lambda: api.order_by_chain(roots, col))
+        del ordered
+        t_cross, cmap = timed(lambda: api.crossing_map(caus, nxt, -half, -half, pixel, n_pix, n_pix))
+        t_edt, dmap = timed(lambda: api.distance_map(cmap, pixel))
+        t_dir, ddir = timed(lambda: api.directional_distance_map(cmap, pixel, 0, 1))
+        gather_bytes = roots.numel() * 8 * 2 + col.numel() * 4
+        post = {"unit": "ms per call (best of 3, CUDA events)", "rows": num_phi, "roots_per_row": n_r,
+                "map": f"{n_pix} x {n_pix} pixels of {pixel:.4f} theta_star",
+                "link_rows": t_link, "rows_not_bijective": int((lbij == 0).sum()),
+                "closed_loops": t_loops, "num_loops": int(cnt.item()), "chains_not_closed": int((lid < 0).sum()),
+                "order_by_chain": t_order, "order_by_chain_GBps": gather_bytes / t_order / 1e6,
+                "crossing_map": t_cross, "max_crossings": int(cmap.max()),
+                "distance_map": t_edt, "directional_distance_map_(0,1)": t_dir,
+                "rays_that_met_a_caustic": float((ddir > 0).double().mean())}
+        del nxt, col, cmap, dmap, ddir
+
     # ---- the same workload with the paper's far-field split of the star sums, outside the timed region ----
     far_field = None
     if world == 1 and args.star_sums == "direct" and not args.no_e2e:
@@ -296,6 +337,36 @@ def main():
                      "note": "mlcc_options.star_sum_mode = MLCC_STAR_SUMS_FMM: stars of the 5x5 nodes around a root directly, "
                              "the rest from the node's order-31 Taylor series; the Aberth sum over roots stays direct. "
                              "Not the headline: BASELINE.json fixes direct O(N) star sums"}
+
+    # ---- the same workload with mlcc_options.trust_predictor (R30), outside the timed region ----
+    predicted = None
+    if world == 1 and args.star_sums == "direct" and not args.no_e2e:
+        predicted = {"unit": UNIT,
+                     "note": "mlcc_options.trust_predictor = 1: rows seeded by the cubic predictor start with Newton steps "
+                             "(no Aberth sum); a step above 1e-8 is discarded and that root gets the full Aberth iteration. "
+                             "Cold rows and fallbacks keep Eq. 17. Not the headline: the headline evaluates the Aberth sum "
+                             "for every root of every row"}
+        for label, mode in (("direct_star_sums", api.MLCC_STAR_SUMS_DIRECT), ("far_field_star_sums", api.MLCC_STAR_SUMS_FMM)):
+            topt = api.options(num_subchains=args.subchains, predictor_order=args.order, min_lanes_per_root=args.min_lanes,
+                               phi_index_offset=phi_off, phi_index_total=phi_total, aberth_sum_precision=args.aberth_sum,
+                               skip_aberth_sum_below=args.skip_aberth_below, star_sum_mode=mode, trust_predictor=1)
+            best, tst = None, None
+            for _ in range(2):
+                torch.cuda.synchronize()
+                f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                f0.record()
+                _, _, _, _, tst = api.curves_and_caustics(fxy, fm, cfg.kappa_s, cfg.gamma, num_phi, cfg.tol, cfg.max_iter,
+                                                          opt=topt, out_roots=caus, out_caustics=prev, want_diagnostics=False)
+                f1.record()
+                torch.cuda.synchronize()
+                t_ms = f0.elapsed_time(f1)
+                best = t_ms if best is None or t_ms < best else best
+            terr, tbij = api.match_root_sets(caus, roots, 1e-10)
+            predicted[label] = {"value": num_phi * n_r / (best * 1e-3), "seconds_per_curve_set": best * 1e-3,
+                                "matches_headline_root_sets": bool(tbij.all()), "max_abs_dz_vs_headline": float(terr.max()),
+                                "unconverged_rows": tst.unconverged_rows,
+                                "root_iterations_per_root": tst.root_iterations / float(num_phi * n_r),
+                                "root_iterations_with_aberth_sum_per_root": tst.root_pairs / float(n_r - 1) / float(num_phi * n_r)}
 
     # ---- end to end through the host-buffer C-ABI call (pinned host memory both ways) ----
     e2e = None
@@ -353,6 +424,10 @@ def main():
                            "root_iterations_per_root": st.root_iterations / float(num_phi * n_r)},
                 "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
                 "far_field": far_field}
+        if post is not None:
+            line["post_processing"] = post
+        if predicted is not None:
+            line["predicted_newton"] = predicted
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

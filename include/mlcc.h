@@ -88,7 +88,15 @@ typedef struct mlcc_options {
     int32_t fmm_order;        /* Taylor order of the node series (1..63); 0 = 31                     */
     int32_t fmm_stars_per_node; /* mean stars per grid node (the grid has ~N / this many nodes);
                                    0 = 4                                                             */
-    int32_t reserved_;        /* 0                                                                   */
+    int32_t trust_predictor;  /* 0 (default): the first iteration of every row evaluates the Aberth sum for
+                                 every root.  1: a row whose seeds come from the predictor at its full
+                                 order (predictor_order >= 1) starts with Newton steps (no Aberth sum);
+                                 a step below skip_aberth_sum_below is applied and confirmed as usual, a
+                                 larger one is discarded and that root gets a full Aberth iteration from
+                                 its seed instead.  Cold rows, low-order rows and every root whose
+                                 prediction was off keep Eq. 17 as printed; the fixed point F = 0 and the
+                                 freeze test are the same (reading R30).  Needs
+                                 skip_aberth_sum_below >= 0.                                         */
     /* Smooth-sheet polynomial (rectangular microlens field, PAPER.md:197-205 and Appendix B).  With
        H(u) = sum_{n=0}^{d} sheet_poly[n] u^n (REAL coefficients) the lens equation becomes
          w = (1-kappa_s) z + gamma conj(z) - conj( sum_i m_i/(z - z_i) + H(z) ),

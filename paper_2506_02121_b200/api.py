@@ -37,7 +37,7 @@ class mlcc_options(C.Structure):
                 ("phi_index_offset", C.c_int64), ("phi_index_total", C.c_int64),
                 ("min_lanes_per_root", C.c_int32), ("aberth_sum_precision", C.c_int32),
                 ("star_sum_mode", C.c_int32), ("fmm_order", C.c_int32),
-                ("fmm_stars_per_node", C.c_int32), ("reserved_", C.c_int32),
+                ("fmm_stars_per_node", C.c_int32), ("trust_predictor", C.c_int32),
                 ("sheet_poly", C.c_void_p), ("sheet_poly_n", C.c_int32), ("reserved2_", C.c_int32),
                 ("seed_radius", C.c_double), ("skip_aberth_sum_below", C.c_double)]
 
@@ -147,7 +147,8 @@ def last_error() -> str:
 
 def options(num_subchains=0, predictor_order=-1, max_iter_cold=0, phi_index_offset=0,
             phi_index_total=0, min_lanes_per_root=0, aberth_sum_precision=0, star_sum_mode=0, fmm_order=0,
-            fmm_stars_per_node=0, sheet_poly=None, seed_radius=0.0, skip_aberth_sum_below=0.0) -> mlcc_options:
+            fmm_stars_per_node=0, sheet_poly=None, seed_radius=0.0, skip_aberth_sum_below=0.0,
+            trust_predictor=0) -> mlcc_options:
     o = mlcc_options()
     lib().mlcc_options_default(C.byref(o))
     o.num_subchains = num_subchains
@@ -161,6 +162,7 @@ def options(num_subchains=0, predictor_order=-1, max_iter_cold=0, phi_index_offs
     o.fmm_order = fmm_order
     o.fmm_stars_per_node = fmm_stars_per_node
     o.skip_aberth_sum_below = skip_aberth_sum_below
+    o.trust_predictor = int(trust_predictor)
     if sheet_poly is not None:
         arr = np.ascontiguousarray(sheet_poly, np.float64)
         o._keep = arr                       # the struct holds a raw host pointer: keep the array alive

@@ -148,6 +148,7 @@ struct Params {
     int poly_n;
     double seed_radius;       // circle of the n_r - 2N extra cold seeds
     double skip_below2;       // a root whose last |Delta|^2 was below this is iterated without the Aberth sum; 0 = never
+    int trust;                // mlcc_options.trust_predictor: rows seeded by the full-order predictor start without A
     // far-field mode (MLCC_STAR_SUMS_FMM): star sums come from k_star_sums, the compute kernel sums root pairs only
     double *ssum;             // [max_slots][n_r][8] star sums of the unfrozen roots, by list position
     int2 *outside;            // [max_slots * n_r] (slot, position) of the roots outside the node grid
@@ -696,6 +697,13 @@ __global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Para
 // root -- do not depend on the timing of this launch: two runs give the same bits.
 // grid: max_slots CTAs of APPLY_THREADS threads
 // ------------------------------------------------------------------------------------------------
+// mlcc_options.trust_predictor (R30): the rows of a step whose seeds come from the predictor at its
+// full order start with every root in the no-Aberth-sum group; k_apply guards that first iteration.
+__device__ __forceinline__ bool trusted_step(const Params &p, int step)
+{
+    return p.trust && p.skip_below2 > 0.0 && p.order >= 1 && step >= 1 && 2 * step - 1 >= p.order + 1;
+}
+
 constexpr int APPLY_THREADS = 1024;
 constexpr int APPLY_ITEMS = 4;
 
@@ -715,6 +723,10 @@ __global__ void __launch_bounds__(APPLY_THREADS) k_apply(Params p)
     const double2 *delta = p.delta + (long long)slot * p.n_r;
     double2 *row = p.roots + p.slot_row[slot] * p.n_r;
     float4 *slot_src = p.src + (size_t)slot * 2 * p.N_pad;
+    // First iteration of a trusted row: the steps were taken without the Aberth sum, i.e. they are Newton steps from
+    // the predicted seeds.  One below the skip threshold is applied as any confirming step is; a larger one says the
+    // prediction was not that good: it is NOT applied and the root gets a full Aberth iteration from its seed next.
+    const bool guard = st.iter == 0 && trusted_step(p, st.step);
     // A survivor (|Delta|^2 >= tol^2) is "large" if |Delta|^2 >= skip_below2, else "small": the next list holds
     // the large ones first, then the small ones, each group in the order of this list.
     // pass 1: the number of large survivors = where the small ones start
@@ -751,12 +763,16 @@ __global__ void __launch_bounds__(APPLY_THREADS) k_apply(Params p)
                 const double2 d = delta[pos];
                 const double d2 = d.x * d.x + d.y * d.y;
                 if (d2 <= 1.79769313486231570e308) {   // finite step
-                    double2 z = row[k];
-                    z.x -= d.x;
-                    z.y -= d.y;
-                    row[k] = z;
-                    store_src<MODE>(slot_src, k, z);
-                    if (!(d2 < p.tol2)) kind[i] = (d2 < p.skip_below2) ? 2 : 1;
+                    if (guard && !(d2 < p.skip_below2)) {
+                        kind[i] = 1;                    // rejected Newton step: back to the Aberth group, z unchanged
+                    } else {
+                        double2 z = row[k];
+                        z.x -= d.x;
+                        z.y -= d.y;
+                        row[k] = z;
+                        store_src<MODE>(slot_src, k, z);
+                        if (!(d2 < p.tol2)) kind[i] = (d2 < p.skip_below2) ? 2 : 1;
+                    }
                 } else {                                // NaN / Inf: freeze where it is, report
                     atomicAdd(&p.state->degenerate, 1);
                 }
@@ -919,7 +935,8 @@ __device__ void build_slots(const Params &p, DevState &st, long long *s_buf)
     if (threadIdx.x < st.n_slots) {
         p.n_active[st.cur * MAX_SLOTS + threadIdx.x] = p.n_r;
         p.n_active[(st.cur ^ 1) * MAX_SLOTS + threadIdx.x] = 0;
-        p.n_small[st.cur * MAX_SLOTS + threadIdx.x] = 0;      // a new row: every root gets the Aberth sum
+        // a new row: every root gets the Aberth sum, unless the step's seeds are trusted (then none does at first)
+        p.n_small[st.cur * MAX_SLOTS + threadIdx.x] = trusted_step(p, st.step) ? p.n_r : 0;
         p.n_small[(st.cur ^ 1) * MAX_SLOTS + threadIdx.x] = 0;
         p.slot_iters[threadIdx.x] = 0;
     }
@@ -1105,6 +1122,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
         return invalid("aberth_sum_precision must be 0, 32 or 64");
     const int mode = opt.aberth_sum_precision == 64 ? MODE_F64 : MODE_F32;
     if (!isfinite(opt.skip_aberth_sum_below)) return invalid("skip_aberth_sum_below");
+    if (opt.trust_predictor != 0 && opt.trust_predictor != 1) return invalid("trust_predictor must be 0 or 1");
     if (opt.star_sum_mode != MLCC_STAR_SUMS_DIRECT && opt.star_sum_mode != MLCC_STAR_SUMS_FMM)
         return invalid("star_sum_mode");
 
@@ -1231,6 +1249,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     const double skip_below = opt.skip_aberth_sum_below == 0.0 ? 1e-8 : opt.skip_aberth_sum_below;
     const bool skip_on = skip_below > 0.0;
     p.skip_below2 = skip_on ? skip_below * skip_below : 0.0;
+    p.trust = opt.trust_predictor != 0 ? 1 : 0;
     p.poly_n = poly_n;
     p.seed_radius = opt.seed_radius;
     if (poly_n > 0) {

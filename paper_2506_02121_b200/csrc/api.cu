@@ -168,7 +168,7 @@ void mlcc_options_default(mlcc_options *opt)
     opt->star_sum_mode = MLCC_STAR_SUMS_DIRECT;
     opt->fmm_order = 0;
     opt->fmm_stars_per_node = 0;
-    opt->reserved_ = 0;
+    opt->trust_predictor = 0;
     opt->sheet_poly = nullptr;
     opt->sheet_poly_n = 0;
     opt->reserved2_ = 0;

@@ -691,6 +691,50 @@ def test_confirm_iterations_without_the_aberth_sum(api, orc):
         assert bool(bij.all())
 
 
+@pytest.mark.parametrize("name,num_phi", [("cfg1", 1000), ("cfg2", 4000), ("cfg3", 5000)])
+def test_trust_predictor_starts_rows_with_newton_steps(api, orc, name, num_phi):
+    """DESIGN.md reading R30 (mlcc_options.trust_predictor): rows seeded by the full-order predictor start without the
+    Aberth sum; a Newton step above the skip threshold is discarded and the root falls back to Eq. 17.  Same root
+    sets as the oracle and as the default path, every row complete (Vieta sums), far fewer (root, root) pairs."""
+    cfg = CONFIGS[name]
+    xy, m, R = field(orc, cfg)
+    rows = np.arange(num_phi) if cfg.N <= 200 else np.array([0, 1, 2, 3, 1249, 2500, 2501, 4999])
+    if cfg.N <= 200:
+        ref, _, un = orc.critical_curves(xy, m, cfg.kappa_s, cfg.gamma, num_phi, cfg.tol, cfg.max_iter)
+    else:
+        ref = np.concatenate([orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, num_phi, [j], cfg.tol,
+                                                      cfg.max_iter)[0] for j in rows])
+    for mode in (api.MLCC_STAR_SUMS_DIRECT, api.MLCC_STAR_SUMS_FMM):
+        base, it0, un0, st0 = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, num_phi, cfg.tol,
+                                                     cfg.max_iter, opt=api.options(star_sum_mode=mode))
+        got, it1, un1, st1 = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, num_phi, cfg.tol,
+                                                    cfg.max_iter, opt=api.options(star_sum_mode=mode, trust_predictor=1))
+        assert int(un1.sum()) == 0 and st1.degenerate_roots == 0 and st1.unconverged_rows == 0
+        assert_rows_match(orc, got.cpu().numpy()[rows], ref)
+        e1, e2 = vieta_all_rows(got, xy, m, cfg.kappa_s, cfg.gamma, num_phi)
+        assert e1 < 1e-12 and e2 < 1e-12, (e1, e2)
+        err, bij = api.match_root_sets(got, base, 1e-12)
+        assert bool(bij.all())
+        if name != "cfg1":     # cfg1's grid is coarse (2 pi / 1000): many predictions miss the threshold and fall back
+            assert st1.root_pairs < 0.5 * st0.root_pairs, (st1.root_pairs, st0.root_pairs)
+            assert st1.root_iterations < 1.35 * st0.root_iterations
+        else:
+            assert st1.root_iterations < 2.5 * st0.root_iterations
+    # fused caustics of the trusted path against the stand-alone kernel on the same roots
+    r, c, _, _, st = api.curves_and_caustics(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, num_phi, cfg.tol, cfg.max_iter,
+                                             opt=api.options(trust_predictor=1))
+    c2 = api.caustics(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, r)
+    assert float((c - c2).abs().max()) <= 1e-11
+    # with the plain previous row as the seed (order 0) nothing is trusted: identical to the default path
+    a, _, _, sa = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, min(num_phi, 200), cfg.tol, cfg.max_iter,
+                                         opt=api.options(predictor_order=0, trust_predictor=1))
+    b, _, _, sb = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, min(num_phi, 200), cfg.tol, cfg.max_iter,
+                                         opt=api.options(predictor_order=0))
+    assert torch.equal(a, b) and sa.root_pairs == sb.root_pairs
+    with pytest.raises(api.MlccError):
+        api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, 8, opt=api.options(trust_predictor=2))
+
+
 def test_crossing_map_full_size_cfg4_sampled_pixels(api, orc):
     """cfg4 at its full size (10^4 phases x 2*10^4 roots = 2*10^8 caustic segments, far-field star sums for speed):
     chains joined on the GPU, 2048^2 map, and a 4 x 4 sample of its pixels recomputed one by one by the oracle's
