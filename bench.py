@@ -195,7 +195,9 @@ def main():
             _, _, _, _, st = api.curves_and_caustics(xy, m, cfg.kappa_s, cfg.gamma, num_phi, cfg.tol, cfg.max_iter,
                                                      opt=opt, out_roots=roots, out_caustics=caus,
                                                      want_diagnostics=False)
-        err, bij = api.match_root_sets(roots, prev, 1e-10)
+        # the very first call has no previous step to compare with (`prev` is uninitialised memory, for which the
+        # matcher falls back to its O(n^2) search): it checks the sets against themselves
+        err, bij = api.match_root_sets(roots, prev if last else roots, 1e-10)
         last.update(stats=st, err=err, bij=bij)
         return st
 
