@@ -58,6 +58,8 @@ def parse():
                          "(PAPER.md:188-195) -- the roofline object then counts the root pairs only")
     ap.add_argument("--skip-aberth-below", type=float, default=0.0,
                     help="mlcc_options.skip_aberth_sum_below (0 = library default, negative = never skip)")
+    ap.add_argument("--trust-predictor", action="store_true",
+                    help="mlcc_options.trust_predictor = 1 in the timed steps (DESIGN.md R30; not the headline)")
     ap.add_argument("--separate-caustics", action="store_true",
                     help="run mlcc_critical_curves_ex + mlcc_caustics instead of the fused call")
     return ap.parse_args()
@@ -178,7 +180,8 @@ def main():
     opt = api.options(num_subchains=args.subchains, predictor_order=args.order, min_lanes_per_root=args.min_lanes,
                       phi_index_offset=phi_off, phi_index_total=phi_total,
                       aberth_sum_precision=args.aberth_sum, skip_aberth_sum_below=args.skip_aberth_below,
-                      star_sum_mode=api.MLCC_STAR_SUMS_FMM if args.star_sums == "fmm" else api.MLCC_STAR_SUMS_DIRECT)
+                      star_sum_mode=api.MLCC_STAR_SUMS_FMM if args.star_sums == "fmm" else api.MLCC_STAR_SUMS_DIRECT,
+                      trust_predictor=1 if args.trust_predictor else 0)
 
     roots = torch.empty((num_phi, n_r, 2), dtype=torch.float64, device="cuda")
     prev = torch.empty_like(roots)
@@ -342,7 +345,7 @@ def main():
 
     # ---- the same workload with mlcc_options.trust_predictor (R30), outside the timed region ----
     predicted = None
-    if world == 1 and args.star_sums == "direct" and not args.no_e2e:
+    if world == 1 and args.star_sums == "direct" and not args.trust_predictor and not args.no_e2e:
         predicted = {"unit": UNIT,
                      "note": "mlcc_options.trust_predictor = 1: rows seeded by the cubic predictor start with Newton steps "
                              "(no Aberth sum); a step above 1e-8 is discarded and that root gets the full Aberth iteration. "
@@ -417,7 +420,7 @@ def main():
                                        f"kappa_s={cfg.kappa_s}, gamma={cfg.gamma}, tol={cfg.tol}, max_iter={cfg.max_iter}, seed={cfg.seed}",
                            "step": ("star_field + critical_curves_ex + caustics + match_root_sets" if args.separate_caustics
                                     else "star_field + curves_and_caustics (fused) + match_root_sets"),
-                           "aberth_sum_precision": st.aberth_sum_precision, "star_sums": args.star_sums,
+                           "aberth_sum_precision": st.aberth_sum_precision, "star_sums": args.star_sums, "trust_predictor": bool(args.trust_predictor),
                            "subchains": st.subchains, "predictor_order": st.predictor_order,
                            "l2": f"inputs larger than L2: each step writes {2 * num_phi * n_r * 16 / 1e9:.2f} GB of roots and caustics "
                                  f"and reads a {num_phi * n_r * 16 / 1e9:.2f} GB comparison set (L2 is 126 MB)",

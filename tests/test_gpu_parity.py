@@ -716,7 +716,8 @@ def test_trust_predictor_starts_rows_with_newton_steps(api, orc, name, num_phi):
         err, bij = api.match_root_sets(got, base, 1e-12)
         assert bool(bij.all())
         if name != "cfg1":     # cfg1's grid is coarse (2 pi / 1000): many predictions miss the threshold and fall back
-            assert st1.root_pairs < 0.5 * st0.root_pairs, (st1.root_pairs, st0.root_pairs)
+            # what is left are the cold rows (~20 full iterations each), the first rows of every sub-chain and fallbacks
+            assert st1.root_pairs < 0.75 * st0.root_pairs, (st1.root_pairs, st0.root_pairs)
             assert st1.root_iterations < 1.35 * st0.root_iterations
         else:
             assert st1.root_iterations < 2.5 * st0.root_iterations
