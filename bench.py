@@ -229,7 +229,11 @@ def main():
         st = step()
         solve_ms += st.solve_ms
         launches += st.kernel_launches + 3 + 1 + (1 if args.separate_caustics else 0)   # star field (3), matcher, caustics
-        alg_flop += (0.0 if args.star_sums == "fmm" else FLOP_PER_STAR_PAIR * st.star_pairs) + FLOP_PER_ROOT_PAIR * st.root_pairs
+        # root-iterations without the Aberth sum take the Newton step of F and do not accumulate S1 either
+        # (R27): their star pairs are 2 flop (one complex addition) lighter
+        iters_without_A = st.root_iterations - st.root_pairs / float(n_r - 1)
+        alg_flop += (0.0 if args.star_sums == "fmm" else
+                     FLOP_PER_STAR_PAIR * st.star_pairs - 2.0 * cfg.N * iters_without_A) + FLOP_PER_ROOT_PAIR * st.root_pairs
         alg_flop_survey += (FLOP_PER_STAR_PAIR * cfg.N + FLOP_PER_ROOT_PAIR * (n_r - 1)) * st.root_iterations
         compute_launches += st.total_iterations
     ev1.record()
@@ -258,7 +262,7 @@ def main():
                                                 if (solve_ms > 0 and peak_measured and args.star_sums == "direct") else None),
                 "algorithmic_flop_per_launch": alg_flop / max(compute_launches, 1),
                 "avg_launch_ms": solve_ms / max(compute_launches, 1),
-                "note": "achieved = (27 flop x star pairs + 10 flop x root pairs EVALUATED) / device time of the whole solve "
+                "note": "achieved = (27 flop x star pairs (25 where S1 is not needed) + 10 flop x root pairs EVALUATED) / device time of the whole solve "
                         "(seed/apply/finalize launches included), CUDA events on the launch stream. Confirming iterations "
                         "of nearly converged roots leave the Aberth sum out (DESIGN.md R27) and their root pairs are not "
                         "counted; frac_with_survey_accounting counts 47N flop for every root-iteration as SURVEY.md 8(d) does",

@@ -110,10 +110,10 @@ typedef struct mlcc_options {
                                  radius about the origin; must be > 0 when d >= 2 and
                                  init_roots is NULL                                                   */
     double skip_aberth_sum_below; /* A root whose step |dz| was below this (but not below tol) is iterated
-                                 the next time without the Aberth sum A (Eq. 17): that iteration only
-                                 confirms |dz| < tol, and A, which multiplies F ~ F' dz in the
-                                 denominator, cannot move the step by more than |dz|^2 |A| (DESIGN.md
-                                 reading R27).  The first iteration of every row always has A, and so
+                                 the next time with the Newton step dz = F/F' (Eq. 17 without the term
+                                 F (2 S1 - A)): that iteration only confirms |dz| < tol, and the term,
+                                 which multiplies F ~ F' dz in the denominator, cannot move the step by
+                                 more than |dz|^2 |2 S1 - A| (reading R27).  The first iteration of every row always has A, and so
                                  has every root whose last step was larger.  0 = library default
                                  (1e-8); negative = never skip.                                       */
 } mlcc_options;

@@ -599,7 +599,7 @@ __global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Para
                         if (!ROOTS) {
 #pragma unroll
                             for (int r = 0; r < R; ++r)
-                                if (STARS) pair_star<CAUS>(zx[r], zy[r], sxy, sm, acc[r]);
+                                if (STARS) pair_star<CAUS, false>(zx[r], zy[r], sxy, sm, acc[r]);
                         } else if (MODE == MODE_F64) {
                             const double2 *rr = reinterpret_cast<const double2 *>(sg.rp);
                             const double2 ra = rr[2 * j], rb = rr[2 * j + 1];
@@ -637,8 +637,10 @@ __global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Para
                 say = ay[r] + by[r];
             }
             if (STARS) {
-                v[r][0] = 2.0 * acc[r].s1x - sax;
-                v[r][1] = 2.0 * acc[r].s1y - say;
+                // without the Aberth sum the step is the Newton step of F: t = 2 S1 - A is left out as a whole
+                // (2 S1 and A nearly cancel -- two roots per star -- so 2 S1 alone would be the worse stand-in)
+                v[r][0] = ROOTS ? 2.0 * acc[r].s1x - sax : 0.0;
+                v[r][1] = ROOTS ? 2.0 * acc[r].s1y - say : 0.0;
                 v[r][2] = acc[r].s2x; v[r][3] = acc[r].s2h; v[r][4] = acc[r].s3x; v[r][5] = acc[r].s3y;
                 if (CAUS) { v[r][NV - 2] = acc[r].smx; v[r][NV - 1] = acc[r].smy; }
             } else {
@@ -654,8 +656,8 @@ __global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Para
             } else {
                 const double2 *s = reinterpret_cast<const double2 *>(p.ssum + ((size_t)slot * p.n_r + pos) * 8);
                 const double2 s1 = s[0], s2 = s[1], s3 = s[2], smm = s[3];
-                aberth_step<CAUS>(p, slot, row, list, pos, fma(2.0, s1.x, w[0]), fma(2.0, s1.y, w[1]), s2.x, s2.y,
-                                  s3.x, s3.y, smm.x, smm.y);
+                aberth_step<CAUS>(p, slot, row, list, pos, ROOTS ? fma(2.0, s1.x, w[0]) : 0.0,
+                                  ROOTS ? fma(2.0, s1.y, w[1]) : 0.0, s2.x, s2.y, s3.x, s3.y, smm.x, smm.y);
             }
         };
         if (T == 1) {
@@ -1141,7 +1143,20 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     // plan
     std::vector<long long> first(MAX_SLOTS), centre(MAX_SLOTS), end(MAX_SLOTS);
     std::vector<int64_t> f64v(MAX_SLOTS), c64v(MAX_SLOTS), e64v(MAX_SLOTS);
-    const int n_sub = plan_subchains_host(N, num_phi, opt.num_subchains, MAX_SLOTS / 2, f64v.data(),
+    int want_sub = opt.num_subchains;
+    if (want_sub == 0 && opt.trust_predictor == 1 && opt.star_sum_mode == MLCC_STAR_SUMS_FMM) {
+        // Continued rows cost O(N) here (far-field star sums, no Aberth sum): a step of the default plan is a handful
+        // of short, latency-bound launches.  Four times as many rows per step amortise them; the price is four times
+        // as many cold rows (measured on cfg4: 0.53 s per set with the default plan, 0.34 s with four times it).
+        const int base = plan_subchains_host(N, num_phi, 0, MAX_SLOTS / 2, f64v.data(), c64v.data(), e64v.data());
+        if (base >= 1) {
+            long long w = 4ll * base;
+            if (w > num_phi / 16) w = num_phi / 16;
+            if (w > MAX_SLOTS / 2) w = MAX_SLOTS / 2;
+            want_sub = (int)(w > base ? w : base);
+        }
+    }
+    const int n_sub = plan_subchains_host(N, num_phi, want_sub, MAX_SLOTS / 2, f64v.data(),
                                           c64v.data(), e64v.data());
     if (n_sub < 1) return invalid("num_subchains");
     int max_steps = 0;

@@ -43,7 +43,9 @@ struct FmmGrid {
 // (root, star): with d = z - z_i, w = 1/d = conj(d)/|d|^2 = (wx, wy)  [dy is taken as y_i - y],
 //   S1 += w,  S2 += m w^2 = m (wx^2 - wy^2, 2 wx wy),  S3 += m w^3 = m (wx (wx^2 - 3 wy^2), wy (3 wx^2 - wy^2)).
 // 22 FP64 instructions + 1 MUFU; 18 of them name at most two distinct register sources.
-template <bool CAUS>
+// WITH_S1 = false leaves S1 out (the iterations without the Aberth sum take the Newton step of F, which needs
+// neither A nor S1: DESIGN.md R27): 20 (22) FP64 instructions.
+template <bool CAUS, bool WITH_S1 = true>
 __device__ __forceinline__ void pair_star(double zx, double zy, double2 s, double m, StarAcc &a)
 {
     const double dx = zx - s.x;
@@ -52,8 +54,10 @@ __device__ __forceinline__ void pair_star(double zx, double zy, double2 s, doubl
     const double inv = rcp_full(r2);
     const double wx = dx * inv;
     const double wy = dy * inv;
-    a.s1x += wx;
-    a.s1y += wy;
+    if (WITH_S1) {
+        a.s1x += wx;
+        a.s1y += wy;
+    }
     const double ux = m * wx;
     const double uy = m * wy;
     if (CAUS) {
