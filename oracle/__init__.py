@@ -50,6 +50,7 @@ def lib():
         L.orc_closed_loops.argtypes = [_pi32, C.c_int64, C.c_int64, C.c_void_p, _pi32, _pi32, _pi32]
         L.orc_distance_map.argtypes = [_pi32, C.c_int32, C.c_int32, C.c_double, _pd, _pi64]
         L.orc_directional_distance_map.argtypes = [_pi32, C.c_int32, C.c_int32, C.c_double, C.c_int32, C.c_int32, _pd]
+        L.orc_distance_histogram.argtypes = [_pd, C.c_void_p, C.c_int64, C.c_double, C.c_int32, C.c_int32, _pi64, _pi64]
         L.orc_star_field.argtypes = [C.c_uint64, C.c_int64, C.c_double, C.c_int, C.c_void_p,
                                      _pd, _pd, C.POINTER(C.c_double)]
         L.orc_star_field_rect.argtypes = [C.c_uint64, C.c_int64, C.c_double, C.c_double, C.c_int, C.c_void_p,
@@ -245,6 +246,18 @@ def directional_distance_map(cmap, pixel, ux, uy):
     _check(lib().orc_directional_distance_map(cmap, nx, ny, float(pixel), int(ux), int(uy), out),
            "directional_distance_map")
     return out
+
+
+def distance_histogram(distance, cmap, bin_width, num_bins, num_counts=1):
+    """distance map [ny,nx] f64, crossing map [ny,nx] int32 or None -> (hist [num_counts, num_bins] int64, pixels left out)."""
+    d = np.ascontiguousarray(distance, _d)
+    cm = None if cmap is None else np.ascontiguousarray(cmap, np.int32)
+    assert cm is None or cm.shape == d.shape
+    hist = np.empty((num_counts, num_bins), np.int64)
+    left = np.zeros(1, np.int64)
+    _check(lib().orc_distance_histogram(d, None if cm is None else cm.ctypes.data, d.size, float(bin_width), int(num_bins),
+                                        int(num_counts), hist, left), "distance_histogram")
+    return hist, int(left[0])
 
 
 def rect_sheet(kappa_star, c1, c2, t, points):

@@ -691,6 +691,35 @@ int orc_directional_distance_map(const int32_t *map, int32_t nx, int32_t ny, dou
 }
 
 /* ------------------------------------------------------------------------------------------
+ * Distribution of the distance to the nearest caustic (Fig. 6: "probability distribution of
+ * the distance to the nearest caustic" per direction of motion; Fig. 7: the same split by "where the source
+ * happens to lie in the map of N_caustic crossings").  A histogram of a distance map: pixel p with a finite
+ * distance d >= 0 (a negative value of the moving-source map is limited by the border of the map and is left
+ * out, so is +inf) is counted in bin floor(d / bin_width) if that is < num_bins, in row
+ * min(max(count_p, 0), num_counts - 1) of the table (row 0 if there is no crossing map).
+ * out_hist [num_counts][num_bins] int64; out_left_out [1] int64 = pixels not counted.
+ * ---------------------------------------------------------------------------------------- */
+int orc_distance_histogram(const double *distance, const int32_t *crossing_map, int64_t num_pixels, double bin_width,
+                           int32_t num_bins, int32_t num_counts, int64_t *out_hist, int64_t *out_left_out)
+{
+    if (num_pixels < 0 || !(bin_width > 0.0) || num_bins < 1 || num_counts < 1) return -2;
+    for (int64_t i = 0; i < (int64_t)num_bins * num_counts; ++i) out_hist[i] = 0;
+    int64_t left = 0;
+    for (int64_t p = 0; p < num_pixels; ++p) {
+        const double d = distance[p];
+        if (!(d >= 0.0) || d == INFINITY) { ++left; continue; }
+        const double b = floor(d / bin_width);
+        if (!(b < (double)num_bins)) { ++left; continue; }
+        int32_t row = crossing_map ? crossing_map[p] : 0;
+        if (row < 0) row = 0;
+        if (row > num_counts - 1) row = num_counts - 1;
+        out_hist[(int64_t)row * num_bins + (int64_t)b] += 1;
+    }
+    if (out_left_out) *out_left_out = left;
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
  * Star-field generator (recipe in DESIGN.md "Input recipe").
  * Counter-based Philox4x32-10 (Salmon, Moraes, Dror & Shaw 2011, "Parallel random numbers:
  * as easy as 1, 2, 3"), restated from the published algorithm.

@@ -228,3 +228,36 @@ def test_directional_distance_against_a_sampled_ray(orc):
                 assert abs(abs(hit) - abs(d[py, px])) < 2 * h, (ux, uy, px, py, hit, d[py, px])
             else:
                 assert hit < 0 or abs(d[py, px]) < abs(hit) + 2 * h
+
+
+def test_distance_histogram_against_numpy_and_a_disc(orc):
+    """The statistics of Fig. 6-7 are histograms of the distance maps.  numpy's histogram is the
+    library routine; a circular caustic gives a closed form: inside a disc of radius r the area at distance
+    [d, d + h) from the rim is pi ((r - d)^2 - (r - d - h)^2)."""
+    rng = np.random.default_rng(12)
+    d = rng.uniform(0, 5, size=(40, 60))
+    d[rng.random(d.shape) < 0.1] *= -1            # border-limited rays
+    d[3, 4] = np.inf
+    cm = rng.integers(-1, 7, size=d.shape).astype(np.int32)
+    h, left = orc.distance_histogram(d, cm, 0.25, 16, 5)
+    ok = (d >= 0) & np.isfinite(d) & (d < 4.0)
+    assert left == (~ok).sum() and h.sum() == ok.sum()
+    rows = np.clip(cm, 0, 4)
+    for r in range(5):
+        want, _ = np.histogram(d[ok & (rows == r)], bins=16, range=(0, 4.0))
+        assert np.array_equal(h[r], want)
+    h1, left1 = orc.distance_histogram(d, None, 0.25, 16)
+    assert np.array_equal(h1[0], h.sum(0)) and left1 == left
+    # disc
+    n, pixel, r = 401, 0.01, 1.5
+    X, Y = np.meshgrid((np.arange(n) - n // 2) * pixel, (np.arange(n) - n // 2) * pixel)
+    rho = np.hypot(X, Y)
+    m = (rho < r).astype(np.int32)
+    dist, _ = orc.distance_map(m, pixel)
+    hist, _ = orc.distance_histogram(dist, m, 0.1, 12, 2)
+    edges = 0.1 * np.arange(13)
+    area_in = np.pi * ((r - edges[:-1]) ** 2 - (r - edges[1:]) ** 2) / pixel ** 2
+    # bins 1..11 of the inside (bin 0 holds the two-pixel-wide caustic band itself)
+    assert np.abs(hist[1, 1:12] / area_in[1:12] - 1).max() < 0.06
+    area_out = np.pi * ((r + edges[1:]) ** 2 - (r + edges[:-1]) ** 2) / pixel ** 2
+    assert np.abs(hist[0, 1:5] / area_out[1:5] - 1).max() < 0.06      # outside, while the rings stay inside the map
