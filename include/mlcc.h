@@ -325,6 +325,22 @@ int mlcc_distance_map(const int32_t *crossing_map, int32_t nx, int32_t ny, doubl
 int mlcc_directional_distance_map(const int32_t *crossing_map, int32_t nx, int32_t ny, double pixel,
                                   int32_t ux, int32_t uy, double *out_distance, void *stream);
 
+/* The statistics of Fig. 6-7: the distribution of the distance to the nearest
+ * caustic, per direction of motion (Fig. 6: one call per mlcc_directional_distance_map) and split by
+ * "where the source happens to lie in the map of N_caustic crossings" (Fig. 7: `crossing_map` given; for
+ * the distance BETWEEN the caustics before and behind a moving source pass the sum of the maps of
+ * (ux, uy) and (-ux, -uy)).  Pixel p with a finite distance d >= 0 is counted in bin
+ * floor(d / bin_width) if that is < num_bins, in row min(max(crossing_map[p], 0), num_counts - 1)
+ * (row 0 when crossing_map is NULL).  Negative values (a ray limited by the border of the map), +inf
+ * and NaN are left out and counted in *out_left_out.
+ *   distance [num_pixels]: device double, read.  crossing_map [num_pixels]: device int32 or NULL.
+ *   out_hist [num_counts][num_bins]: device int64, written.  out_left_out [1]: device int64, written.
+ * Integer counts: exact and independent of timing.  Asynchronous on `stream`.
+ * Errors: INVALID_ARG (also num_bins * num_counts > 2^26), CUDA.                                    */
+int mlcc_distance_histogram(const double *distance, const int32_t *crossing_map, int64_t num_pixels,
+                            double bin_width, int32_t num_bins, int32_t num_counts,
+                            int64_t *out_hist, int64_t *out_left_out, void *stream);
+
 /* (f) NEXT-3: the rectangular sheet of Appendix B as a polynomial (host-only, no CUDA call).
  * For stars in the rectangle with corner c = c1 + i c2 and smooth compensation kappa_star, Eq. B2
  * truncated at the odd power t and extended to an infinite sheet is

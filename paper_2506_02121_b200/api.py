@@ -105,6 +105,7 @@ def lib() -> C.CDLL:
         L.mlcc_order_by_chain.argtypes = [vp, vp, i64, i64, vp, vp]
         L.mlcc_distance_map.argtypes = [vp, i32, i32, dbl, vp, vp, vp]
         L.mlcc_directional_distance_map.argtypes = [vp, i32, i32, dbl, i32, i32, vp, vp]
+        L.mlcc_distance_histogram.argtypes = [vp, vp, i64, dbl, i32, i32, vp, vp, vp]
         L.mlcc_star_sums.argtypes = [vp, vp, i64, vp, i64, C.c_int, C.c_int, C.c_int, vp, vp]
         L.mlcc_plan_subchains.argtypes = [i64, i64, i32, i32, vp, vp, vp]
         L.mlcc_critical_curves_host.argtypes = [vp, vp, i64, dbl, dbl, i64, dbl, i32, vp]
@@ -391,6 +392,21 @@ def directional_distance_map(cmap, pixel, ux, uy):
     if rc != MLCC_OK:
         _raise(rc)
     return out
+
+
+def distance_histogram(distance, cmap, bin_width, num_bins, num_counts=1):
+    """mlcc_distance_histogram: distance map f64, crossing map i32 or None (same shape) ->
+    (hist [num_counts, num_bins] i64, left_out [1] i64) on the device."""
+    if cmap is not None and tuple(cmap.shape) != tuple(distance.shape):
+        raise ValueError("cmap must have the shape of distance")
+    hist = torch.empty((num_counts, num_bins), dtype=torch.int64, device=distance.device)
+    left = torch.empty((1,), dtype=torch.int64, device=distance.device)
+    rc = lib().mlcc_distance_histogram(_dev(distance, name="distance"), _dev(cmap, torch.int32, "cmap"),
+                                       distance.numel(), float(bin_width), int(num_bins), int(num_counts),
+                                       hist.data_ptr(), left.data_ptr(), _stream())
+    if rc != MLCC_OK:
+        _raise(rc)
+    return hist, left
 
 
 def star_sums(star_xy, masses, points, mode=MLCC_STAR_SUMS_DIRECT, fmm_order=0, fmm_stars_per_node=0):

@@ -60,6 +60,8 @@ int order_by_chain_impl(const double *, const int32_t *, int64_t, int64_t, doubl
 int distance_map_impl(const int32_t *, int32_t, int32_t, double, double *, int64_t *, cudaStream_t);
 int directional_distance_map_impl(const int32_t *, int32_t, int32_t, double, int32_t, int32_t, double *,
                                   cudaStream_t);
+int distance_histogram_impl(const double *, const int32_t *, int64_t, double, int32_t, int32_t, int64_t *, int64_t *,
+                            cudaStream_t);
 int match_root_sets_impl(const double *, const double *, int64_t, int64_t, double, double *, int32_t *,
                          cudaStream_t);
 
@@ -300,6 +302,13 @@ int mlcc_directional_distance_map(const int32_t *crossing_map, int32_t nx, int32
 {
     return directional_distance_map_impl(crossing_map, nx, ny, pixel, ux, uy, out_distance,
                                          static_cast<cudaStream_t>(stream));
+}
+
+int mlcc_distance_histogram(const double *distance, const int32_t *crossing_map, int64_t num_pixels, double bin_width,
+                            int32_t num_bins, int32_t num_counts, int64_t *out_hist, int64_t *out_left_out, void *stream)
+{
+    return distance_histogram_impl(distance, crossing_map, num_pixels, bin_width, num_bins, num_counts, out_hist,
+                                   out_left_out, static_cast<cudaStream_t>(stream));
 }
 
 int mlcc_star_sums(const double *star_xy, const double *masses, int64_t N, const double *points, int64_t P,

@@ -107,7 +107,67 @@ __global__ void __launch_bounds__(BLOCK) k_directional(const int *__restrict__ m
     out[p] = hit ? d : -d;
 }
 
+// Histogram of a distance map by bin and crossing count (the statistics of Fig. 6-7).
+// Grid-stride over the pixels, loads coalesced; each CTA counts into its own shared-memory table (when the
+// table fits) and adds it to the global one at the end: 64-bit integer atomics, result independent of timing.
+constexpr int HIST_SMEM_BINS = 8192;
+
+__global__ void __launch_bounds__(BLOCK) k_distance_histogram(const double *__restrict__ dist, const int *__restrict__ cmap,
+                                                              long long P, double bin_width, int num_bins, int num_counts,
+                                                              int use_smem, unsigned long long *hist,
+                                                              unsigned long long *left_out)
+{
+    __shared__ unsigned int s_hist[HIST_SMEM_BINS];
+    const int table = num_bins * num_counts;
+    if (use_smem) {
+        for (int i = threadIdx.x; i < table; i += BLOCK) s_hist[i] = 0u;
+        __syncthreads();
+    }
+    unsigned int left = 0;
+    for (long long p = (long long)blockIdx.x * BLOCK + threadIdx.x; p < P; p += (long long)gridDim.x * BLOCK) {
+        const double d = dist[p];
+        if (!(d >= 0.0) || d > 1.79769313486231570e308) { ++left; continue; }
+        const double b = floor(__ddiv_rn(d, bin_width));
+        if (!(b < (double)num_bins)) { ++left; continue; }
+        int row = cmap ? cmap[p] : 0;
+        row = row < 0 ? 0 : (row > num_counts - 1 ? num_counts - 1 : row);
+        const int at = row * num_bins + (int)b;
+        if (use_smem) atomicAdd(&s_hist[at], 1u);
+        else atomicAdd(&hist[at], 1ull);
+    }
+    for (int o = 16; o > 0; o >>= 1) left += __shfl_xor_sync(0xffffffffu, left, o);
+    if ((threadIdx.x & 31) == 0 && left) atomicAdd(left_out, (unsigned long long)left);
+    if (use_smem) {
+        __syncthreads();
+        for (int i = threadIdx.x; i < table; i += BLOCK)
+            if (s_hist[i]) atomicAdd(&hist[i], (unsigned long long)s_hist[i]);
+    }
+}
+
 }  // namespace
+
+int distance_histogram_impl(const double *distance, const int32_t *crossing_map, int64_t num_pixels, double bin_width,
+                            int32_t num_bins, int32_t num_counts, int64_t *out_hist, int64_t *out_left_out,
+                            cudaStream_t stream)
+{
+    if (!out_hist || !out_left_out || (num_pixels > 0 && !distance)) return invalid("null pointer");
+    if (num_pixels < 0 || num_pixels > (1ll << 40)) return invalid("num_pixels out of range");
+    if (!(bin_width > 0.0) || !isfinite(bin_width)) return invalid("bin_width");
+    if (num_bins < 1 || num_counts < 1 || (long long)num_bins * num_counts > (1ll << 26)) return invalid("table size");
+    const long long table = (long long)num_bins * num_counts;
+    MLCC_CUDA(cudaMemsetAsync(out_hist, 0, sizeof(int64_t) * table, stream));
+    MLCC_CUDA(cudaMemsetAsync(out_left_out, 0, sizeof(int64_t), stream));
+    if (num_pixels == 0) return MLCC_OK;
+    long long blocks = (num_pixels + BLOCK - 1) / BLOCK;
+    const long long cap = 8ll * device_sm_count();        // a CTA counts < 2^32 pixels in its shared table
+    if (blocks > cap) blocks = cap;
+    k_distance_histogram<<<(unsigned)blocks, BLOCK, 0, stream>>>(distance, crossing_map, (long long)num_pixels, bin_width,
+                                                                num_bins, num_counts, table <= HIST_SMEM_BINS ? 1 : 0,
+                                                                reinterpret_cast<unsigned long long *>(out_hist),
+                                                                reinterpret_cast<unsigned long long *>(out_left_out));
+    MLCC_CUDA(cudaGetLastError());
+    return MLCC_OK;
+}
 
 int distance_map_impl(const int32_t *map, int32_t nx, int32_t ny, double pixel, double *out, int64_t *out_d2,
                       cudaStream_t stream)

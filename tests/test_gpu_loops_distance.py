@@ -273,6 +273,52 @@ def test_distance_maps_full_size(api, orc):
     assert np.allclose(d[0, :], -0.5 * pixel, rtol=1e-15)
 
 
+@pytest.mark.parametrize("num_bins,num_counts", [(16, 5), (1, 1), (4096, 2), (5000, 4)])
+def test_distance_histogram_against_oracle(api, orc, num_bins, num_counts):
+    """Small tables (counted in shared memory) and one beyond 8192 entries (global atomics); negative, infinite and NaN
+    distances and out-of-range counts on both sides.  Integer counts: exact."""
+    rng = np.random.default_rng(num_bins + num_counts)
+    shape = (301, 517)
+    d = rng.uniform(0, 6, size=shape)
+    d[rng.random(shape) < 0.1] *= -1
+    d[rng.random(shape) < 0.01] = np.inf
+    d[rng.random(shape) < 0.01] = np.nan
+    d[0, :7] = 0.5 * np.arange(7)                        # values on bin edges
+    cm = rng.integers(-2, 8, size=shape).astype(np.int32)
+    bw = 5.0 / num_bins if num_bins > 1 else 0.5
+    for cmap in (cm, None):
+        ref, ref_left = orc.distance_histogram(d, cmap, bw, num_bins, num_counts)
+        got, left = api.distance_histogram(dev(d), None if cmap is None else dev(cmap, torch.int32), bw, num_bins,
+                                           num_counts)
+        assert np.array_equal(got.cpu().numpy(), ref) and int(left.item()) == ref_left
+        assert ref.sum() + ref_left == d.size
+    empty = api.distance_histogram(torch.empty((0, 5), dtype=torch.float64, device="cuda"), None, 0.5, 4)
+    assert int(empty[0].sum()) == 0 and int(empty[1].item()) == 0
+
+
+def test_distance_statistics_of_a_caustic_network(api, orc):
+    """Fig. 6 / Fig. 7 on the oracle's crossing map of cfg1: histogram of the moving-source distance per direction,
+    and of the distance between the caustics before and behind the source split by the crossing count."""
+    cmap, pixel = crossing_map_of(orc, "cfg1", 720, 96)
+    g_map = dev(cmap, torch.int32)
+    for ux, uy in [(1, 0), (0, 1), (2, 3)]:
+        fwd = api.directional_distance_map(g_map, pixel, ux, uy)
+        bwd = api.directional_distance_map(g_map, pixel, -ux, -uy)
+        o_fwd = orc.directional_distance_map(cmap, pixel, ux, uy)
+        o_bwd = orc.directional_distance_map(cmap, pixel, -ux, -uy)
+        ref, ref_left = orc.distance_histogram(o_fwd, None, 2 * pixel, 24)
+        got, left = api.distance_histogram(fwd, None, 2 * pixel, 24)
+        assert np.array_equal(got.cpu().numpy(), ref) and int(left.item()) == ref_left and ref.sum() > 1000
+        both = torch.where((fwd > 0) & (bwd > 0), fwd + bwd, torch.full_like(fwd, -1.0))
+        o_both = np.where((o_fwd > 0) & (o_bwd > 0), o_fwd + o_bwd, -1.0)
+        ref, ref_left = orc.distance_histogram(o_both, cmap, 2 * pixel, 24, int(cmap.max()) + 1)
+        got, left = api.distance_histogram(both, g_map, 2 * pixel, 24, int(cmap.max()) + 1)
+        assert np.array_equal(got.cpu().numpy(), ref) and int(left.item()) == ref_left
+        # every pixel inside a caustic (count >= 1) whose chord ends on caustics at both ends is in the table or left out
+        inside = (cmap >= 1) & (o_both > 0)
+        assert ref[1:].sum() == (inside & (o_both < 48 * pixel)).sum() > 0
+
+
 def test_argument_checks(api):
     cm = torch.zeros((4, 4), dtype=torch.int32, device="cuda")
     with pytest.raises(api.MlccError) as e:
