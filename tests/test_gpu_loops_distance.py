@@ -316,7 +316,7 @@ def test_distance_statistics_of_a_caustic_network(api, orc):
         assert np.array_equal(got.cpu().numpy(), ref) and int(left.item()) == ref_left
         # every pixel inside a caustic (count >= 1) whose chord ends on caustics at both ends is in the table or left out
         inside = (cmap >= 1) & (o_both > 0)
-        assert ref[1:].sum() == (inside & (o_both < 48 * pixel)).sum() > 0
+        assert ref[1:].sum() == (inside & (np.floor(o_both / (2 * pixel)) < 24)).sum() > 0
 
 
 def test_argument_checks(api):
