@@ -58,6 +58,8 @@ def parse():
                          "(PAPER.md:188-195) -- the roofline object then counts the root pairs only")
     ap.add_argument("--skip-aberth-below", type=float, default=0.0,
                     help="mlcc_options.skip_aberth_sum_below (0 = library default, negative = never skip)")
+    ap.add_argument("--clock-sample-ms", type=int, default=200,
+                    help="period of the nvidia-smi clock / throttle-reason samples taken during the timed region")
     ap.add_argument("--trust-predictor", action="store_true",
                     help="mlcc_options.trust_predictor = 1 in the timed steps (DESIGN.md R30; not the headline)")
     ap.add_argument("--separate-caustics", action="store_true",
@@ -71,13 +73,13 @@ class ClockSampler:
          "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
-    def __init__(self, gpu_index=0):
-        self.rows, self.proc, self.thread, self.gpu = [], None, None, gpu_index
+    def __init__(self, gpu_index=0, period_ms=200):
+        self.rows, self.proc, self.thread, self.gpu, self.period_ms = [], None, None, gpu_index, int(period_ms)
 
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-lms", "200", "-i", str(self.gpu)], stdout=subprocess.PIPE,
+                                          "-lms", str(self.period_ms), "-i", str(self.gpu)], stdout=subprocess.PIPE,
                                          stderr=subprocess.DEVNULL, text=True)
         except OSError:
             self.proc = None
@@ -214,7 +216,7 @@ def main():
         step()
         prev.copy_(roots)
     barrier()
-    sampler = ClockSampler(local_rank)
+    sampler = ClockSampler(local_rank, args.clock_sample_ms)
     if rank == 0:
         sampler.start()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
