@@ -474,9 +474,10 @@ __global__ void __launch_bounds__(BLOCK) k_star_sums_outside(Params p)
 // read costs the same wavefronts whatever T is, and each value read is used for R roots.
 // STARS = false (far-field mode): the stages carry root entries only and the star sums are read
 // from p.ssum; the loop body is then two packed FP32 root pairs per root, hence the larger R.
-// ROOTS = false: the variant without the Aberth sum (A = 0).  It takes the unfrozen roots whose last step was below
+// ROOTS = false: the variant without the Aberth sum: the Newton step of F, t = 2 S1 - A left out as a whole, S1 not
+// accumulated.  It takes the unfrozen roots whose last step was below
 // the skip threshold (the tail [n_active - n_small, n_active) of every slot's list, tile set 1); the full kernel
-// takes the others (tile set 0).  DESIGN.md reading R27.
+// takes the others (tile set 0).  DESIGN.md readings R27, R30 (with trust_predictor: whole rows in their first iteration).
 template <int MODE, bool CAUS, bool STARS, bool ROOTS, int R>
 __global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Params p)
 {

@@ -167,6 +167,35 @@ def test_full_size_sampled_rows_and_invariants(api, orc, name, sample_rows):
                              cplx(roots[int(j)].cpu().numpy()))
 
 
+def test_bench_configuration_full_size_cfg4(api, orc):
+    """The call bench.py times, as it times it: mlcc_star_field + the FUSED mlcc_curves_and_caustics with default
+    options on cfg4 at its full size (10^4 phases x 2*10^4 roots) + mlcc_match_root_sets.  Sampled rows (roots and
+    their fused caustic points) against the oracle, Vieta sums and the device validator on every row, and a second
+    run that must give the same bits."""
+    cfg = CONFIGS["cfg4"]
+    xy, m, R = api.star_field(cfg.seed, cfg.N, cfg.kappa_star, cfg.mass_model, cfg.mass_params)
+    oxy, om, oR = field(orc, cfg)
+    assert R == oR and np.array_equal(xy.cpu().numpy(), oxy)
+    xy_o, m_o = dev(oxy), dev(om)                    # both sides solve the oracle generator's field
+    roots, caus, iters, unconv, st = api.curves_and_caustics(xy_o, m_o, cfg.kappa_s, cfg.gamma, cfg.num_phi, cfg.tol,
+                                                             cfg.max_iter, want_diagnostics=False)
+    assert st.unconverged_rows == 0 and st.degenerate_roots == 0 and st.subchains >= 2
+    e1, e2 = vieta_all_rows(roots, oxy, om, cfg.kappa_s, cfg.gamma, cfg.num_phi)
+    assert e1 < 1e-12 and e2 < 1e-12, (e1, e2)
+    for j in (17, 5000, 7321, 9999):
+        ref, _, un = orc.critical_curve_rows(oxy, om, cfg.kappa_s, cfg.gamma, cfg.num_phi, [j], cfg.tol, cfg.max_iter)
+        assert un.sum() == 0
+        g = roots[j:j + 1].cpu().numpy()
+        assert_rows_match(orc, g, ref)
+        w_ref = orc.caustics(oxy, om, cfg.kappa_s, cfg.gamma, ref)
+        assert_caustics_match(g[0], caus[j].cpu().numpy(), ref[0], w_ref[0])
+    again, caus2, _, _, _ = api.curves_and_caustics(xy_o, m_o, cfg.kappa_s, cfg.gamma, cfg.num_phi, cfg.tol,
+                                                    cfg.max_iter, want_diagnostics=False)
+    err, bij = api.match_root_sets(again, roots, 1e-10)
+    assert bool(bij.all()) and float(err.max()) == 0.0
+    assert torch.equal(again, roots) and torch.equal(caus2, caus)
+
+
 # ---------------------------------------------------------------------------------------------
 # options do not change the answer (the iteration path is not part of the contract)
 # ---------------------------------------------------------------------------------------------
