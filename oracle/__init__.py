@@ -51,6 +51,8 @@ def lib():
         L.orc_distance_map.argtypes = [_pi32, C.c_int32, C.c_int32, C.c_double, _pd, _pi64]
         L.orc_directional_distance_map.argtypes = [_pi32, C.c_int32, C.c_int32, C.c_double, C.c_int32, C.c_int32, _pd]
         L.orc_distance_histogram.argtypes = [_pd, C.c_void_p, C.c_int64, C.c_double, C.c_int32, C.c_int32, _pi64, _pi64]
+        L.orc_vieta_residuals.argtypes = [_pd, _pd, C.c_int64, C.c_double, C.c_double, _pd, C.c_int64, C.c_int64,
+                                          C.c_int64, _pd, _pd]
         L.orc_star_field.argtypes = [C.c_uint64, C.c_int64, C.c_double, C.c_int, C.c_void_p,
                                      _pd, _pd, C.POINTER(C.c_double)]
         L.orc_star_field_rect.argtypes = [C.c_uint64, C.c_int64, C.c_double, C.c_double, C.c_int, C.c_void_p,
@@ -165,6 +167,18 @@ def residuals(star_xy, masses, kappa_s, gamma, phi_index, num_phi_total, points,
              flat.shape[0], out), "residuals")
     return {"F": out[:, 0] + 1j * out[:, 1], "Fp": out[:, 2] + 1j * out[:, 3],
             "inv_mu": out[:, 4].copy(), "newton": out[:, 5].copy()}
+
+
+def vieta_residuals(star_xy, masses, kappa_s, gamma, roots, j_offset=0, num_phi_total=None):
+    """roots [num_phi, 2N, 2] -> (e1 [num_phi], e2 [num_phi]): relative defects of Vieta's first two sums per row."""
+    xy, m, N = _stars(star_xy, masses)
+    r = np.ascontiguousarray(roots, _d)
+    assert r.ndim == 3 and r.shape[1] == 2 * N and r.shape[2] == 2
+    e1 = np.empty(r.shape[0], _d)
+    e2 = np.empty(r.shape[0], _d)
+    _check(lib().orc_vieta_residuals(xy, m, N, float(kappa_s), float(gamma), r, r.shape[0], int(j_offset),
+                                     int(num_phi_total or r.shape[0]), e1, e2), "vieta_residuals")
+    return e1, e2
 
 
 def star_sums(star_xy, masses, points, long_double=True):

@@ -219,6 +219,49 @@ int orc_match_root_sets(const double *a, const double *b, int64_t S, int64_t n, 
 }
 
 /* ------------------------------------------------------------------------------------------
+ * Completeness certificate of a claimed root set (SURVEY.md 8(c) pin P5; BASELINE.json north_star: "exactly
+ * the paper's degree of distinct roots per phase").  P(z; phi) = F(z, phi) prod_i (z - z_i)^2 has
+ * degree 2N with leading coefficient -c(phi), c = (1 - kappa_s) e^{-i phi} - gamma; expanding its two next
+ * coefficients gives Vieta's sums of the 2N roots:
+ *   sum_k z_k = 2 sum_i z_i,     sum_k z_k^2 = 2 sum_i z_i^2 + 2 (sum_i m_i) / c(phi).
+ * A duplicated, missing or misplaced root breaks the first by its displacement.  Per row j,
+ * phi_j = 2 pi (j + j_offset)/num_phi_total, straight long double sums:
+ *   out_e1[j] = |sum z_k - 2 sum z_i| / sum |z_k|,
+ *   out_e2[j] = |sum z_k^2 - 2 sum z_i^2 - 2 M / c_j| / sum |z_k|^2.
+ * ---------------------------------------------------------------------------------------- */
+int orc_vieta_residuals(const double *star_xy, const double *masses, int64_t N, double kappa_s, double gamma,
+                        const double *roots, int64_t num_phi, int64_t j_offset, int64_t num_phi_total,
+                        double *out_e1, double *out_e2)
+{
+    if (N < 1 || num_phi < 1 || num_phi_total < 1) return -2;
+    long double complex sz = 0, sz2 = 0;
+    long double M = 0;
+    for (int64_t i = 0; i < N; ++i) {
+        const long double complex zi = (long double)star_xy[2 * i] + I * (long double)star_xy[2 * i + 1];
+        sz += zi;
+        sz2 += zi * zi;
+        M += masses[i];
+    }
+    const long double two_pi = 6.283185307179586476925286766559L;
+    for (int64_t j = 0; j < num_phi; ++j) {
+        const long double phi = two_pi * (long double)(j + j_offset) / (long double)num_phi_total;
+        const long double complex c = (1.0L - (long double)kappa_s) * (cosl(phi) - I * sinl(phi)) - (long double)gamma;
+        long double complex s1 = 0, s2 = 0;
+        long double a1 = 0, a2 = 0;
+        for (int64_t k = 0; k < 2 * N; ++k) {
+            const long double complex z = (long double)roots[2 * (j * 2 * N + k)] + I * (long double)roots[2 * (j * 2 * N + k) + 1];
+            s1 += z;
+            s2 += z * z;
+            a1 += cabsl(z);
+            a2 += cabsl(z) * cabsl(z);
+        }
+        out_e1[j] = (double)(cabsl(s1 - 2.0L * sz) / a1);
+        out_e2[j] = (double)(cabsl(s2 - 2.0L * sz2 - 2.0L * M / c) / a2);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
  * Rectangular field of microlenses (Section 4.2, Appendix A at :386-401 and
  * Appendix B at :405-457).  The smooth term alpha_s(z) of a rectangular sheet with corner
  * c = c1 + i c2, its logarithms Taylor-expanded about the origin and truncated at power t

@@ -467,3 +467,45 @@ def test_star_sums_consistent_with_residuals_and_caustics(orc):
     w = cplx(orc.caustics(xy, m, ks, g, pts, long_double=True))
     z = pts[:, 0] + 1j * pts[:, 1]
     assert np.abs((1 - ks) * z + g * np.conj(z) - np.conj(out[:, 6] + 1j * out[:, 7]) - w).max() < 1e-12
+
+
+def test_vieta_residuals_certify_complete_root_sets(orc):
+    """orc_vieta_residuals against things it does not compute itself: roots of the EXPANDED polynomial from numpy's
+    companion-matrix solver (N <= 5) must pass; the closed-form Chang-Refsdal roots must pass; and a set with one
+    root replaced by a copy of another fails by exactly the displacement |z_b - z_a| / sum |z_k|."""
+    rng = np.random.default_rng(21)
+    for N in (1, 2, 3, 5):
+        zs = rng.uniform(-2, 2, N) + 1j * rng.uniform(-2, 2, N)
+        ms = rng.uniform(0.3, 1.5, N)
+        xy = np.stack([zs.real, zs.imag], axis=1)
+        kappa_s, gamma, num_phi = 0.15, 0.3, 7
+        rows = []
+        for j in range(num_phi):
+            r = np.roots(expanded_polynomial(zs, ms, kappa_s, gamma, 2 * np.pi * j / num_phi))
+            assert len(r) == 2 * N
+            rows.append(np.stack([r.real, r.imag], axis=1))
+        rows = np.stack(rows)
+        e1, e2 = orc.vieta_residuals(xy, ms, kappa_s, gamma, rows)
+        assert e1.max() < 1e-9 and e2.max() < 1e-9            # numpy's roots of an expanded polynomial: ~1e-11
+        # a sub-grid of a finer one: rows 3..4 of 14 phases are phases 2 pi 3/14, 2 pi 4/14
+        fine = np.stack([np.stack([r.real, r.imag], axis=1) for r in
+                         (np.roots(expanded_polynomial(zs, ms, kappa_s, gamma, 2 * np.pi * j / 14)) for j in (3, 4))])
+        f1, f2 = orc.vieta_residuals(xy, ms, kappa_s, gamma, fine, j_offset=3, num_phi_total=14)
+        assert f1.max() < 1e-9 and f2.max() < 1e-9
+        w1, w2 = orc.vieta_residuals(xy, ms, kappa_s, gamma, fine, j_offset=0, num_phi_total=14)
+        assert w2.max() > 1e-4                                  # the wrong phase: the second sum notices
+        if N >= 2:
+            bad = rows.copy()
+            bad[2, 0] = bad[2, 1]                                # one root duplicated, one missing
+            b1, b2 = orc.vieta_residuals(xy, ms, kappa_s, gamma, bad)
+            shift = abs(cplx(rows[2, 1]) - cplx(rows[2, 0]))
+            assert abs(b1[2] - shift / np.abs(cplx(bad[2])).sum()) < 1e-9 and b1[2] > 1e-3
+            assert np.delete(b1, 2).max() < 1e-9
+    # Chang-Refsdal closed form z = +-sqrt(m / c(phi))
+    m, kappa_s, gamma, num_phi = 0.8, 0.2, 0.35, 12
+    rows = []
+    for j in range(num_phi):
+        z = np.sqrt(m / c_phi(kappa_s, gamma, 2 * np.pi * j / num_phi))
+        rows.append([[z.real, z.imag], [-z.real, -z.imag]])
+    e1, e2 = orc.vieta_residuals(np.zeros((1, 2)), np.array([m]), kappa_s, gamma, np.array(rows))
+    assert e1.max() < 1e-15 and e2.max() < 1e-15
