@@ -203,7 +203,8 @@ def main():
         # the very first call has no previous step to compare with (`prev` is uninitialised memory, for which the
         # matcher falls back to its O(n^2) search): it checks the sets against themselves
         err, bij = api.match_root_sets(roots, prev if last else roots, 1e-10)
-        last.update(stats=st, err=err, bij=bij)
+        v1, v2 = api.vieta_residuals(xy, m, cfg.kappa_s, cfg.gamma, roots, phi_off, phi_total)   # completeness of every row
+        last.update(stats=st, err=err, bij=bij, v1=v1, v2=v2)
         return st
 
     def barrier():
@@ -230,7 +231,7 @@ def main():
     for _ in range(args.steps):
         st = step()
         solve_ms += st.solve_ms
-        launches += st.kernel_launches + 3 + 1 + (1 if args.separate_caustics else 0)   # star field (3), matcher, caustics
+        launches += st.kernel_launches + 3 + 1 + 2 + (1 if args.separate_caustics else 0)   # star field (3), matcher, Vieta sums (2), caustics
         # root-iterations without the Aberth sum take the Newton step of F and do not accumulate S1 either
         # (R27): their star pairs are 2 flop (one complex addition) lighter
         iters_without_A = st.root_iterations - st.root_pairs / float(n_r - 1)
@@ -244,6 +245,7 @@ def main():
     clocks = sampler.stop() if rank == 0 else None
     st = last["stats"]
     assert bool(last["bij"].all()), "validator: this step's root sets differ from the previous step's"
+    assert float(last["v1"].max()) < 1e-12 and float(last["v2"].max()) < 1e-12, "validator: a row fails Vieta's sums"
     assert st.unconverged_rows == 0 and st.degenerate_roots == 0
     t = torch.tensor([ms], dtype=torch.float64, device="cuda")
     if world > 1:
@@ -424,8 +426,8 @@ def main():
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                 "config": {"workload": f"{cfg.name}: N={cfg.N} stars, {num_phi} phases per GPU, kappa_star={cfg.kappa_star}, "
                                        f"kappa_s={cfg.kappa_s}, gamma={cfg.gamma}, tol={cfg.tol}, max_iter={cfg.max_iter}, seed={cfg.seed}",
-                           "step": ("star_field + critical_curves_ex + caustics + match_root_sets" if args.separate_caustics
-                                    else "star_field + curves_and_caustics (fused) + match_root_sets"),
+                           "step": ("star_field + critical_curves_ex + caustics + match_root_sets + vieta_residuals" if args.separate_caustics
+                                    else "star_field + curves_and_caustics (fused) + match_root_sets + vieta_residuals"),
                            "aberth_sum_precision": st.aberth_sum_precision, "star_sums": args.star_sums, "trust_predictor": bool(args.trust_predictor),
                            "subchains": st.subchains, "predictor_order": st.predictor_order,
                            "l2": f"inputs larger than L2: each step writes {2 * num_phi * n_r * 16 / 1e9:.2f} GB of roots and caustics "

@@ -244,6 +244,25 @@ int mlcc_star_sums(const double *star_xy, const double *masses, int64_t N, const
 int mlcc_match_root_sets(const double *a, const double *b, int64_t S, int64_t n, double rel_tol,
                          double *out_max_err, int32_t *out_bijective, void *stream);
 
+/* a8, invariants  Completeness certificate of the root sets (BASELINE.json
+ * north_star: "exactly the paper's degree of distinct roots per phase").  P(z; phi) =
+ * F(z, phi) prod_i (z - z_i)^2 has degree 2N and leading coefficient -c(phi),
+ * c = (1 - kappa_s) e^{-i phi} - gamma; its next two coefficients give Vieta's sums
+ *   sum_k z_k = 2 sum_i z_i,      sum_k z_k^2 = 2 sum_i z_i^2 + 2 (sum_i m_i) / c(phi),
+ * which hold for the full set of 2N roots and fail by the displacement if a root is duplicated,
+ * missing or misplaced.  O(2N) per row, no second solve needed.  Disc fields only (no sheet_poly).
+ *   roots [num_phi][2N][2]: device, read; row j has phase 2 pi (j + phi_index_offset) / phi_index_total
+ *   (phi_index_total = 0: num_phi).
+ *   out_e1 [num_phi]: device, |sum z_k - 2 sum z_i| / sum |z_k|.
+ *   out_e2 [num_phi]: device, |sum z_k^2 - 2 sum z_i^2 - 2 M / c| / sum |z_k|^2.
+ * Converged fp64 root sets give values of order 1e-14 (1e-12 is a safe threshold); a duplicated root
+ * gives |z_a - z_b| / sum |z_k|.  Sums in a fixed order: the same bits on every run.
+ * Asynchronous on `stream`.  Errors: INVALID_ARG, CUDA, NOMEM.                                    */
+int mlcc_vieta_residuals(const double *star_xy, const double *masses, int64_t N, double kappa_s,
+                         double gamma, const double *roots, int64_t num_phi,
+                         int64_t phi_index_offset, int64_t phi_index_total,
+                         double *out_e1, double *out_e2, void *stream);
+
 /* (f) NEXT-4, as far as the crossing map needs it: chain joining (fn. 5 at :217: "the
  * start of one chain is the end of another, with chains joining together until closed loops are
  * formed").  Row s of `rows` holds n points in any column order (the root sets of consecutive

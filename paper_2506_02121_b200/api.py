@@ -106,6 +106,7 @@ def lib() -> C.CDLL:
         L.mlcc_distance_map.argtypes = [vp, i32, i32, dbl, vp, vp, vp]
         L.mlcc_directional_distance_map.argtypes = [vp, i32, i32, dbl, i32, i32, vp, vp]
         L.mlcc_distance_histogram.argtypes = [vp, vp, i64, dbl, i32, i32, vp, vp, vp]
+        L.mlcc_vieta_residuals.argtypes = [vp, vp, i64, dbl, dbl, vp, i64, i64, i64, vp, vp, vp]
         L.mlcc_star_sums.argtypes = [vp, vp, i64, vp, i64, C.c_int, C.c_int, C.c_int, vp, vp]
         L.mlcc_plan_subchains.argtypes = [i64, i64, i32, i32, vp, vp, vp]
         L.mlcc_critical_curves_host.argtypes = [vp, vp, i64, dbl, dbl, i64, dbl, i32, vp]
@@ -304,6 +305,22 @@ def caustics(star_xy, masses, kappa_s, gamma, points, out=None):
     if rc != MLCC_OK:
         _raise(rc)
     return out
+
+
+def vieta_residuals(star_xy, masses, kappa_s, gamma, roots, phi_index_offset=0, phi_index_total=0):
+    """mlcc_vieta_residuals: roots [num_phi, 2N, 2] -> (e1 [num_phi], e2 [num_phi]) relative defects of Vieta's sums."""
+    N = masses.shape[0]
+    if roots.dim() != 3 or roots.shape[1] != 2 * N or roots.shape[2] != 2:
+        raise ValueError("roots must be [num_phi, 2N, 2]")
+    num_phi = roots.shape[0]
+    e1 = torch.empty((num_phi,), dtype=torch.float64, device=roots.device)
+    e2 = torch.empty((num_phi,), dtype=torch.float64, device=roots.device)
+    rc = lib().mlcc_vieta_residuals(_dev(star_xy, name="star_xy"), _dev(masses, name="masses"), N, float(kappa_s),
+                                    float(gamma), _dev(roots, name="roots"), num_phi, int(phi_index_offset),
+                                    int(phi_index_total), e1.data_ptr(), e2.data_ptr(), _stream())
+    if rc != MLCC_OK:
+        _raise(rc)
+    return e1, e2
 
 
 def link_rows(rows):

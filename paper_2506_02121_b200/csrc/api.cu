@@ -64,6 +64,8 @@ int distance_histogram_impl(const double *, const int32_t *, int64_t, double, in
                             cudaStream_t);
 int match_root_sets_impl(const double *, const double *, int64_t, int64_t, double, double *, int32_t *,
                          cudaStream_t);
+int vieta_residuals_impl(const double *, const double *, int64_t, double, double, const double *, int64_t, int64_t,
+                         int64_t, double *, double *, cudaStream_t);
 
 namespace {
 
@@ -309,6 +311,14 @@ int mlcc_distance_histogram(const double *distance, const int32_t *crossing_map,
 {
     return distance_histogram_impl(distance, crossing_map, num_pixels, bin_width, num_bins, num_counts, out_hist,
                                    out_left_out, static_cast<cudaStream_t>(stream));
+}
+
+int mlcc_vieta_residuals(const double *star_xy, const double *masses, int64_t N, double kappa_s, double gamma,
+                         const double *roots, int64_t num_phi, int64_t phi_index_offset, int64_t phi_index_total,
+                         double *out_e1, double *out_e2, void *stream)
+{
+    return vieta_residuals_impl(star_xy, masses, N, kappa_s, gamma, roots, num_phi, phi_index_offset, phi_index_total,
+                                out_e1, out_e2, static_cast<cudaStream_t>(stream));
 }
 
 int mlcc_star_sums(const double *star_xy, const double *masses, int64_t N, const double *points, int64_t P,

@@ -174,7 +174,105 @@ __global__ void __launch_bounds__(BLOCK) k_match(const double2 *__restrict__ a, 
     }
 }
 
+// ---- completeness certificate: Vieta's first two sums of every row ----
+// P(z; phi) = F(z, phi) prod (z - z_i)^2 has degree 2N and leading coefficient -c(phi); its next two
+// coefficients give  sum_k z_k = 2 sum_i z_i  and  sum_k z_k^2 = 2 sum_i z_i^2 + 2 (sum_i m_i)/c(phi).
+constexpr int VBLOCK = 256;
+
+// block-wide sum of NQ doubles per thread in a fixed order (the same bits every run); result in every thread
+template <int NQ>
+__device__ __forceinline__ void block_sum(double (&v)[NQ], double *s_buf /*[NQ][VBLOCK / 32]*/)
+{
+#pragma unroll
+    for (int q = 0; q < NQ; ++q)
+        for (int o = 16; o > 0; o >>= 1) v[q] += __shfl_xor_sync(0xffffffffu, v[q], o);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    __syncthreads();
+    if (lane == 0)
+#pragma unroll
+        for (int q = 0; q < NQ; ++q) s_buf[q * (VBLOCK / 32) + warp] = v[q];
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) {
+        double t = 0.0;
+        for (int w = 0; w < VBLOCK / 32; ++w) t += s_buf[q * (VBLOCK / 32) + w];
+        v[q] = t;
+    }
+}
+
+// one CTA: star_sums = {Re sum z_i, Im sum z_i, Re sum z_i^2, Im sum z_i^2, sum m_i}
+__global__ void __launch_bounds__(VBLOCK) k_vieta_stars(const double2 *__restrict__ stars, const double *__restrict__ masses,
+                                                        int N, double *star_sums)
+{
+    __shared__ double s_buf[5 * (VBLOCK / 32)];
+    double v[5] = {0, 0, 0, 0, 0};
+    for (int i = threadIdx.x; i < N; i += VBLOCK) {
+        const double2 z = stars[i];
+        v[0] += z.x; v[1] += z.y;
+        v[2] += z.x * z.x - z.y * z.y; v[3] += 2.0 * z.x * z.y;
+        v[4] += masses[i];
+    }
+    block_sum<5>(v, s_buf);
+    if (threadIdx.x < 5) star_sums[threadIdx.x] = v[threadIdx.x];
+}
+
+// one CTA per row (grid-stride): relative defects of the two sums
+__global__ void __launch_bounds__(VBLOCK) k_vieta_rows(const double2 *__restrict__ roots, long long num_phi, int n_r,
+                                                       const double *__restrict__ star_sums, double omk, double gamma,
+                                                       long long phi_off, long long phi_total,
+                                                       double *__restrict__ out_e1, double *__restrict__ out_e2)
+{
+    __shared__ double s_buf[6 * (VBLOCK / 32)];
+    for (long long j = blockIdx.x; j < num_phi; j += gridDim.x) {
+        const double2 *row = roots + j * n_r;
+        double v[6] = {0, 0, 0, 0, 0, 0};
+        for (int k = threadIdx.x; k < n_r; k += VBLOCK) {
+            const double2 z = row[k];
+            const double a2 = z.x * z.x + z.y * z.y;
+            v[0] += z.x; v[1] += z.y;
+            v[2] += z.x * z.x - z.y * z.y; v[3] += 2.0 * z.x * z.y;
+            v[4] += sqrt(a2); v[5] += a2;
+        }
+        block_sum<6>(v, s_buf);
+        if (threadIdx.x == 0) {
+            double sn, cs;
+            sincospi(2.0 * (double)(j + phi_off) / (double)phi_total, &sn, &cs);
+            const double cx = omk * cs - gamma, cy = -omk * sn;            // c = (1 - kappa_s) e^{-i phi} - gamma
+            const double c2 = cx * cx + cy * cy;
+            const double qx = 2.0 * star_sums[4] * cx / c2, qy = -2.0 * star_sums[4] * cy / c2;   // 2 M / c
+            const double d1x = v[0] - 2.0 * star_sums[0], d1y = v[1] - 2.0 * star_sums[1];
+            const double d2x = v[2] - 2.0 * star_sums[2] - qx, d2y = v[3] - 2.0 * star_sums[3] - qy;
+            out_e1[j] = sqrt(d1x * d1x + d1y * d1y) / v[4];
+            out_e2[j] = sqrt(d2x * d2x + d2y * d2y) / v[5];
+        }
+        __syncthreads();
+    }
+}
+
 }  // namespace
+
+int vieta_residuals_impl(const double *star_xy, const double *masses, int64_t N, double kappa_s, double gamma,
+                         const double *roots, int64_t num_phi, int64_t phi_index_offset, int64_t phi_index_total,
+                         double *out_e1, double *out_e2, cudaStream_t stream)
+{
+    if (num_phi < 0) return invalid("num_phi < 0");
+    if (N < 1 || N > (1 << 28)) return invalid("N out of range");
+    if (!isfinite(kappa_s) || !isfinite(gamma)) return invalid("kappa_s / gamma not finite");
+    if (num_phi == 0) return MLCC_OK;
+    if (!star_xy || !masses || !roots || !out_e1 || !out_e2) return invalid("null pointer");
+    const int64_t total = phi_index_total > 0 ? phi_index_total : num_phi;
+    Workspace ws(stream);
+    double *star_sums = nullptr;
+    MLCC_CUDA(ws.alloc(&star_sums, 5));
+    k_vieta_stars<<<1, VBLOCK, 0, stream>>>(reinterpret_cast<const double2 *>(star_xy), masses, (int)N, star_sums);
+    long long grid = 8ll * device_sm_count();
+    if (grid > num_phi) grid = num_phi;
+    k_vieta_rows<<<(unsigned)grid, VBLOCK, 0, stream>>>(reinterpret_cast<const double2 *>(roots), (long long)num_phi,
+                                                       (int)(2 * N), star_sums, 1.0 - kappa_s, gamma,
+                                                       (long long)phi_index_offset, (long long)total, out_e1, out_e2);
+    MLCC_CUDA(cudaGetLastError());
+    return MLCC_OK;
+}
 
 static int match_launch(const double *a, const double *b, int64_t S, int64_t n, double rel_tol,
                         double *out_max_err, int32_t *out_bijective, long long b_shift, int32_t *out_index,

@@ -146,6 +146,13 @@ def test_invalid_arguments_fail_before_any_cuda_call(lib):
     assert L.mlcc_distance_histogram(one, None, 64, 0.0, 8, 1, one, one, None) == api.MLCC_ERR_INVALID_ARG
     assert L.mlcc_distance_histogram(one, None, 64, 0.1, 0, 1, one, one, None) == api.MLCC_ERR_INVALID_ARG
     assert L.mlcc_distance_histogram(one, None, 64, 0.1, 1 << 20, 1 << 10, one, one, None) == api.MLCC_ERR_INVALID_ARG
+    L.mlcc_vieta_residuals.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_double, C.c_void_p, C.c_int64,
+                                       C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
+    assert L.mlcc_vieta_residuals(None, one, 3, 0.0, 0.1, one, 4, 0, 0, one, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_vieta_residuals(one, one, 0, 0.0, 0.1, one, 4, 0, 0, one, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_vieta_residuals(one, one, 3, float("nan"), 0.1, one, 4, 0, 0, one, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_vieta_residuals(one, one, 3, 0.0, 0.1, one, 4, 0, 0, None, one, None) == api.MLCC_ERR_INVALID_ARG
+    assert L.mlcc_vieta_residuals(one, one, 3, 0.0, 0.1, None, 0, 0, 0, None, None, None) == api.MLCC_OK    # no rows
     o = api.mlcc_options()
     L.mlcc_options_default(C.byref(o))
     assert o.struct_size == C.sizeof(api.mlcc_options) and o.star_sum_mode == api.MLCC_STAR_SUMS_DIRECT

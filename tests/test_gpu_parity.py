@@ -167,6 +167,41 @@ def test_full_size_sampled_rows_and_invariants(api, orc, name, sample_rows):
                              cplx(roots[int(j)].cpu().numpy()))
 
 
+@pytest.mark.parametrize("name,num_phi", [("cfg1", 1000), ("cfg2", 777), ("cfg3", 64)])
+def test_vieta_residuals_against_oracle(api, orc, name, num_phi):
+    """mlcc_vieta_residuals (the validator's invariant half) on GPU root sets: tiny on every row, equal to the oracle's
+    long-double evaluation within rounding; a duplicated root and a wrong phase offset are reported by both alike."""
+    cfg = CONFIGS[name]
+    xy, m, R = field(orc, cfg)
+    roots, _, unconv, _ = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, num_phi, cfg.tol, cfg.max_iter)
+    assert int(unconv.sum()) == 0
+    e1, e2 = api.vieta_residuals(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, roots)
+    o1, o2 = orc.vieta_residuals(xy, m, cfg.kappa_s, cfg.gamma, roots.cpu().numpy())
+    assert float(e1.max()) < 1e-12 and float(e2.max()) < 1e-12 and o1.max() < 1e-12 and o2.max() < 1e-12
+    assert np.abs(e1.cpu().numpy() - o1).max() < 1e-14 and np.abs(e2.cpu().numpy() - o2).max() < 1e-14
+    bad = roots.clone()
+    bad[5, 3] = bad[5, 4]                                  # row 5: one root twice, one missing
+    bad[9, 0, 0] += 1e-6                                    # row 9: one root misplaced by 1e-6
+    b1, b2 = api.vieta_residuals(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, bad)
+    p1, p2 = orc.vieta_residuals(xy, m, cfg.kappa_s, cfg.gamma, bad.cpu().numpy())
+    assert np.allclose(b1.cpu().numpy()[[5, 9]], p1[[5, 9]], rtol=1e-6) and np.allclose(b2.cpu().numpy()[[5, 9]], p2[[5, 9]], rtol=1e-6)
+    assert float(b1[5]) > 1e-6 and float(b1[9]) > 1e-6 / float(roots[9].norm(dim=1).sum()) * 0.99
+    ok = np.ones(num_phi, bool)
+    ok[[5, 9]] = False
+    assert float(b1.cpu().numpy()[ok].max()) < 1e-12
+    # rows of a larger grid (multi-GPU sharding, mlcc_options.phi_index_offset / _total)
+    part, _, _, _ = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, 16, cfg.tol, cfg.max_iter,
+                                           opt=api.options(phi_index_offset=40, phi_index_total=num_phi))
+    s1, s2 = api.vieta_residuals(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, part, 40, num_phi)
+    q1, q2 = orc.vieta_residuals(xy, m, cfg.kappa_s, cfg.gamma, part.cpu().numpy(), 40, num_phi)
+    assert float(s2.max()) < 1e-12 and q2.max() < 1e-12
+    w1, w2 = api.vieta_residuals(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, part, 0, num_phi)       # wrong offset
+    assert float(w2.min()) > 1e-9 and float(w1.max()) < 1e-12                                    # only the second sum has phi
+    empty = api.vieta_residuals(dev(xy), dev(m), cfg.kappa_s, cfg.gamma,
+                                torch.empty((0, 2 * cfg.N, 2), dtype=torch.float64, device="cuda"))
+    assert empty[0].shape == (0,)
+
+
 def test_bench_configuration_full_size_cfg4(api, orc):
     """The call bench.py times, as it times it: mlcc_star_field + the FUSED mlcc_curves_and_caustics with default
     options on cfg4 at its full size (10^4 phases x 2*10^4 roots) + mlcc_match_root_sets.  Sampled rows (roots and
@@ -189,6 +224,8 @@ def test_bench_configuration_full_size_cfg4(api, orc):
         assert_rows_match(orc, g, ref)
         w_ref = orc.caustics(oxy, om, cfg.kappa_s, cfg.gamma, ref)
         assert_caustics_match(g[0], caus[j].cpu().numpy(), ref[0], w_ref[0])
+    g1, g2 = api.vieta_residuals(xy_o, m_o, cfg.kappa_s, cfg.gamma, roots)       # the library's own certificate
+    assert float(g1.max()) < 1e-12 and float(g2.max()) < 1e-12
     again, caus2, _, _, _ = api.curves_and_caustics(xy_o, m_o, cfg.kappa_s, cfg.gamma, cfg.num_phi, cfg.tol,
                                                     cfg.max_iter, want_diagnostics=False)
     err, bij = api.match_root_sets(again, roots, 1e-10)
