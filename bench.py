@@ -75,8 +75,25 @@ class ClockSampler:
 
     def __init__(self, gpu_index=0, period_ms=200):
         self.rows, self.proc, self.thread, self.gpu, self.period_ms = [], None, None, gpu_index, int(period_ms)
+        self.nvml, self.handle, self.running, self.smax = None, None, False, 0.0
 
     def start(self):
+        # In-process NVML first (four light queries per sample).  An nvidia-smi -lms loop beside the run was measured
+        # to stall this process's kernel launches now and then (profiles/r01_bench_cfg4.md: 85 ms of non-solve time per
+        # step without it, 85-260 ms with it); it is kept only as the fallback when pynvml is not importable.
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nvml = pynvml
+            self.handle = pynvml.nvmlDeviceGetHandleByIndex(self.gpu)
+            self.smax = float(pynvml.nvmlDeviceGetMaxClockInfo(self.handle, pynvml.NVML_CLOCK_SM))
+            self.running = True
+            self.proc = "nvml"
+            self.thread = threading.Thread(target=self._read_nvml, daemon=True)
+            self.thread.start()
+            return
+        except Exception:
+            self.nvml = None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
                                           "-lms", str(self.period_ms), "-i", str(self.gpu)], stdout=subprocess.PIPE,
@@ -87,21 +104,44 @@ class ClockSampler:
         self.thread = threading.Thread(target=self._read, daemon=True)
         self.thread.start()
 
+    def _read_nvml(self):
+        nv, h = self.nvml, self.handle
+        bits = ((nv.nvmlClocksThrottleReasonHwSlowdown, 5), (nv.nvmlClocksThrottleReasonHwThermalSlowdown, 6),
+                (nv.nvmlClocksThrottleReasonSwThermalSlowdown, 7), (nv.nvmlClocksThrottleReasonSwPowerCap, 8))
+        while self.running:
+            try:
+                row = [str(self.gpu), str(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)), str(self.smax),
+                       str(nv.nvmlDeviceGetPowerUsage(h) / 1000.0), "", "", "", "", ""]
+                mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                for bit, col in bits:
+                    row[col] = "Active" if (mask & bit) else "Not Active"
+                self.rows.append((time.time(), row))
+            except Exception:
+                pass
+            time.sleep(self.period_ms / 1000.0)
+
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append([c.strip() for c in line.split(",")])
+            self.rows.append((time.time(), [c.strip() for c in line.split(",")]))
 
-    def stop(self):
+    def stop(self, t_begin=None, t_end=None):
+        """Summary of the samples that arrived in [t_begin, t_end] (the timed region; None = all of them)."""
         if not self.proc:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        self.proc.terminate()
-        try:
-            self.proc.wait(timeout=5)
-        except subprocess.TimeoutExpired:
-            self.proc.kill()
+        if self.proc == "nvml":
+            self.running = False
+            self.thread.join(timeout=5)
+        else:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except subprocess.TimeoutExpired:
+                self.proc.kill()
         sm, smax, power, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for r in self.rows:
+        for when, r in self.rows:
+            if (t_begin is not None and when < t_begin) or (t_end is not None and when > t_end):
+                continue
             if len(r) < 9:
                 continue
             try:
@@ -112,7 +152,8 @@ class ClockSampler:
                 if v.lower().startswith("active"):
                     reasons.add(n)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
-                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons),
+                "source": "nvml (in-process)" if self.proc == "nvml" else "nvidia-smi -lms"}
 
 
 def oracle_sample(cfg, rows, num_phi_total, j_offset=0):
@@ -212,14 +253,17 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    # The clock sampler is started BEFORE the warm-up: nvidia-smi takes a few hundred ms to attach to the driver, and
+    # while it does, kernel launches of this process can stall (seen as 100-200 ms added to one timed step).  Only the
+    # samples that arrive inside the timed region are reported.
+    sampler = ClockSampler(local_rank, args.clock_sample_ms)
+    if rank == 0 and args.clock_sample_ms > 0:
+        sampler.start()
     # warm-up (also fills `prev` for the validator)
     for w in range(max(args.warmup, 1)):
         step()
         prev.copy_(roots)
     barrier()
-    sampler = ClockSampler(local_rank, args.clock_sample_ms)
-    if rank == 0:
-        sampler.start()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     solve_ms = 0.0
     launches = 0
@@ -227,6 +271,7 @@ def main():
     alg_flop_survey = 0.0
     compute_launches = 0
     barrier()
+    t_begin = time.time()
     ev0.record()
     for _ in range(args.steps):
         st = step()
@@ -242,7 +287,7 @@ def main():
     ev1.record()
     barrier()
     ms = ev0.elapsed_time(ev1)
-    clocks = sampler.stop() if rank == 0 else None
+    clocks = sampler.stop(t_begin, time.time()) if rank == 0 else None
     st = last["stats"]
     assert bool(last["bij"].all()), "validator: this step's root sets differ from the previous step's"
     assert float(last["v1"].max()) < 1e-12 and float(last["v2"].max()) < 1e-12, "validator: a row fails Vieta's sums"

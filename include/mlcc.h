@@ -391,7 +391,11 @@ int mlcc_plan_subchains(int64_t N, int64_t num_phi, int32_t num_subchains, int32
 /* Host-buffer variants (every pointer is a HOST pointer; the library allocates device memory,
  * copies in, runs the device path above on the default stream, copies out and frees).
  * mlcc_curves_and_caustics_host runs the fused a1..a7 pass (mlcc_curves_and_caustics);
- * out_caustics may be NULL (critical curves only).                                               */
+ * out_caustics may be NULL (critical curves only).  If out_roots (and out_caustics) are pinned or
+ * registered host memory, the rows of every finished step are copied device -> host on a second
+ * stream while the later rows are still being solved (a sub-chain's finished rows are one interval
+ * growing at both ends), so the 32 bytes per root cross PCIe under the kernels;
+ * pageable outputs are copied once at the end.  The results are the same bits either way.          */
 int mlcc_critical_curves_host(const double *star_xy, const double *masses, int64_t N,
                               double kappa_s, double gamma, int64_t num_phi, double tol,
                               int32_t max_iter, double *out_roots);

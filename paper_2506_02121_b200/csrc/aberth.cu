@@ -37,6 +37,7 @@
 #include "star_sums.cuh"
 
 #include <math.h>
+#include <algorithm>
 #include <vector>
 
 namespace mlcc {
@@ -1094,11 +1095,16 @@ int plan_subchains_host(int64_t N, int64_t num_phi, int32_t num_subchains, int32
     return (int)n;
 }
 
+// h_roots / h_caustics (host-buffer entry points; may be null): PINNED host arrays of the shape of out_roots /
+// out_caustics.  Rows are final as soon as their step is over (nothing writes them again, the predictor only reads
+// them) and a sub-chain's finished rows are one interval that grows at both ends, so the rows each poll of the state
+// reports finished are copied device -> host on a second, non-blocking stream while the solve goes on: the 16 bytes
+// per root and per caustic point of the output cross PCIe under the kernels instead of after them.
 int critical_curves_impl(const double *star_xy, const double *masses, int64_t N, double kappa_s,
                          double gamma, int64_t num_phi, double tol, int32_t max_iter,
                          double *out_roots, double *out_caustics, const mlcc_options *opt_in,
                          const double *init_roots, int32_t *out_iters, int32_t *out_unconverged,
-                         mlcc_stats *out_stats, cudaStream_t stream)
+                         mlcc_stats *out_stats, cudaStream_t stream, double *h_roots, double *h_caustics)
 {
     if (!star_xy || !masses || !out_roots) return invalid("null pointer");
     if (N < 1 || N > (1 << 28)) return invalid("N out of range");
@@ -1322,6 +1328,28 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     int which = 0;
     bool finished = false;
     int rc = MLCC_OK;
+    // progressive copy of finished rows to the host (see the comment above the function)
+    cudaStream_t copy_stream = nullptr;
+    std::vector<long long> c_lo(n_sub, 0), c_hi(n_sub, -1);   // rows of sub-chain c already handed to the copy stream
+    if (h_roots) MLCC_CUDA(cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking));
+    auto copy_rows = [&](long long a, long long b) {
+        if (a > b) return;
+        const size_t off = (size_t)a * n_r * 2, bytes = (size_t)(b - a + 1) * n_r * 2 * sizeof(double);
+        cudaMemcpyAsync(h_roots + off, out_roots + off, bytes, cudaMemcpyDeviceToHost, copy_stream);
+        if (h_caustics && out_caustics)
+            cudaMemcpyAsync(h_caustics + off, out_caustics + off, bytes, cudaMemcpyDeviceToHost, copy_stream);
+    };
+    // the rows solved in steps < steps_final are final: row centre +- q, q < steps_final, inside the sub-chain
+    auto copy_finished = [&](long long steps_final) {
+        if (!h_roots || steps_final < 1) return;
+        for (int c = 0; c < n_sub; ++c) {
+            const long long lo = std::max(first[c], centre[c] - (steps_final - 1));
+            const long long hi = std::min(end[c] - 1, centre[c] + (steps_final - 1));
+            if (c_lo[c] > c_hi[c]) copy_rows(lo, hi);
+            else { copy_rows(lo, c_lo[c] - 1); copy_rows(c_hi[c] + 1, hi); }
+            c_lo[c] = lo; c_hi[c] = hi;
+        }
+    };
     while (!finished && groups < max_groups + 2 * chunk) {
         for (int g = 0; g < chunk; ++g) {
             ks.seed<<<grid_seed, BLOCK, 0, stream>>>(p);
@@ -1343,6 +1371,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
             cudaError_t es = cudaEventSynchronize(ev_poll[which ^ 1]);
             if (es != cudaSuccess) { rc = cuda_fail(es, "cudaEventSynchronize", __FILE__, __LINE__); break; }
             if (h_state[which ^ 1].done) finished = true;
+            copy_finished(h_state[which ^ 1].step);   // that snapshot is complete: every launch before it has run
         }
         which ^= 1;
     }
@@ -1354,6 +1383,12 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
         if (es == cudaSuccess) es = cudaGetLastError();
         if (es != cudaSuccess) rc = cuda_fail(es, "critical-curve kernels", __FILE__, __LINE__);
         else fin = h_state[0];
+    }
+    if (copy_stream) {
+        if (rc == MLCC_OK && fin.done) copy_finished((long long)max_steps + 1);   // whatever is left
+        cudaError_t es = cudaStreamSynchronize(copy_stream);
+        cudaStreamDestroy(copy_stream);
+        if (rc == MLCC_OK && es != cudaSuccess) rc = cuda_fail(es, "device -> host copy of the rows", __FILE__, __LINE__);
     }
     float ms = 0.f;
     if (rc == MLCC_OK) cudaEventElapsedTime(&ms, ev0, ev1);

@@ -45,7 +45,7 @@ int device_sm_count()
 int plan_subchains_host(int64_t, int64_t, int32_t, int32_t, int64_t *, int64_t *, int64_t *);
 int critical_curves_impl(const double *, const double *, int64_t, double, double, int64_t, double, int32_t,
                          double *, double *, const mlcc_options *, const double *, int32_t *, int32_t *,
-                         mlcc_stats *, cudaStream_t);
+                         mlcc_stats *, cudaStream_t, double *h_roots = nullptr, double *h_caustics = nullptr);
 int caustics_impl(const double *, const double *, int64_t, double, double, const double *, int64_t, double *,
                   cudaStream_t);
 int star_field_impl(uint64_t, int64_t, double, int, const double *, double, double *, double *, double *, double *,
@@ -124,6 +124,16 @@ __global__ void __launch_bounds__(256) k_issue_probe(double *sink, int iters, do
 #pragma unroll
     for (int u = 0; u < 8; ++u) s += x[u] + __longlong_as_double((long long)f[u]);
     if (s == 1.2345e-300) sink[0] = s;  // never true; keeps the chains alive
+}
+
+bool host_is_pinned(const void *p)
+{
+    cudaPointerAttributes a{};
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return a.type == cudaMemoryTypeHost;
 }
 
 struct DeviceBuffer {
@@ -358,14 +368,20 @@ int mlcc_curves_and_caustics_host(const double *star_xy, const double *masses, i
     if (out_caustics) MLCC_CUDA(d_caus.alloc(sizeof(double) * 2 * n_pts));
     MLCC_CUDA(cudaMemcpyAsync(d_xy.p, star_xy, sizeof(double) * 2 * (size_t)N, cudaMemcpyHostToDevice, 0));
     MLCC_CUDA(cudaMemcpyAsync(d_m.p, masses, sizeof(double) * (size_t)N, cudaMemcpyHostToDevice, 0));
+    // Pinned (or registered) host outputs receive the finished rows while the solve runs; pageable ones would make
+    // every copy block the host thread that feeds the launches, so they are copied once, at the end.
+    const bool overlap = host_is_pinned(out_roots) && (!out_caustics || host_is_pinned(out_caustics));
     const int rc = critical_curves_impl(d_xy.as<double>(), d_m.as<double>(), N, kappa_s, gamma, num_phi, tol,
                                         max_iter, d_roots.as<double>(), out_caustics ? d_caus.as<double>() : nullptr,
-                                        opt, nullptr, nullptr, nullptr, out_stats, nullptr);
+                                        opt, nullptr, nullptr, nullptr, out_stats, nullptr,
+                                        overlap ? out_roots : nullptr, overlap ? out_caustics : nullptr);
     if (rc != MLCC_OK && rc != MLCC_ERR_NOT_CONVERGED && rc != MLCC_ERR_DEGENERATE) return rc;
     const std::string keep = g_last_error;
-    MLCC_CUDA(cudaMemcpyAsync(out_roots, d_roots.p, sizeof(double) * 2 * n_pts, cudaMemcpyDeviceToHost, 0));
-    if (out_caustics)
-        MLCC_CUDA(cudaMemcpyAsync(out_caustics, d_caus.p, sizeof(double) * 2 * n_pts, cudaMemcpyDeviceToHost, 0));
+    if (!overlap) {
+        MLCC_CUDA(cudaMemcpyAsync(out_roots, d_roots.p, sizeof(double) * 2 * n_pts, cudaMemcpyDeviceToHost, 0));
+        if (out_caustics)
+            MLCC_CUDA(cudaMemcpyAsync(out_caustics, d_caus.p, sizeof(double) * 2 * n_pts, cudaMemcpyDeviceToHost, 0));
+    }
     MLCC_CUDA(cudaStreamSynchronize(0));
     if (rc != MLCC_OK) g_last_error = keep;
     return rc;

@@ -456,6 +456,36 @@ def test_host_buffer_entry_points(api, orc):
     assert np.abs(c2 - orc.caustics(xy, m, cfg.kappa_s, cfg.gamma, ref)).max() < 1e-12
 
 
+@pytest.mark.parametrize("name,num_phi,subchains", [("cfg1", 1000, 0), ("cfg2", 4000, 0), ("cfg2", 1501, 5),
+                                                    ("cfg3", 640, 0), ("cfg3", 97, 1)])
+def test_host_entry_point_with_pinned_outputs_copies_rows_while_solving(api, orc, name, num_phi, subchains):
+    """Pinned host outputs get the finished rows on a second stream while the solve runs (pageable ones are copied
+    once at the end).  Both must deliver, in every row, exactly the bits the device path computes; sentinel values in
+    the destination show that no row is left out, whatever the sub-chain layout and the number of polls."""
+    cfg = CONFIGS[name]
+    xy, m, R = field(orc, cfg)
+    opt = api.options(num_subchains=subchains)
+    d_roots, d_caus, _, _, st = api.curves_and_caustics(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, num_phi, cfg.tol,
+                                                        cfg.max_iter, opt=opt)
+    n_r = 2 * cfg.N
+    p_roots = torch.full((num_phi, n_r, 2), float("nan"), dtype=torch.float64).pin_memory()
+    p_caus = torch.full((num_phi, n_r, 2), float("nan"), dtype=torch.float64).pin_memory()
+    api.curves_and_caustics_host(xy, m, cfg.kappa_s, cfg.gamma, num_phi, cfg.tol, cfg.max_iter, opt=opt,
+                                 out_roots=p_roots, out_caustics=p_caus)
+    assert torch.equal(p_roots, d_roots.cpu()) and torch.equal(p_caus, d_caus.cpu())
+    n_roots, n_caus, _ = api.curves_and_caustics_host(xy, m, cfg.kappa_s, cfg.gamma, num_phi, cfg.tol, cfg.max_iter,
+                                                      opt=opt)                      # pageable numpy outputs
+    assert np.array_equal(n_roots, p_roots.numpy()) and np.array_equal(n_caus, p_caus.numpy())
+    # roots only, pinned
+    p_only = torch.full((num_phi, n_r, 2), float("nan"), dtype=torch.float64).pin_memory()
+    api.curves_and_caustics_host(xy, m, cfg.kappa_s, cfg.gamma, num_phi, cfg.tol, cfg.max_iter, opt=opt,
+                                 out_roots=p_only, want_caustics=False)
+    assert torch.equal(p_only, p_roots)
+    ref_rows = [0, num_phi // 2, num_phi - 1]
+    ref, _, un = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, num_phi, ref_rows[:1], cfg.tol, cfg.max_iter)
+    assert_rows_match(orc, p_roots.numpy()[:1], ref)
+
+
 def test_fp64_peak_probe_is_plausible(api):
     tf = api.fp64_peak(20.0)
     assert 5.0 < tf < 80.0, tf
