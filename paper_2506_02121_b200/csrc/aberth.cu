@@ -1269,7 +1269,11 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     p.grid_ctas = grid_compute;
     p.R = ks.R;
     const double skip_below = opt.skip_aberth_sum_below == 0.0 ? 1e-8 : opt.skip_aberth_sum_below;
-    const bool skip_on = skip_below > 0.0;
+    // The second compute launch per iteration pays off where the Aberth sum is the bulk of the work.  Small fields are
+    // launch bound (cfg1: 2.7 ms per curve set with it, 2.0 ms without): there it is used only if asked for by
+    // an explicit threshold or by trust_predictor.
+    const bool skip_on = skip_below > 0.0 &&
+                         (N >= 512 || opt.skip_aberth_sum_below > 0.0 || opt.trust_predictor != 0);
     p.skip_below2 = skip_on ? skip_below * skip_below : 0.0;
     p.trust = opt.trust_predictor != 0 ? 1 : 0;
     p.poly_n = poly_n;
