@@ -37,6 +37,7 @@
 #include "star_sums.cuh"
 
 #include <math.h>
+#include <stdlib.h>
 #include <algorithm>
 #include <vector>
 
@@ -1095,6 +1096,35 @@ int plan_subchains_host(int64_t N, int64_t num_phi, int32_t num_subchains, int32
     return (int)n;
 }
 
+// The iteration groups are replayed from a CUDA graph (below), and stream capture is not allowed on the legacy
+// default stream: a call on that stream runs on a library-owned stream instead, ordered after the caller's stream by
+// an event at the start; the call synchronises before it returns, which orders it before whatever follows.
+struct RunStream {
+    cudaStream_t run = nullptr;
+    bool owned = false;
+    cudaError_t open(cudaStream_t caller)
+    {
+        run = caller;
+        if (caller != nullptr && caller != cudaStreamLegacy) return cudaSuccess;
+        cudaStream_t s = nullptr;
+        cudaError_t e = cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking);
+        if (e != cudaSuccess) return e;
+        cudaEvent_t ready = nullptr;
+        e = cudaEventCreateWithFlags(&ready, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventRecord(ready, caller);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(s, ready, 0);
+        if (ready) cudaEventDestroy(ready);
+        if (e != cudaSuccess) { cudaStreamDestroy(s); return e; }
+        run = s;
+        owned = true;
+        return cudaSuccess;
+    }
+    ~RunStream()
+    {
+        if (owned) { cudaStreamSynchronize(run); cudaStreamDestroy(run); }
+    }
+};
+
 // h_roots / h_caustics (host-buffer entry points; may be null): PINNED host arrays of the shape of out_roots /
 // out_caustics.  Rows are final as soon as their step is over (nothing writes them again, the predictor only reads
 // them) and a sub-chain's finished rows are one interval that grows at both ends, so the rows each poll of the state
@@ -1191,6 +1221,9 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     const long long n_half = (n_r + 1) / 2 > N ? (n_r + 1) / 2 : N;
     const int N_pad = (int)((n_half + S_TILE - 1) / S_TILE) * S_TILE;
 
+    RunStream run_stream;            // declared before the workspace: destroyed after it
+    MLCC_CUDA(run_stream.open(stream));
+    stream = run_stream.run;
     Workspace ws(stream);
     Params p{};
     double2 *d_rot = nullptr;
@@ -1302,8 +1335,11 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     MLCC_CUDA(cudaEventCreate(&ev1));
     MLCC_CUDA(cudaEventCreateWithFlags(&ev_poll[0], cudaEventDisableTiming));
     MLCC_CUDA(cudaEventCreateWithFlags(&ev_poll[1], cudaEventDisableTiming));
-    DevState *h_state = nullptr;   // pinned, two snapshots
-    MLCC_CUDA(cudaMallocHost(&h_state, 2 * sizeof(DevState)));
+    // pinned, two snapshots.  Allocated once per host thread and kept: cudaMallocHost / cudaFreeHost per call cost
+    // 80-120 ms every few calls on the bench box (seen as calls 5.17-5.21 s long with 5.09 s of solve).
+    static thread_local DevState *tl_state = nullptr;
+    if (!tl_state) MLCC_CUDA(cudaMallocHost(&tl_state, 2 * sizeof(DevState)));
+    DevState *h_state = tl_state;
     h_state[0].done = h_state[1].done = 0;
 
     MLCC_CUDA(cudaEventRecord(ev0, stream));
@@ -1315,7 +1351,6 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
         if (frc != MLCC_OK) {
             cudaEventDestroy(ev0); cudaEventDestroy(ev1);
             cudaEventDestroy(ev_poll[0]); cudaEventDestroy(ev_poll[1]);
-            cudaFreeHost(h_state);
             return frc;
         }
         launches += 9;
@@ -1354,7 +1389,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
             c_lo[c] = lo; c_hi[c] = hi;
         }
     };
-    while (!finished && groups < max_groups + 2 * chunk) {
+    auto enqueue_chunk = [&]() {
         for (int g = 0; g < chunk; ++g) {
             ks.seed<<<grid_seed, BLOCK, 0, stream>>>(p);
             if (use_fmm) {
@@ -1365,6 +1400,36 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
             if (skip_on) ks.compute_noA<<<grid_compute, CTA, 0, stream>>>(p);
             ks.apply<<<grid_apply, APPLY_THREADS, 0, stream>>>(p);
             k_finalize<<<1, FIN, 0, stream>>>(p);
+        }
+    };
+    // Every launch of a chunk has the same arguments (the state lives on the device), so the chunk is captured once
+    // and replayed: small fields are pure launch latency (cfg1: ~8 us per launch from the host).  Any failure of the
+    // capture falls back to plain launches.
+    cudaGraphExec_t chunk_exec = nullptr;
+    {
+        // kernels are loaded lazily at their first launch, and loading is not allowed inside a capture: touch them first
+        cudaFuncAttributes fa;
+        const void *fns[] = {(const void *)ks.seed, (const void *)ks.compute, (const void *)ks.compute_noA,
+                             (const void *)ks.apply, (const void *)k_finalize, (const void *)k_star_sums,
+                             (const void *)k_star_sums_outside};
+        for (const void *f : fns) cudaFuncGetAttributes(&fa, f);
+        cudaGetLastError();
+        cudaGraph_t graph = nullptr;
+        const char *no_graph = getenv("MLCC_NO_GRAPH");   // diagnosis: plain launches
+        if (!(no_graph && no_graph[0] == '1') &&
+            cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+            enqueue_chunk();
+            if (cudaStreamEndCapture(stream, &graph) == cudaSuccess && graph) {
+                if (cudaGraphInstantiate(&chunk_exec, graph, 0) != cudaSuccess) chunk_exec = nullptr;
+            }
+            if (graph) cudaGraphDestroy(graph);
+        }
+        if (!chunk_exec) cudaGetLastError();
+    }
+    while (!finished && groups < max_groups + 2 * chunk) {
+        if (!chunk_exec || cudaGraphLaunch(chunk_exec, stream) != cudaSuccess) {
+            if (chunk_exec) { cudaGetLastError(); cudaGraphExecDestroy(chunk_exec); chunk_exec = nullptr; }
+            enqueue_chunk();
         }
         launches += ((use_fmm ? 6 : 4) + (skip_on ? 1 : 0)) * chunk;
         groups += chunk;
@@ -1379,6 +1444,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
         }
         which ^= 1;
     }
+    if (chunk_exec) cudaGraphExecDestroy(chunk_exec);
     DevState fin{};
     if (rc == MLCC_OK) {
         cudaEventRecord(ev1, stream);
@@ -1398,7 +1464,6 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     if (rc == MLCC_OK) cudaEventElapsedTime(&ms, ev0, ev1);
     cudaEventDestroy(ev0); cudaEventDestroy(ev1);
     cudaEventDestroy(ev_poll[0]); cudaEventDestroy(ev_poll[1]);
-    cudaFreeHost(h_state);
     if (rc != MLCC_OK) return rc;
     if (!fin.done) {
         set_last_error("internal: state machine did not finish");
