@@ -176,14 +176,19 @@ def check_row_invariants(orc, xy, m, kappa_s, gamma, row_index, num_phi, z, min_
     ulp = np.spacing(np.abs(z))
     # residual certificate: the long-double Newton step from the fp64 root is at rounding level.  "Rounding level" is
     # the spacing of z, or -- for an ill-conditioned root (small |F'|) -- what the fp64 evaluation of F itself allows:
-    # F is a sum of N terms m_i/(z-z_i)^2, each term and each addition rounded, so |dF| ~ a few 2^-53 sum |terms| and
-    # the root cannot be placed better than |dF|/|F'| (reading R16; cfg4 has roots with |F'| ~ 1e-3).
+    # F is a sum of N terms m_i/(z-z_i)^2 added one after the other, every addition rounding by up to
+    # 2^-53 |partial sum| <= 2^-53 sum |terms|; N independent roundings add up like a random walk, so F carries
+    # |dF| ~ sqrt(N) 2^-53 sum |terms| and the iteration cannot place the root better than |dF|/|F'| (DESIGN.md reading
+    # R16; the outer pair of cfg4 near phi = 0 sits at |z| ~ 2R where every term has the same phase and |F'| ~ 2e-4).
+    # The factor 4 is the margin over that estimate; `test_r16_condition_term_on_the_oracles_own_cfg4_rows` shows the
+    # oracle's own double solve needs the term on those rows and its long-double solve does not.
     plain = 4 * ulp + 1e-13
     over = np.where(res["newton"] > plain)[0]          # only these need the conditioning term (few, if any)
     for k in over:
-        floor = 8 * 2.0 ** -53 * (m / np.abs(z[k] - zs) ** 2).sum() / np.abs(res["Fp"][k])
+        floor = 4 * np.sqrt(N) * 2.0 ** -53 * (m / np.abs(z[k] - zs) ** 2).sum() / np.abs(res["Fp"][k])
         assert res["newton"][k] <= plain[k] + floor, (k, res["newton"][k], plain[k], floor)
     assert len(over) <= max(2, len(z) // 1000)
+    res["needed_condition_term"] = over
     # scaled det J bound (App. C linearised)
     bound = 1e-10 + 4 * (1 - kappa_s) * np.abs(res["Fp"]) * 2.0 ** -52 * (1 + np.abs(z))
     assert np.all(np.abs(res["inv_mu"]) <= bound), (np.abs(res["inv_mu"]) / bound).max()
@@ -220,6 +225,29 @@ def test_p5_p6_p7_invariants_cfg3_row(orc):
     assert unconv.sum() == 0
     for q, j in enumerate(rows):
         check_row_invariants(orc, xy, m, cfg.kappa_s, cfg.gamma, j, cfg.num_phi, cplx(roots)[q])
+
+
+def test_r16_condition_term_on_the_oracles_own_cfg4_rows(orc):
+    """DESIGN.md reading R16 on the ORACLE's rows (no GPU): the conditioning term of the residual certificate is what
+    an fp64 solve needs, not a kernel allowance.  cfg4, row 0 (phi = 0: |c(phi)| = 0.05, the outer pair at |z| ~ 2R,
+    PAPER.md:422 fn. 7, with |F'| ~ 2e-4) and row 5000 (phi = pi, no such pair): the double solve passes every row
+    invariant, needs the term for a handful of roots on row 0 and for none on row 5000; the long-double solve of the
+    same rows, rounded to fp64, needs it nowhere."""
+    cfg = CONFIGS["cfg4"]
+    xy, m, R = _field(orc, cfg)
+    rows = [0, 5000]
+    need = {}
+    for ld in (False, True):
+        roots, iters, unconv = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, cfg.num_phi, rows, cfg.tol,
+                                                       cfg.max_iter, long_double=ld)
+        assert unconv.sum() == 0 and iters.max() < cfg.max_iter
+        for q, j in enumerate(rows):
+            res = check_row_invariants(orc, xy, m, cfg.kappa_s, cfg.gamma, j, cfg.num_phi, cplx(roots)[q])
+            need[(ld, j)] = np.abs(cplx(roots)[q][res["needed_condition_term"]])   # |z| of the roots that needed it
+    assert 1 <= len(need[(False, 0)]) <= 20          # the fp64 floor is real: the oracle's own double row needs it
+    assert np.all(need[(False, 0)] > 1.5 * R)        # ... and only for the outer pair
+    assert len(need[(False, 5000)]) == 0
+    assert len(need[(True, 0)]) == 0 and len(need[(True, 5000)]) == 0
 
 
 def test_double_vs_long_double_rows(orc):

@@ -59,6 +59,30 @@ def test_b4_bounds_the_truncation_error(orc):
     assert 0.1 * np.pi <= r <= 0.9 * np.pi
 
 
+@pytest.mark.parametrize("ks,c1,c2,s,eps", [(0.4, 4.0, 2.5, 1.5, 1e-9), (0.3, 3.0, 3.0, 1.2, 1e-6), (0.2, 10.0, 1.0, 2.0, 1e-12),
+                                             (0.45, 5.0, 5.0 * np.tan(np.pi / 10), 1.5, 1e-9), (0.1, 1.0, 2.0, 1.05, 1e-3)])
+def test_truncation_power_is_the_smallest_admissible_one(orc, ks, c1, c2, s, eps):
+    """`orc_rect_truncation` returns THE SMALLEST odd t that meets both rules of Appendix B: the error bound B5
+     below eps on |z| <= |c|/s, and (t-1) Arg c at least 0.1 pi away from the multiples of pi
+    (PAPER.md:456).  Brute force over every smaller odd power: each one breaks B5 or the Arg rule."""
+    c, theta = abs(c1 + 1j * c2), np.arctan2(c2, c1)
+
+    def b5_ok(t):
+        return ks / np.pi * 4 / (t + 1) * s ** -(t + 1) * c * (s + 1) / (s - 1) <= eps
+
+    def arg_ok(t):
+        r = ((t - 1) * theta) % np.pi
+        return 0.1 * np.pi <= r <= 0.9 * np.pi
+
+    t = orc.rect_truncation(ks, c1, c2, s, eps)
+    assert t % 2 == 1 and b5_ok(t) and arg_ok(t)
+    smaller = [q for q in range(1, t, 2) if b5_ok(q) and arg_ok(q)]
+    assert smaller == [], smaller
+    # the cases cover both ways of stopping: B5 alone decides (t - 2 breaks it), or the Arg rule pushed t up
+    if b5_ok(t - 2):
+        assert not arg_ok(t - 2)
+
+
 @pytest.mark.parametrize("t", [5, 9, 15])
 def test_b7_b9_are_the_derivatives_of_b2(orc, t):
     """Wirtinger derivatives by central differences: d/dzbar = (d/dx + i d/dy)/2, d/dz = (d/dx - i d/dy)/2."""
