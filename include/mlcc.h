@@ -25,6 +25,10 @@
  *    synchronise that stream before returning.  Entry points without a stream argument use the
  *    default stream and synchronise it.
  *  - Workspace is allocated per call with the stream-ordered allocator and released before return.
+ *    Side effect, process-wide: the first call on a device sets the release threshold of that device's
+ *    DEFAULT CUDA memory pool to "keep" (cudaMemPoolAttrReleaseThreshold), so that the GB-sized scratch is
+ *    not returned to the driver at every synchronisation.  Other cudaMallocAsync users of the same pool see
+ *    their freed blocks cached as well; cudaMemPoolTrimTo releases them.
  *  - Return value: mlcc_status.  Errors never throw or exit; mlcc_last_error() gives the text
  *    of the last failure on the calling thread.
  *  - Thread-safety: re-entrant; concurrent calls must use distinct streams.
@@ -264,6 +268,27 @@ int mlcc_vieta_residuals(const double *star_xy, const double *masses, int64_t N,
                          int64_t phi_index_offset, int64_t phi_index_total,
                          double *out_e1, double *out_e2, void *stream);
 
+/* a8, invariants  det J certificate of stored roots (BASELINE.json north_star: "|det J| <= 1e-10 at every root";
+ * Eq. C1 first line; the bound of C3).  One pass of the star sums at every point:
+ *   F = gamma + S2 - (1 - kappa_s) e^{-i phi}  (Eq. 15),  F' = -2 S3  (Eq. 19),
+ *   1/mu = det J = (1 - kappa_s)^2 - |gamma + S2|^2,      newton = |F| / |F'|,
+ * newton being, to first order, the distance from the point to the exact root of F.  The plain 1e-10 of
+ * BASELINE.json is below what fp64 can represent once |F'| >~ 1e4 (a root 0.03 theta_star from a star, N >~ 2000:
+ * SURVEY.md 0.2), so the certificate is scale-aware:
+ *   bound_k = 1e-10 + 4 (1 - kappa_s) |F'(z_k)| 2^-52 (1 + |z_k|)          (App. C linearised; R16).
+ *   points [num_phi][n][2]: device, read; row j has phase 2 pi (j + phi_index_offset) / phi_index_total
+ *     (phi_index_total = 0: num_phi).  n is free (2N for the root sets of a disc field).
+ *   out_residuals [num_phi][n][6]: device or NULL, written: Re F, Im F, Re F', Im F', 1/mu, newton.
+ *   out_row_newton [num_phi]: device, written: max_k newton.
+ *   out_row_detj [num_phi]: device, written: max_k |1/mu_k| / bound_k  (<= 1 certifies the row).
+ * A point on a star or a non-finite point gives +inf in both row outputs.  Disc fields only (no sheet_poly).
+ * Cost: N pair evaluations per point (20 FP64 instructions each), i.e. about what one confirming iteration of the
+ * solver costs for that point.  Asynchronous on `stream`.  Errors: INVALID_ARG, CUDA, NOMEM.                    */
+int mlcc_detj_residuals(const double *star_xy, const double *masses, int64_t N, double kappa_s, double gamma,
+                        const double *points, int64_t num_phi, int64_t n,
+                        int64_t phi_index_offset, int64_t phi_index_total,
+                        double *out_residuals, double *out_row_newton, double *out_row_detj, void *stream);
+
 /* (f) NEXT-4, as far as the crossing map needs it: chain joining (fn. 5 at :217: "the
  * start of one chain is the end of another, with chains joining together until closed loops are
  * formed").  Row s of `rows` holds n points in any column order (the root sets of consecutive
@@ -406,22 +431,6 @@ int mlcc_curves_and_caustics_host(const double *star_xy, const double *masses, i
                                   double kappa_s, double gamma, int64_t num_phi, double tol,
                                   int32_t max_iter, const mlcc_options *opt,
                                   double *out_roots, double *out_caustics, mlcc_stats *out_stats);
-
-/* Measurement helper: runs a dependent-free DFMA loop on every SM for about `ms_target`
- * milliseconds and returns the FP64 FMA rate reached, in TFLOP/s (2 flop per FMA) through
- * *out_tflops (host).  This is the measured denominator of the "alu" roofline in bench.py
- * (MEASURED_PEAKS.json has no FP64 entry).  Synchronises `stream`.                               */
-int mlcc_fp64_peak(double ms_target, double *out_tflops, void *stream);
-
-/* Measurement helper behind DESIGN.md "Measured issue model": the same loop with other operand forms,
- * rate returned as 2 x FP64 instructions per second / 1e12 (so form 0 equals mlcc_fp64_peak).
- *   form 0: DFMA, two distinct register sources (the peak form)
- *   form 1: DFMA, three distinct register sources
- *   form 2: DADD, two distinct register sources
- *   form 3: form 0 interleaved 1:1 with packed FP32 FMAs (fma.f32x2, three 64-bit sources); the
- *           rate counts the FP64 instructions only
- * Synchronises `stream`.  Errors: INVALID_ARG, CUDA.                                              */
-int mlcc_fp64_issue_probe(int form, double ms_target, double *out_rate, void *stream);
 
 #ifdef __cplusplus
 }

@@ -107,6 +107,7 @@ def lib() -> C.CDLL:
         L.mlcc_directional_distance_map.argtypes = [vp, i32, i32, dbl, i32, i32, vp, vp]
         L.mlcc_distance_histogram.argtypes = [vp, vp, i64, dbl, i32, i32, vp, vp, vp]
         L.mlcc_vieta_residuals.argtypes = [vp, vp, i64, dbl, dbl, vp, i64, i64, i64, vp, vp, vp]
+        L.mlcc_detj_residuals.argtypes = [vp, vp, i64, dbl, dbl, vp, i64, i64, i64, i64, vp, vp, vp, vp]
         L.mlcc_star_sums.argtypes = [vp, vp, i64, vp, i64, C.c_int, C.c_int, C.c_int, vp, vp]
         L.mlcc_plan_subchains.argtypes = [i64, i64, i32, i32, vp, vp, vp]
         L.mlcc_critical_curves_host.argtypes = [vp, vp, i64, dbl, dbl, i64, dbl, i32, vp]
@@ -321,6 +322,24 @@ def vieta_residuals(star_xy, masses, kappa_s, gamma, roots, phi_index_offset=0, 
     if rc != MLCC_OK:
         _raise(rc)
     return e1, e2
+
+
+def detj_residuals(star_xy, masses, kappa_s, gamma, points, phi_index_offset=0, phi_index_total=0, want_points=False):
+    """mlcc_detj_residuals: points [num_phi, n, 2] -> (row_newton [num_phi], row_detj [num_phi], residuals [num_phi, n, 6] or
+    None): per row max |F|/|F'| and max |1/mu| / bound; per point Re F, Im F, Re F', Im F', 1/mu, |F|/|F'|."""
+    if points.dim() != 3 or points.shape[2] != 2:
+        raise ValueError("points must be [num_phi, n, 2]")
+    num_phi, n, _ = points.shape
+    rn = torch.empty((num_phi,), dtype=torch.float64, device=points.device)
+    rd = torch.empty((num_phi,), dtype=torch.float64, device=points.device)
+    res = torch.empty((num_phi, n, 6), dtype=torch.float64, device=points.device) if want_points else None
+    rc = lib().mlcc_detj_residuals(_dev(star_xy, name="star_xy"), _dev(masses, name="masses"), masses.shape[0],
+                                   float(kappa_s), float(gamma), _dev(points, name="points") if num_phi else None,
+                                   num_phi, n, int(phi_index_offset), int(phi_index_total),
+                                   res.data_ptr() if res is not None else None, rn.data_ptr(), rd.data_ptr(), _stream())
+    if rc != MLCC_OK:
+        _raise(rc)
+    return rn, rd, res
 
 
 def link_rows(rows):

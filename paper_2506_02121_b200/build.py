@@ -8,7 +8,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libmlcc.so")
 UNITS = ["api.cu", "aberth.cu", "caustics.cu", "starfield.cu", "match.cu", "fmm.cu", "crossing.cu", "loops.cu",
-         "distance.cu"]
+         "distance.cu", "probe.cu", "certify.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--fmad=true", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
@@ -38,8 +38,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     for u in UNITS:
         obj = os.path.join(objdir, u.replace(".cu", ".o"))
         objs.append(obj)
-        extra = os.environ.get("MLCC_EXTRA_NVCC_FLAGS", "").split()   # tuning experiments only
-        cmd = [nvcc, *NVCC_FLAGS, *extra, "-I", INCLUDE, "-c", os.path.join(CSRC, u), "-o", obj]
+        cmd = [nvcc, *NVCC_FLAGS, "-I", INCLUDE, "-c", os.path.join(CSRC, u), "-o", obj]
         procs.append((u, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     log = []
     for u, pr in procs:

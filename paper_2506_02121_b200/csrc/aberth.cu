@@ -709,6 +709,17 @@ __device__ __forceinline__ bool trusted_step(const Params &p, int step)
     return p.trust && p.skip_below2 > 0.0 && p.order >= 1 && step >= 1 && 2 * step - 1 >= p.order + 1;
 }
 
+// What becomes of a root after a finite step of squared size d2 (both passes of k_apply use this one predicate):
+//   0 frozen (|Delta| < tol), 1 "large": iterated next with the Aberth sum, 2 "small": iterated next without it.
+// guard = first iteration of a trusted row (the steps were Newton steps from predicted seeds): a step of at least
+// the skip threshold is REJECTED -- kind 1 whatever tol is, z unchanged -- and a smaller one is applied.
+__device__ __forceinline__ int step_kind(double d2, double tol2, double skip2, bool guard)
+{
+    if (guard && !(d2 < skip2)) return 1;
+    if (d2 < tol2) return 0;
+    return d2 < skip2 ? 2 : 1;
+}
+
 constexpr int APPLY_THREADS = 1024;
 constexpr int APPLY_ITEMS = 4;
 
@@ -739,7 +750,7 @@ __global__ void __launch_bounds__(APPLY_THREADS) k_apply(Params p)
     for (int pos = tid; pos < n_act; pos += APPLY_THREADS) {
         const double2 d = delta[pos];
         const double d2 = d.x * d.x + d.y * d.y;
-        if (d2 <= 1.79769313486231570e308 && !(d2 < p.tol2) && !(d2 < p.skip_below2)) ++n_large;
+        if (d2 <= 1.79769313486231570e308 && step_kind(d2, p.tol2, p.skip_below2, guard) == 1) ++n_large;
     }
     for (int o = 16; o > 0; o >>= 1) n_large += __shfl_xor_sync(0xffffffffu, n_large, o);
     if (lane == 0) s_warp[warp] = n_large;
@@ -768,15 +779,13 @@ __global__ void __launch_bounds__(APPLY_THREADS) k_apply(Params p)
                 const double2 d = delta[pos];
                 const double d2 = d.x * d.x + d.y * d.y;
                 if (d2 <= 1.79769313486231570e308) {   // finite step
-                    if (guard && !(d2 < p.skip_below2)) {
-                        kind[i] = 1;                    // rejected Newton step: back to the Aberth group, z unchanged
-                    } else {
+                    kind[i] = step_kind(d2, p.tol2, p.skip_below2, guard);
+                    if (!(guard && kind[i] == 1)) {     // (a rejected Newton step leaves z where it is)
                         double2 z = row[k];
                         z.x -= d.x;
                         z.y -= d.y;
                         row[k] = z;
                         store_src<MODE>(slot_src, k, z);
-                        if (!(d2 < p.tol2)) kind[i] = (d2 < p.skip_below2) ? 2 : 1;
                     }
                 } else {                                // NaN / Inf: freeze where it is, report
                     atomicAdd(&p.state->degenerate, 1);
@@ -1330,16 +1339,15 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     p.max_steps = max_steps;
     p.max_slots = max_slots;
 
-    cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev_poll[2] = {nullptr, nullptr};
-    MLCC_CUDA(cudaEventCreate(&ev0));
-    MLCC_CUDA(cudaEventCreate(&ev1));
-    MLCC_CUDA(cudaEventCreateWithFlags(&ev_poll[0], cudaEventDisableTiming));
-    MLCC_CUDA(cudaEventCreateWithFlags(&ev_poll[1], cudaEventDisableTiming));
-    // pinned, two snapshots.  Allocated once per host thread and kept: cudaMallocHost / cudaFreeHost per call cost
-    // 80-120 ms every few calls on the bench box (seen as calls 5.17-5.21 s long with 5.09 s of solve).
-    static thread_local DevState *tl_state = nullptr;
-    if (!tl_state) MLCC_CUDA(cudaMallocHost(&tl_state, 2 * sizeof(DevState)));
-    DevState *h_state = tl_state;
+    Event ev0, ev1, ev_poll[2];
+    MLCC_CUDA(ev0.create());
+    MLCC_CUDA(ev1.create());
+    MLCC_CUDA(ev_poll[0].create(cudaEventDisableTiming));
+    MLCC_CUDA(ev_poll[1].create(cudaEventDisableTiming));
+    // pinned, two snapshots of the device state, kept per host thread (PinnedBlock)
+    static thread_local PinnedBlock tl_state;
+    MLCC_CUDA(tl_state.reserve(2 * sizeof(DevState)));
+    DevState *h_state = static_cast<DevState *>(tl_state.p);
     h_state[0].done = h_state[1].done = 0;
 
     MLCC_CUDA(cudaEventRecord(ev0, stream));
@@ -1348,11 +1356,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
         MLCC_CUDA(ws.alloc(&p.ssum, (size_t)max_slots * n_r * 8));
         MLCC_CUDA(ws.alloc(&p.outside, (size_t)max_slots * n_r));
         const int frc = fmm_build(p.stars, masses, (int)N, opt.fmm_order, opt.fmm_stars_per_node, ws, &p.fmm, stream);
-        if (frc != MLCC_OK) {
-            cudaEventDestroy(ev0); cudaEventDestroy(ev1);
-            cudaEventDestroy(ev_poll[0]); cudaEventDestroy(ev_poll[1]);
-            return frc;
-        }
+        if (frc != MLCC_OK) return frc;
         launches += 9;
     }
     const int grid_seed = sms * 4;
@@ -1368,9 +1372,9 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     bool finished = false;
     int rc = MLCC_OK;
     // progressive copy of finished rows to the host (see the comment above the function)
-    cudaStream_t copy_stream = nullptr;
+    OwnedStream copy_stream;
     std::vector<long long> c_lo(n_sub, 0), c_hi(n_sub, -1);   // rows of sub-chain c already handed to the copy stream
-    if (h_roots) MLCC_CUDA(cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking));
+    if (h_roots) MLCC_CUDA(copy_stream.create());
     auto copy_rows = [&](long long a, long long b) {
         if (a > b) return;
         const size_t off = (size_t)a * n_r * 2, bytes = (size_t)(b - a + 1) * n_r * 2 * sizeof(double);
@@ -1415,9 +1419,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
         for (const void *f : fns) cudaFuncGetAttributes(&fa, f);
         cudaGetLastError();
         cudaGraph_t graph = nullptr;
-        const char *no_graph = getenv("MLCC_NO_GRAPH");   // diagnosis: plain launches
-        if (!(no_graph && no_graph[0] == '1') &&
-            cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+        if (cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
             enqueue_chunk();
             if (cudaStreamEndCapture(stream, &graph) == cudaSuccess && graph) {
                 if (cudaGraphInstantiate(&chunk_exec, graph, 0) != cudaSuccess) chunk_exec = nullptr;
@@ -1454,16 +1456,13 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
         if (es != cudaSuccess) rc = cuda_fail(es, "critical-curve kernels", __FILE__, __LINE__);
         else fin = h_state[0];
     }
-    if (copy_stream) {
+    if (copy_stream.s) {
         if (rc == MLCC_OK && fin.done) copy_finished((long long)max_steps + 1);   // whatever is left
         cudaError_t es = cudaStreamSynchronize(copy_stream);
-        cudaStreamDestroy(copy_stream);
         if (rc == MLCC_OK && es != cudaSuccess) rc = cuda_fail(es, "device -> host copy of the rows", __FILE__, __LINE__);
     }
     float ms = 0.f;
     if (rc == MLCC_OK) cudaEventElapsedTime(&ms, ev0, ev1);
-    cudaEventDestroy(ev0); cudaEventDestroy(ev1);
-    cudaEventDestroy(ev_poll[0]); cudaEventDestroy(ev_poll[1]);
     if (rc != MLCC_OK) return rc;
     if (!fin.done) {
         set_last_error("internal: state machine did not finish");

@@ -67,64 +67,10 @@ int match_root_sets_impl(const double *, const double *, int64_t, int64_t, doubl
 int vieta_residuals_impl(const double *, const double *, int64_t, double, double, const double *, int64_t, int64_t,
                          int64_t, double *, double *, cudaStream_t);
 
+int detj_residuals_impl(const double *, const double *, int64_t, double, double, const double *, int64_t, int64_t,
+                        int64_t, int64_t, double *, double *, double *, cudaStream_t);
+
 namespace {
-
-// FP64 FMA peak probe: 8 independent chains per thread of x = fma(x, y, x) with per-thread register
-// operands (two distinct register pairs: the form that issues at the full rate; measured 63.7 of 64
-// lanes/clk/SM, whereas constant-bank operands reach 58.7 and three distinct register pairs 42.5).
-__global__ void __launch_bounds__(256) k_dfma_peak(double *sink, int iters, double a)
-{
-    const double t = threadIdx.x * 1e-12;
-    double x0 = t, x1 = t + 1, x2 = t + 2, x3 = t + 3, x4 = t + 4, x5 = t + 5, x6 = t + 6, x7 = t + 7;
-    double y0 = a + t, y1 = a + 2 * t, y2 = a + 3 * t, y3 = a + 4 * t, y4 = a + 5 * t, y5 = a + 6 * t,
-           y6 = a + 7 * t, y7 = a + 8 * t;
-    for (int i = 0; i < iters; ++i) {
-#pragma unroll
-        for (int u = 0; u < 8; ++u) {
-            x0 = fma(x0, y0, x0); x1 = fma(x1, y1, x1); x2 = fma(x2, y2, x2); x3 = fma(x3, y3, x3);
-            x4 = fma(x4, y4, x4); x5 = fma(x5, y5, x5); x6 = fma(x6, y6, x6); x7 = fma(x7, y7, x7);
-        }
-    }
-    const double s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
-    if (s == 1.2345e-300) sink[0] = s;  // never true; keeps the chains alive
-}
-
-// Issue-model probes (mlcc_fp64_issue_probe): the same loop shape as k_dfma_peak with other operand forms.
-// FORM 1: DFMA with three distinct register sources.  FORM 2: DADD with two distinct sources.
-// FORM 3: the peak form interleaved 1:1 with packed FP32 FMAs (fma.rn.f32x2, three 64-bit sources): shows
-// that the FP32 instructions draw on the same register-operand bandwidth as the FP64 ones.
-template <int FORM>
-__global__ void __launch_bounds__(256) k_issue_probe(double *sink, int iters, double a)
-{
-    const double t = threadIdx.x * 1e-12;
-    double x[8], y[8], z[8];
-    unsigned long long f[8], gq[8], hq[8];
-#pragma unroll
-    for (int u = 0; u < 8; ++u) {
-        x[u] = t + u; y[u] = a + (u + 1) * t; z[u] = a * 0.5 + (u + 2) * t;
-        f[u] = (unsigned long long)__double_as_longlong(1.0 + u + t);
-        gq[u] = (unsigned long long)__double_as_longlong(0.5 + t);
-        hq[u] = (unsigned long long)__double_as_longlong(0.25 + u * t);
-    }
-    for (int i = 0; i < iters; ++i) {
-#pragma unroll
-        for (int r = 0; r < 8; ++r) {
-#pragma unroll
-            for (int u = 0; u < 8; ++u) {
-                if (FORM == 1) x[u] = fma(x[u], y[u], z[u]);
-                else if (FORM == 2) x[u] = x[u] + y[u];
-                else {
-                    x[u] = fma(x[u], y[u], x[u]);
-                    asm volatile("fma.rn.ftz.f32x2 %0, %0, %1, %2;" : "+l"(f[u]) : "l"(gq[u]), "l"(hq[u]));
-                }
-            }
-        }
-    }
-    double s = 0.0;
-#pragma unroll
-    for (int u = 0; u < 8; ++u) s += x[u] + __longlong_as_double((long long)f[u]);
-    if (s == 1.2345e-300) sink[0] = s;  // never true; keeps the chains alive
-}
 
 bool host_is_pinned(const void *p)
 {
@@ -331,6 +277,16 @@ int mlcc_vieta_residuals(const double *star_xy, const double *masses, int64_t N,
                                 out_e1, out_e2, static_cast<cudaStream_t>(stream));
 }
 
+int mlcc_detj_residuals(const double *star_xy, const double *masses, int64_t N, double kappa_s, double gamma,
+                        const double *points, int64_t num_phi, int64_t n, int64_t phi_index_offset,
+                        int64_t phi_index_total, double *out_residuals, double *out_row_newton, double *out_row_detj,
+                        void *stream)
+{
+    return detj_residuals_impl(star_xy, masses, N, kappa_s, gamma, points, num_phi, n, phi_index_offset,
+                               phi_index_total, out_residuals, out_row_newton, out_row_detj,
+                               static_cast<cudaStream_t>(stream));
+}
+
 int mlcc_star_sums(const double *star_xy, const double *masses, int64_t N, const double *points, int64_t P,
                    int mode, int fmm_order, int fmm_stars_per_node, double *out_sums, void *stream)
 {
@@ -418,59 +374,5 @@ int mlcc_caustics_host(const double *star_xy, const double *masses, int64_t N, d
     return MLCC_OK;
 }
 
-static int fp64_probe(int form, double ms_target, double *out_tflops, void *stream_);
-
-int mlcc_fp64_peak(double ms_target, double *out_tflops, void *stream_)
-{
-    return fp64_probe(0, ms_target, out_tflops, stream_);
-}
-
-int mlcc_fp64_issue_probe(int form, double ms_target, double *out_rate, void *stream_)
-{
-    if (form < 0 || form > 3) return invalid("form must be 0..3");
-    return fp64_probe(form, ms_target, out_rate, stream_);
-}
-
 }  // extern "C"
 
-static int fp64_probe(int form, double ms_target, double *out_tflops, void *stream_)
-{
-    if (!out_tflops) return invalid("null pointer");
-    if (!(ms_target > 0.0) || ms_target > 10000.0) return invalid("ms_target out of range");
-    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
-    const int sms = device_sm_count();
-    const int grid = sms * 4, block = 256;
-    Workspace ws(stream);
-    double *sink = nullptr;
-    MLCC_CUDA(ws.alloc(&sink, 1));
-    cudaEvent_t e0, e1;
-    MLCC_CUDA(cudaEventCreate(&e0));
-    MLCC_CUDA(cudaEventCreate(&e1));
-    int iters = 2000;
-    double best = 0.0;
-    for (int rep = 0; rep < 6; ++rep) {
-        cudaEventRecord(e0, stream);
-        if (form == 0) k_dfma_peak<<<grid, block, 0, stream>>>(sink, iters, -1e-7);
-        else if (form == 1) k_issue_probe<1><<<grid, block, 0, stream>>>(sink, iters, -1e-7);
-        else if (form == 2) k_issue_probe<2><<<grid, block, 0, stream>>>(sink, iters, -1e-7);
-        else k_issue_probe<3><<<grid, block, 0, stream>>>(sink, iters, -1e-7);
-        cudaEventRecord(e1, stream);
-        cudaError_t es = cudaEventSynchronize(e1);
-        if (es != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); return cuda_fail(es, "peak probe", __FILE__, __LINE__); }
-        float ms = 0.f;
-        cudaEventElapsedTime(&ms, e0, e1);
-        const double flop = 2.0 * 64.0 * (double)iters * (double)grid * (double)block;
-        const double tf = flop / ((double)ms * 1e-3) / 1e12;
-        if (rep >= 2 && tf > best) best = tf;
-        if (rep == 0 && ms > 0.f) {   // resize the loop to the requested duration
-            double scale = ms_target / (double)ms;
-            if (scale > 1000.0) scale = 1000.0;
-            if (scale < 0.01) scale = 0.01;
-            iters = (int)fmax(100.0, (double)iters * scale);
-        }
-    }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    *out_tflops = best;
-    return MLCC_OK;
-}

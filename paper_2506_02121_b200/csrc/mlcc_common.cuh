@@ -27,15 +27,21 @@ inline int invalid(const char *msg)
 
 // The stream-ordered allocator gives freed memory back to the driver at every synchronisation unless told
 // otherwise, and every call here would then pay for fresh device allocations (hundreds of ms for the GB-sized
-// scratch of the matcher): raise the device pool's release threshold once per device.
+// scratch of the matcher): the first library call on a device raises the release threshold of that device's
+// DEFAULT memory pool to "keep everything".  This is a process-wide setting of the CUDA runtime: other users of
+// cudaMallocAsync on the same device (PyTorch's default caching allocator is not one) keep their freed blocks
+// cached too until cudaMemPoolTrimTo is called.  Documented in include/mlcc.h.
 void keep_pool_memory();
 
 // Stream-ordered workspace that frees itself (cudaFreeAsync) when it goes out of scope.
 struct Workspace {
+    static constexpr int CAP = 64;
     cudaStream_t stream;
-    void *ptrs[48];
+    void *ptrs[CAP];
     int n = 0;
     explicit Workspace(cudaStream_t s) : stream(s) { keep_pool_memory(); }
+    Workspace(const Workspace &) = delete;
+    Workspace &operator=(const Workspace &) = delete;
     ~Workspace()
     {
         for (int i = n - 1; i >= 0; --i) cudaFreeAsync(ptrs[i], stream);
@@ -43,12 +49,53 @@ struct Workspace {
     template <typename T>
     cudaError_t alloc(T **out, size_t count)
     {
+        *out = nullptr;
+        if (n >= CAP) return cudaErrorMemoryAllocation;   // never hand out a block that would not be freed
         void *p = nullptr;
         cudaError_t e = cudaMallocAsync(&p, count * sizeof(T) > 0 ? count * sizeof(T) : 16, stream);
         if (e != cudaSuccess) return e;
-        if (n < 48) ptrs[n++] = p;
+        ptrs[n++] = p;
         *out = static_cast<T *>(p);
         return cudaSuccess;
+    }
+};
+
+// Small owners, so that every early return releases what the call created.
+struct Event {
+    cudaEvent_t e = nullptr;
+    Event() = default;
+    Event(const Event &) = delete;
+    Event &operator=(const Event &) = delete;
+    ~Event() { if (e) cudaEventDestroy(e); }
+    cudaError_t create(unsigned flags = cudaEventDefault) { return cudaEventCreateWithFlags(&e, flags); }
+    operator cudaEvent_t() const { return e; }
+};
+struct OwnedStream {
+    cudaStream_t s = nullptr;
+    OwnedStream() = default;
+    OwnedStream(const OwnedStream &) = delete;
+    OwnedStream &operator=(const OwnedStream &) = delete;
+    ~OwnedStream() { if (s) { cudaStreamSynchronize(s); cudaStreamDestroy(s); } }
+    cudaError_t create() { return cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking); }
+    operator cudaStream_t() const { return s; }
+};
+// Pinned host block kept per host thread (cudaMallocHost / cudaFreeHost per call cost 80-120 ms every few calls
+// on the bench box); freed when the thread ends (at process exit the runtime may already be gone: the error of
+// that late cudaFreeHost is ignored).
+struct PinnedBlock {
+    void *p = nullptr;
+    size_t bytes = 0;
+    PinnedBlock() = default;
+    PinnedBlock(const PinnedBlock &) = delete;
+    PinnedBlock &operator=(const PinnedBlock &) = delete;
+    ~PinnedBlock() { if (p) { cudaFreeHost(p); cudaGetLastError(); } }
+    cudaError_t reserve(size_t n)
+    {
+        if (n <= bytes) return cudaSuccess;
+        if (p) { cudaFreeHost(p); p = nullptr; bytes = 0; }
+        cudaError_t e = cudaMallocHost(&p, n);
+        if (e == cudaSuccess) bytes = n;
+        return e;
     }
 };
 

@@ -136,10 +136,32 @@ def vieta_all_rows(roots, xy, m, kappa_s, gamma, num_phi):
     return float(e1.max()), float(e2.max())
 
 
-@pytest.mark.parametrize("name,sample_rows", [("cfg3", [0, 1, 1250, 2499, 2500, 4999]),
-                                              ("cfg4", [0, 4999, 9999]),
-                                              ("cfg5", [1000])])
-def test_full_size_sampled_rows_and_invariants(api, orc, name, sample_rows):
+def certify_every_row(api, xy_d, m_d, cfg, roots, phi_off=0, phi_total=0):
+    """mlcc_detj_residuals on EVERY row (BASELINE.json north_star: "|det J| <= 1e-10 at every root", with the scale-aware
+    bound of SURVEY.md 0.2): max_k |1/mu_k| / bound_k <= 1 and max_k |F|/|F'| far inside the parity tolerance, so a
+    root that stopped 1e-9 from its place cannot pass (Vieta's sums would not see it)."""
+    rn, rd, _ = api.detj_residuals(xy_d, m_d, cfg.kappa_s, cfg.gamma, roots, phi_off, phi_total)
+    assert float(rd.max()) <= 1.0, (int(rd.argmax()), float(rd.max()))
+    assert float(rn.max()) < 1e-11, (int(rn.argmax()), float(rn.max()))
+    return rn, rd
+
+
+def rows_beside_the_centres(api, cfg, which, halfwidth=2):
+    """Rows centre-halfwidth .. centre+halfwidth of the listed sub-chains of the library's default plan: the rows whose
+    predictor stencil is shortened (the first continued rows of a chain)."""
+    first, centre, end = api.plan_subchains(cfg.N, cfg.num_phi, 0)
+    out = []
+    for c in which:
+        c = c % len(centre)
+        out.append([int(r) for r in range(int(centre[c]) - halfwidth, int(centre[c]) + halfwidth + 1)
+                    if first[c] <= r < end[c]])
+    return out, len(centre)
+
+
+@pytest.mark.parametrize("name,sample_rows,centres,halfwidth", [("cfg3", [0, 1, 1250, 2499, 2500, 4999], [0, 17], 2),
+                                                                 ("cfg4", [0, 4999, 9999], [0, 5], 2),
+                                                                 ("cfg5", [], [1], 1)])
+def test_full_size_sampled_rows_and_invariants(api, orc, name, sample_rows, centres, halfwidth):
     cfg = CONFIGS[name]
     xy, m, R = field(orc, cfg)
     roots, iters, unconv, stats = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, cfg.num_phi,
@@ -147,9 +169,10 @@ def test_full_size_sampled_rows_and_invariants(api, orc, name, sample_rows):
     torch.cuda.synchronize()
     assert int(unconv.sum()) == 0 and stats.degenerate_roots == 0
     assert int(iters.min()) >= 1
-    # properties that hold at any size, every row: Vieta sums (complete, no duplicated root)
+    # properties that hold at any size, every row: Vieta sums (complete, no duplicated root), det J and Newton residual
     e1, e2 = vieta_all_rows(roots, xy, m, cfg.kappa_s, cfg.gamma, cfg.num_phi)
     assert e1 < 1e-12 and e2 < 1e-12, (e1, e2)
+    certify_every_row(api, dev(xy), dev(m), cfg, roots)
     # sampled rows against the oracle (each row cold-started by the oracle on its own)
     for j in sample_rows:
         ref, _, un = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, cfg.num_phi, [j], cfg.tol, cfg.max_iter)
@@ -160,11 +183,80 @@ def test_full_size_sampled_rows_and_invariants(api, orc, name, sample_rows):
         w_gpu = api.caustics(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, roots[j:j + 1].contiguous()).cpu().numpy()
         w_ref = orc.caustics(xy, m, cfg.kappa_s, cfg.gamma, ref)
         assert_caustics_match(g[0], w_gpu[0], ref[0], w_ref[0])
-    # certificates on more rows than the oracle can solve: long-double residuals, det J, distinctness
+    # the rows beside sub-chain centres (cold row, then the rows seeded with a shortened predictor stencil): the oracle
+    # cold-starts the first of them and continues through the rest
+    groups, n_sub = rows_beside_the_centres(api, cfg, centres, halfwidth)
+    assert n_sub == stats.subchains
+    oracle_row = {}
+    for rows in groups:
+        ref, _, un = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, cfg.num_phi, rows, cfg.tol, cfg.max_iter)
+        assert un.sum() == 0
+        g = roots[rows[0]:rows[-1] + 1].cpu().numpy()
+        assert_rows_match(orc, g, ref)
+        oracle_row[rows[0]] = ref[0]
+    # certificates on more rows than the oracle can solve: long-double residuals, det J, distinctness; and the kernel's
+    # worst long-double residual of a row is held to twice that of the oracle's own fp64 solve of the same row
     rng = np.random.default_rng(1)
-    for j in rng.choice(cfg.num_phi, size=4, replace=False):
-        check_row_invariants(orc, xy, m, cfg.kappa_s, cfg.gamma, int(j), cfg.num_phi,
-                             cplx(roots[int(j)].cpu().numpy()))
+    extra = [groups[0][0]] if groups else []
+    for j in list(rng.choice(cfg.num_phi, size=4, replace=False)) + extra:
+        res = check_row_invariants(orc, xy, m, cfg.kappa_s, cfg.gamma, int(j), cfg.num_phi,
+                                   cplx(roots[int(j)].cpu().numpy()))
+        if int(j) in extra:
+            worst_gpu = res["newton"].max()
+            res_o = orc.residuals(xy, m, cfg.kappa_s, cfg.gamma, int(j), cfg.num_phi, oracle_row[int(j)])   # the oracle's fp64 solve
+            assert worst_gpu <= 2 * res_o["newton"].max() + 1e-13, (worst_gpu, res_o["newton"].max())
+
+
+@pytest.mark.parametrize("name,rows", [("cfg1", [0, 499, 500]), ("cfg2", [0, 7, 2000]), ("cfg3", [1250]), ("cfg4", [0])])
+def test_detj_residuals_against_oracle(api, orc, name, rows):
+    """mlcc_detj_residuals element by element against the oracle's long-double F, F', 1/mu, |F|/|F'| (orc_residuals_ld):
+    at converged roots (where F is a rounding-level residue of terms of size sum |m/(z-z_i)^2|) and at displaced
+    points (where F is O(1) and the comparison is relative)."""
+    cfg = CONFIGS[name]
+    xy, m, R = field(orc, cfg)
+    zs = xy[:, 0] + 1j * xy[:, 1]
+    ref, _, un = orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, cfg.num_phi, rows[:1], cfg.tol, cfg.max_iter)
+    assert un.sum() == 0
+    rng = np.random.default_rng(5)
+    n = min(2 * cfg.N, 4000)                                          # (n is free: a part of the row is enough at N = 10^4)
+    pts = np.empty((len(rows), n, 2))
+    pts[0] = ref[0][-n:]                                              # converged roots (phase of rows[0])
+    for q in range(1, len(rows)):                                     # displaced points, other phases
+        pts[q] = ref[0][-n:] + rng.normal(scale=0.05, size=(n, 2))
+    xy_d, m_d = dev(xy), dev(m)
+    for q, j in enumerate(rows):
+        rn, rd, res = api.detj_residuals(xy_d, m_d, cfg.kappa_s, cfg.gamma, dev(pts[q:q + 1]), j, cfg.num_phi,
+                                         want_points=True)
+        res = res.cpu().numpy()[0]
+        o = orc.residuals(xy, m, cfg.kappa_s, cfg.gamma, j, cfg.num_phi, pts[q])
+        z = pts[q, :, 0] + 1j * pts[q, :, 1]
+        d = np.abs(z[:, None] - zs[None, :])
+        t2 = (m[None, :] / d ** 2).sum(axis=1) + abs(cfg.gamma) + (1 - cfg.kappa_s)      # size of the terms of F
+        t3 = 2 * (m[None, :] / d ** 3).sum(axis=1)                                         # ... of F'
+        F, Fp = res[:, 0] + 1j * res[:, 1], res[:, 2] + 1j * res[:, 3]
+        assert (np.abs(F - o["F"]) <= 1e-12 * t2).all()
+        assert (np.abs(Fp - o["Fp"]) <= 1e-12 * t3).all()
+        assert (np.abs(res[:, 4] - o["inv_mu"]) <= 1e-12 * t2 ** 2).all()
+        assert (np.abs(res[:, 5] - o["newton"]) <= 1e-12 * t2 / np.abs(o["Fp"]) + 1e-12 * o["newton"] * t3 / np.abs(o["Fp"])).all()
+        # the row outputs are the maxima of the point outputs
+        bound = 1e-10 + 4 * (1 - cfg.kappa_s) * np.abs(Fp) * 2.0 ** -52 * (1 + np.abs(z))
+        assert float(rn[0]) == res[:, 5].max()
+        assert abs(float(rd[0]) - (np.abs(res[:, 4]) / bound).max()) <= 1e-12 * float(rd[0])
+        if q == 0:
+            assert float(rd[0]) <= 1.0 and float(rn[0]) < 1e-11       # the oracle's own converged row is certified
+        else:
+            assert float(rd[0]) > 1.0                                 # displaced points are not
+    # several rows in one call = the rows one by one; a wrong phase offset is seen; a point on a star gives +inf
+    rn_all, rd_all, _ = api.detj_residuals(xy_d, m_d, cfg.kappa_s, cfg.gamma, dev(np.repeat(pts[:1], 3, axis=0)), rows[0],
+                                           cfg.num_phi)
+    # det J = 0 on the critical curve whatever phi is: only the Newton residual of F sees the phase (rows[0]+1, +2)
+    assert float(rd_all.max()) <= 1.0 and float(rn_all[0]) < 1e-11 and float(rn_all[1]) > 1e-7 and float(rn_all[2]) > float(rn_all[1])
+    bad = pts[:1].copy()
+    bad[0, 3] = xy[0]
+    rn_b, rd_b, _ = api.detj_residuals(xy_d, m_d, cfg.kappa_s, cfg.gamma, dev(bad), rows[0], cfg.num_phi)
+    assert np.isinf(float(rn_b[0])) or np.isinf(float(rd_b[0]))
+    empty = api.detj_residuals(xy_d, m_d, cfg.kappa_s, cfg.gamma, torch.empty((0, n, 2), dtype=torch.float64, device="cuda"))
+    assert empty[0].shape == (0,)
 
 
 @pytest.mark.parametrize("name,num_phi", [("cfg1", 1000), ("cfg2", 777), ("cfg3", 64)])
@@ -224,8 +316,9 @@ def test_bench_configuration_full_size_cfg4(api, orc):
         assert_rows_match(orc, g, ref)
         w_ref = orc.caustics(oxy, om, cfg.kappa_s, cfg.gamma, ref)
         assert_caustics_match(g[0], caus[j].cpu().numpy(), ref[0], w_ref[0])
-    g1, g2 = api.vieta_residuals(xy_o, m_o, cfg.kappa_s, cfg.gamma, roots)       # the library's own certificate
+    g1, g2 = api.vieta_residuals(xy_o, m_o, cfg.kappa_s, cfg.gamma, roots)       # the library's own certificates
     assert float(g1.max()) < 1e-12 and float(g2.max()) < 1e-12
+    certify_every_row(api, xy_o, m_o, cfg, roots)
     again, caus2, _, _, _ = api.curves_and_caustics(xy_o, m_o, cfg.kappa_s, cfg.gamma, cfg.num_phi, cfg.tol,
                                                     cfg.max_iter, want_diagnostics=False)
     err, bij = api.match_root_sets(again, roots, 1e-10)
@@ -830,6 +923,28 @@ def test_trust_predictor_starts_rows_with_newton_steps(api, orc, name, num_phi):
     assert torch.equal(a, b) and sa.root_pairs == sb.root_pairs
     with pytest.raises(api.MlccError):
         api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, 8, opt=api.options(trust_predictor=2))
+
+
+@pytest.mark.parametrize("tol,skip", [(1e-6, 0.0), (1e-6, 1e-9), (1e-12, 1e-13)])
+def test_trust_predictor_with_a_skip_threshold_below_tol(api, orc, tol, skip):
+    """The guarded first iteration of a trusted row when skip_aberth_sum_below < tol (library default 1e-8 against
+    tol = 1e-6, or an explicit threshold below tol): rejected Newton steps between the two thresholds must stay in the
+    list -- k_apply's two passes use one predicate (step_kind) -- so no root is left at its predictor seed: every row
+    complete (Vieta), every root certified by its Newton residual, none unconverged, sets equal to the oracle's."""
+    cfg = CONFIGS["cfg2"]
+    xy, m, R = field(orc, cfg)
+    num_phi = 1200
+    got, it, un, st = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, num_phi, tol, cfg.max_iter,
+                                             opt=api.options(trust_predictor=1, skip_aberth_sum_below=skip))
+    assert int(un.sum()) == 0 and st.unconverged_rows == 0 and st.degenerate_roots == 0
+    ref, _, uno = orc.critical_curves(xy, m, cfg.kappa_s, cfg.gamma, num_phi, tol, cfg.max_iter)
+    assert uno.sum() == 0
+    # a step below tol = 1e-6 was still APPLIED: the error left is of second order in it
+    assert_rows_match(orc, got.cpu().numpy(), ref, tol=1e-10 if tol < 1e-9 else 1e-9)
+    e1, e2 = vieta_all_rows(got, xy, m, cfg.kappa_s, cfg.gamma, num_phi)
+    assert e1 < 1e-9 and e2 < 1e-9, (e1, e2)
+    rn, rd, _ = api.detj_residuals(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, got)
+    assert float(rn.max()) < (1e-11 if tol < 1e-9 else 1e-9), float(rn.max())
 
 
 def test_crossing_map_full_size_cfg4_sampled_pixels(api, orc):
