@@ -67,6 +67,15 @@ enum { MLCC_MASS_EQUAL = 0, MLCC_MASS_POWER_LAW = 1, MLCC_MASS_BROKEN_POWER_LAW 
  *         tolerance.  The Aberth sum over the other roots stays direct in both modes.             */
 enum { MLCC_STAR_SUMS_DIRECT = 0, MLCC_STAR_SUMS_FMM = 1 };
 
+/* Kernel regimes of the solver (mlcc_options.regime; how much of the GPU one phase fills).
+ * TILED: every iteration of all rows in flight is a few launches over a persistent grid that tiles roots and
+ *        sources through shared memory (any N; the path for N >~ 10^3).
+ * CHAIN: one CTA owns a sub-chain and runs all its rows and iterations out of shared memory, one launch per call
+ *        (fields of up to about 1200 stars; direct star sums, disc fields, FP64 Aberth sum, no trust_predictor).
+ * AUTO:  CHAIN where it applies and n_r <= 2400, else TILED.  The root sets are the same within the parity
+ *        tolerance; the bits differ (other summation order).                                              */
+enum { MLCC_REGIME_AUTO = 0, MLCC_REGIME_TILED = 1, MLCC_REGIME_CHAIN = 2 };
+
 /* Options of mlcc_critical_curves_ex.  Zero-initialise, or call mlcc_options_default(). */
 typedef struct mlcc_options {
     int32_t struct_size;      /* = sizeof(mlcc_options)                                             */
@@ -85,9 +94,11 @@ typedef struct mlcc_options {
                                    (Eq. 17).  A multiplies F in the denominator of the
                                    update, so it steers the convergence rate only: the fixed point
                                    F = 0 and the freeze test do not depend on it (R19).
-                                   0 or 32 = double-single FP32 (z = hi + lo, differences exact to
-                                   ~2^-23 |z_k - z_r|); 64 = FP64 differences with the 20-bit
-                                   reciprocal seed.  Star sums (F, F') are FP64 in both.            */
+                                   0 or 64 = FP64 differences with the 20-bit reciprocal seed (the
+                                   default: every pair of the iteration is FP64 arithmetic);
+                                   32 = double-single FP32 (z = hi + lo, differences exact to
+                                   ~2^-23 |z_k - z_r|, packed f32x2 instructions; tiled regime only;
+                                   about 7 % faster at N = 10^4).  Star sums (F, F') are FP64 in both. */
     int32_t star_sum_mode;    /* MLCC_STAR_SUMS_DIRECT (default) or MLCC_STAR_SUMS_FMM               */
     int32_t fmm_order;        /* Taylor order of the node series (1..63); 0 = 31                     */
     int32_t fmm_stars_per_node; /* mean stars per grid node (the grid has ~N / this many nodes);
@@ -109,7 +120,7 @@ typedef struct mlcc_options {
        Eq. B2; the caller adds its gamma_shift to gamma.  NULL / 0 = the infinite sheet of a disc. */
     const double *sheet_poly; /* HOST pointer, [sheet_poly_n]; the last coefficient must be non-zero  */
     int32_t sheet_poly_n;     /* d + 1, at most 512; 0 = none                                        */
-    int32_t reserved2_;       /* 0                                                                   */
+    int32_t regime;           /* MLCC_REGIME_AUTO (default), _TILED or _CHAIN: see the enum above                    */
     double seed_radius;       /* the d - 1 extra cold seeds are spread evenly on the circle of this
                                  radius about the origin; must be > 0 when d >= 2 and
                                  init_roots is NULL                                                   */
@@ -129,8 +140,9 @@ typedef struct mlcc_stats {
     int64_t star_pairs;        /* (root, star) pair evaluations  = root_iterations * N                  */
     int64_t root_pairs;        /* (root, root) pair evaluations: (2N - 1) per root-iteration that had the
                                   Aberth sum (see mlcc_options.skip_aberth_sum_below)                    */
-    int64_t kernel_launches;   /* kernels launched by the call                                          */
-    int32_t total_iterations;  /* Aberth iterations summed over steps (one step = all chains advance 1 row) */
+    int64_t kernel_launches;   /* kernels launched by the call (chain regime: 2)                        */
+    int32_t total_iterations;  /* Aberth iterations summed over steps (one step = all chains advance 1 row);
+                                  chain regime: those of the sub-chain that ran the most (the critical path)  */
     int32_t steps;             /* steps taken (cold step included)                                      */
     int32_t subchains;         /* sub-chains used                                                       */
     int32_t predictor_order;   /* predictor order used                                                  */
@@ -138,6 +150,8 @@ typedef struct mlcc_stats {
     int32_t degenerate_roots;  /* NaN/Inf steps seen                                                    */
     float   solve_ms;          /* device time of the call's kernels, CUDA events on `stream`            */
     int32_t aberth_sum_precision; /* 32 or 64: the Aberth-sum arithmetic used                           */
+    int32_t regime;            /* MLCC_REGIME_TILED or MLCC_REGIME_CHAIN: the regime used               */
+    int32_t reserved_;
 } mlcc_stats;
 
 int         mlcc_version(void);                 /* major*10000 + minor*100 + patch                       */

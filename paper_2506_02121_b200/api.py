@@ -23,6 +23,7 @@ MLCC_ERR_NOT_CONVERGED = 4
 MLCC_ERR_DEGENERATE = 5
 MLCC_STAR_SUMS_DIRECT = 0
 MLCC_STAR_SUMS_FMM = 1
+MLCC_REGIME_AUTO, MLCC_REGIME_TILED, MLCC_REGIME_CHAIN = 0, 1, 2
 
 
 class MlccError(RuntimeError):
@@ -38,7 +39,7 @@ class mlcc_options(C.Structure):
                 ("min_lanes_per_root", C.c_int32), ("aberth_sum_precision", C.c_int32),
                 ("star_sum_mode", C.c_int32), ("fmm_order", C.c_int32),
                 ("fmm_stars_per_node", C.c_int32), ("trust_predictor", C.c_int32),
-                ("sheet_poly", C.c_void_p), ("sheet_poly_n", C.c_int32), ("reserved2_", C.c_int32),
+                ("sheet_poly", C.c_void_p), ("sheet_poly_n", C.c_int32), ("regime", C.c_int32),
                 ("seed_radius", C.c_double), ("skip_aberth_sum_below", C.c_double)]
 
 
@@ -47,7 +48,8 @@ class mlcc_stats(C.Structure):
                 ("kernel_launches", C.c_int64), ("total_iterations", C.c_int32), ("steps", C.c_int32),
                 ("subchains", C.c_int32), ("predictor_order", C.c_int32),
                 ("unconverged_rows", C.c_int32), ("degenerate_roots", C.c_int32),
-                ("solve_ms", C.c_float), ("aberth_sum_precision", C.c_int32)]
+                ("solve_ms", C.c_float), ("aberth_sum_precision", C.c_int32), ("regime", C.c_int32),
+                ("reserved_", C.c_int32)]
 
 
 @dataclass
@@ -65,6 +67,7 @@ class Stats:
     solve_ms: float
     status: int = 0
     aberth_sum_precision: int = 0
+    regime: int = 0
 
 
 _lib = None
@@ -151,7 +154,7 @@ def last_error() -> str:
 def options(num_subchains=0, predictor_order=-1, max_iter_cold=0, phi_index_offset=0,
             phi_index_total=0, min_lanes_per_root=0, aberth_sum_precision=0, star_sum_mode=0, fmm_order=0,
             fmm_stars_per_node=0, sheet_poly=None, seed_radius=0.0, skip_aberth_sum_below=0.0,
-            trust_predictor=0) -> mlcc_options:
+            trust_predictor=0, regime=0) -> mlcc_options:
     o = mlcc_options()
     lib().mlcc_options_default(C.byref(o))
     o.num_subchains = num_subchains
@@ -166,6 +169,7 @@ def options(num_subchains=0, predictor_order=-1, max_iter_cold=0, phi_index_offs
     o.fmm_stars_per_node = fmm_stars_per_node
     o.skip_aberth_sum_below = skip_aberth_sum_below
     o.trust_predictor = int(trust_predictor)
+    o.regime = int(regime)
     if sheet_poly is not None:
         arr = np.ascontiguousarray(sheet_poly, np.float64)
         o._keep = arr                       # the struct holds a raw host pointer: keep the array alive
@@ -241,7 +245,7 @@ def critical_curves(star_xy, masses, kappa_s, gamma, num_phi, tol=1e-12, max_ite
 def _stats(st: mlcc_stats, rc: int) -> Stats:
     return Stats(st.root_iterations, st.star_pairs, st.root_pairs, st.kernel_launches,
                  st.total_iterations, st.steps, st.subchains, st.predictor_order,
-                 st.unconverged_rows, st.degenerate_roots, st.solve_ms, rc, st.aberth_sum_precision)
+                 st.unconverged_rows, st.degenerate_roots, st.solve_ms, rc, st.aberth_sum_precision, st.regime)
 
 
 def critical_curves_ex(star_xy, masses, kappa_s, gamma, num_phi, tol=1e-12, max_iter=50, opt=None,

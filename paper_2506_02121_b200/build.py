@@ -8,7 +8,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libmlcc.so")
 UNITS = ["api.cu", "aberth.cu", "caustics.cu", "starfield.cu", "match.cu", "fmm.cu", "crossing.cu", "loops.cu",
-         "distance.cu", "probe.cu", "certify.cu"]
+         "distance.cu", "probe.cu", "certify.cu", "chain.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--fmad=true", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

@@ -42,7 +42,26 @@
 #include <vector>
 
 namespace mlcc {
+
+// chain.cu: the small-field regime (one CTA per sub-chain)
+struct ChainRun {
+    unsigned long long root_iterations, root_iterations_noA;
+    int max_iterations, unconverged_rows, degenerate;
+};
+int chain_capacity(int64_t N, int64_t n_r, bool caus);
+int chain_launch(const double *star_xy, const double *masses, int64_t N, int64_t n_r, double gamma, double omk,
+                 double tol, double skip_below, int max_iter, int max_iter_cold, int order, const void *d_rot,
+                 const double *init_roots, double *roots, double *caustics, int *out_iters, int *out_unconverged,
+                 int n_sub, const long long *d_first, const long long *d_centre, const long long *d_end,
+                 void *d_counters, cudaStream_t stream);
+size_t chain_counters_bytes();
+void chain_read_counters(const void *h_counters, ChainRun *out);
+
 namespace {
+
+// Fields of up to this many roots per phase go to the chain regime when they fit it (mlcc_options.regime = AUTO);
+// measured crossover: DESIGN.md "Kernel regimes".
+constexpr int CHAIN_AUTO_MAX_ROOTS = 2400;
 
 constexpr int CTA = 128;          // threads per CTA of the compute kernel
 #ifndef MLCC_ROOTS_PER_THREAD
@@ -61,6 +80,12 @@ constexpr int S_TILE = 256;       // stars per stage; a stage also holds the 2*S
 constexpr int STAGE_BYTES = S_TILE * 16 + S_TILE * 8 + 2 * S_TILE * 16;
 constexpr int BLOCK = 256;        // threads per CTA of the small kernels
 constexpr int MAX_ORDER = 5;      // highest predictor order
+// Library defaults of the predictor order (mlcc_options.predictor_order = -1), by measurement (R18): the
+// higher the order, the more roots are within tol of their seed and freeze in the first iteration (cfg4: 79 % at
+// order 3, 96 % at order 4, 98 % at order 5), but the extrapolation weights (sum |c_q| = 15, 31, 63) also amplify the
+// rounding of the stored rows, which leaves more stragglers iterations behind in the large fields.
+constexpr int DEFAULT_ORDER_TILED = 4;
+constexpr int DEFAULT_ORDER_CHAIN = 5;
 constexpr int MAX_SLOTS = 1024;   // most slots in one step (2 per sub-chain)
 constexpr double TINY = 1e-300;   // added to |d|^2 (FP64 root pairs): makes the self pair finite
 constexpr float TINYF = 1e-30f;   // same for the FP32 root pairs
@@ -105,6 +130,7 @@ struct Params {
     int n_r;                  // 2N
     int N_pad;                // N rounded up to a multiple of S_TILE
     double gamma;
+    double mass0;             // masses[0]: the mass of every star in an equal-mass field (EQM kernels)
     double omk;               // 1 - kappa_s
     double tol2;              // tol^2
     int max_iter;
@@ -143,6 +169,8 @@ struct Params {
                               //   skip threshold last time: they sit at the END of the slot's list
     int *list;                // [2][max_slots][n_r]
     double2 *delta;           // [max_slots][n_r]
+    int2 *chunk_count;        // [max_slots][chunks] survivors (with, without the Aberth sum) of every chunk of a slot's list
+    unsigned *ticket;         // [1] CTAs of the running k_apply_write that are through
     int max_slots;            // slots that can be live at once (2 n_sub)
     int R;                    // roots per thread of the compute kernel in use
     // smooth-sheet polynomial H(u) = sum poly[n] u^n (rectangular field, Appendix B); poly_n = 0: none
@@ -480,7 +508,8 @@ __global__ void __launch_bounds__(BLOCK) k_star_sums_outside(Params p)
 // accumulated.  It takes the unfrozen roots whose last step was below
 // the skip threshold (the tail [n_active - n_small, n_active) of every slot's list, tile set 1); the full kernel
 // takes the others (tile set 0).  DESIGN.md readings R27, R30 (with trust_predictor: whole rows in their first iteration).
-template <int MODE, bool CAUS, bool STARS, bool ROOTS, int R>
+// EQM: every star has the mass p.mass0: the lighter pair body of star_sums.cuh (20 instead of 24 FP64 instructions).
+template <int MODE, bool CAUS, bool STARS, bool ROOTS, int R, bool EQM = false>
 __global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Params p)
 {
     __shared__ Stage s_stage[2];
@@ -597,18 +626,24 @@ __global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Para
                         double sm = 0.0;
                         if (STARS) {
                             sxy = sg.sxy[j];
-                            sm = sg.sm[j];
+                            if (!EQM) sm = sg.sm[j];
                         }
                         if (!ROOTS) {
 #pragma unroll
                             for (int r = 0; r < R; ++r)
-                                if (STARS) pair_star<CAUS, false>(zx[r], zy[r], sxy, sm, acc[r]);
+                                if (STARS) {
+                                    if (EQM) pair_star_eq<CAUS, false>(zx[r], zy[r], sxy, acc[r]);
+                                    else pair_star<CAUS, false>(zx[r], zy[r], sxy, sm, acc[r]);
+                                }
                         } else if (MODE == MODE_F64) {
                             const double2 *rr = reinterpret_cast<const double2 *>(sg.rp);
                             const double2 ra = rr[2 * j], rb = rr[2 * j + 1];
 #pragma unroll
                             for (int r = 0; r < R; ++r) {
-                                if (STARS) pair_star<CAUS>(zx[r], zy[r], sxy, sm, acc[r]);
+                                if (STARS) {
+                                    if (EQM) pair_star_eq<CAUS>(zx[r], zy[r], sxy, acc[r]);
+                                    else pair_star<CAUS>(zx[r], zy[r], sxy, sm, acc[r]);
+                                }
                                 pair_root_f64(zx[r], zy[r], ra, ax[r], ay[r]);
                                 pair_root_f64(zx[r], zy[r], rb, bx[r], by[r]);
                             }
@@ -616,7 +651,10 @@ __global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Para
                             const float4 h = sg.rp[2 * j], l = sg.rp[2 * j + 1];
 #pragma unroll
                             for (int r = 0; r < R; ++r) {
-                                if (STARS) pair_star<CAUS>(zx[r], zy[r], sxy, sm, acc[r]);
+                                if (STARS) {
+                                    if (EQM) pair_star_eq<CAUS>(zx[r], zy[r], sxy, acc[r]);
+                                    else pair_star<CAUS>(zx[r], zy[r], sxy, sm, acc[r]);
+                                }
                                 pair_root2_f32(make_float2(zxh[r], zxh[r]), make_float2(zyh[r], zyh[r]),
                                                make_float2(zxl[r], zxl[r]), make_float2(zyl[r], zyl[r]), h, l,
                                                fx[r], fy[r]);
@@ -639,6 +677,7 @@ __global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Para
                 sax = ax[r] + bx[r];
                 say = ay[r] + by[r];
             }
+            if (STARS && EQM) star_sums_scale<CAUS, ROOTS>(acc[r], p.mass0);
             if (STARS) {
                 // without the Aberth sum the step is the Newton step of F: t = 2 S1 - A is left out as a whole
                 // (2 S1 and A nearly cancel -- two roots per star -- so 2 S1 alone would be the worse stand-in)
@@ -696,11 +735,7 @@ __global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Para
 }
 
 // ------------------------------------------------------------------------------------------------
-// apply kernel: z_k -= Delta_k, freeze converged roots, compact the list of unfrozen roots.
-// One CTA per slot walks the slot's list in chunks and keeps the survivors IN ORDER (block-wide
-// exclusive scan), so the next iteration's tiles -- and with them the summation order of every
-// root -- do not depend on the timing of this launch: two runs give the same bits.
-// grid: max_slots CTAs of APPLY_THREADS threads
+// helpers of the apply kernels (below, after the state machine they end in)
 // ------------------------------------------------------------------------------------------------
 // mlcc_options.trust_predictor (R30): the rows of a step whose seeds come from the predictor at its
 // full order start with every root in the no-Aberth-sum group; k_apply guards that first iteration.
@@ -720,119 +755,8 @@ __device__ __forceinline__ int step_kind(double d2, double tol2, double skip2, b
     return d2 < skip2 ? 2 : 1;
 }
 
-constexpr int APPLY_THREADS = 1024;
-constexpr int APPLY_ITEMS = 4;
-
-template <int MODE>
-__global__ void __launch_bounds__(APPLY_THREADS) k_apply(Params p)
-{
-    __shared__ int s_warp[32];
-    __shared__ int s_total;
-    const DevState st = *p.state;
-    if (st.done) return;
-    const int slot = blockIdx.x;
-    if (slot >= st.n_slots) return;
-    const int n_act = p.n_active[st.cur * MAX_SLOTS + slot];
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int *list = p.list + ((long long)st.cur * p.max_slots + slot) * p.n_r;
-    int *next = p.list + ((long long)(st.cur ^ 1) * p.max_slots + slot) * p.n_r;
-    const double2 *delta = p.delta + (long long)slot * p.n_r;
-    double2 *row = p.roots + p.slot_row[slot] * p.n_r;
-    float4 *slot_src = p.src + (size_t)slot * 2 * p.N_pad;
-    // First iteration of a trusted row: the steps were taken without the Aberth sum, i.e. they are Newton steps from
-    // the predicted seeds.  One below the skip threshold is applied as any confirming step is; a larger one says the
-    // prediction was not that good: it is NOT applied and the root gets a full Aberth iteration from its seed next.
-    const bool guard = st.iter == 0 && trusted_step(p, st.step);
-    // A survivor (|Delta|^2 >= tol^2) is "large" if |Delta|^2 >= skip_below2, else "small": the next list holds
-    // the large ones first, then the small ones, each group in the order of this list.
-    // pass 1: the number of large survivors = where the small ones start
-    int n_large = 0;
-    for (int pos = tid; pos < n_act; pos += APPLY_THREADS) {
-        const double2 d = delta[pos];
-        const double d2 = d.x * d.x + d.y * d.y;
-        if (d2 <= 1.79769313486231570e308 && step_kind(d2, p.tol2, p.skip_below2, guard) == 1) ++n_large;
-    }
-    for (int o = 16; o > 0; o >>= 1) n_large += __shfl_xor_sync(0xffffffffu, n_large, o);
-    if (lane == 0) s_warp[warp] = n_large;
-    __syncthreads();
-    if (tid == 0) {
-        int t = 0;
-        for (int w = 0; w < APPLY_THREADS / 32; ++w) t += s_warp[w];
-        s_total = t;
-    }
-    __syncthreads();
-    n_large = s_total;
-    __syncthreads();
-    // pass 2: apply the steps, write both groups in order (counts packed: large in the low 16 bits, small above)
-    int base_l = 0, base_s = n_large;
-    for (int c0 = 0; c0 < n_act; c0 += APPLY_THREADS * APPLY_ITEMS) {
-        int ks[APPLY_ITEMS];
-        int kind[APPLY_ITEMS];   // 0 frozen, 1 large, 2 small
-        int cnt = 0;
-#pragma unroll
-        for (int i = 0; i < APPLY_ITEMS; ++i) {
-            const int pos = c0 + tid * APPLY_ITEMS + i;
-            kind[i] = 0;
-            ks[i] = 0;
-            if (pos < n_act) {
-                const int k = list[pos];
-                const double2 d = delta[pos];
-                const double d2 = d.x * d.x + d.y * d.y;
-                if (d2 <= 1.79769313486231570e308) {   // finite step
-                    kind[i] = step_kind(d2, p.tol2, p.skip_below2, guard);
-                    if (!(guard && kind[i] == 1)) {     // (a rejected Newton step leaves z where it is)
-                        double2 z = row[k];
-                        z.x -= d.x;
-                        z.y -= d.y;
-                        row[k] = z;
-                        store_src<MODE>(slot_src, k, z);
-                    }
-                } else {                                // NaN / Inf: freeze where it is, report
-                    atomicAdd(&p.state->degenerate, 1);
-                }
-                ks[i] = k;
-                cnt += kind[i] == 1 ? 1 : (kind[i] == 2 ? (1 << 16) : 0);
-            }
-        }
-        int incl = cnt;   // inclusive scan over the warp, then over the warps
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int n = __shfl_up_sync(0xffffffffu, incl, o);
-            if (lane >= o) incl += n;
-        }
-        if (lane == 31) s_warp[warp] = incl;
-        __syncthreads();
-        if (warp == 0) {
-            const int w = s_warp[lane];
-            int wi = w;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int n = __shfl_up_sync(0xffffffffu, wi, o);
-                if (lane >= o) wi += n;
-            }
-            s_warp[lane] = wi - w;
-            if (lane == 31) s_total = wi;
-        }
-        __syncthreads();
-        const int excl = s_warp[warp] + incl - cnt;
-        int off_l = base_l + (excl & 0xffff), off_s = base_s + (excl >> 16);
-#pragma unroll
-        for (int i = 0; i < APPLY_ITEMS; ++i) {
-            if (kind[i] == 1) next[off_l++] = ks[i];
-            else if (kind[i] == 2) next[off_s++] = ks[i];
-        }
-        base_l += s_total & 0xffff;
-        base_s += s_total >> 16;
-        __syncthreads();
-    }
-    if (tid == 0) {
-        p.n_active[(st.cur ^ 1) * MAX_SLOTS + slot] = base_s;
-        p.n_small[(st.cur ^ 1) * MAX_SLOTS + slot] = base_s - n_large;
-    }
-}
-
 // ------------------------------------------------------------------------------------------------
-// state machine (k_init, k_finalize): one CTA of FIN threads, thread s looks after slot s
+// state machine (k_init, finalize_iteration): one CTA of FIN threads, thread s looks after slot s
 // (MAX_SLOTS = FIN), sums and prefix sums over the slots by block-wide scans
 // ------------------------------------------------------------------------------------------------
 constexpr int FIN = MAX_SLOTS;
@@ -916,8 +840,8 @@ __device__ void build_tiles_of(const Params &p, DevState &st, int K, int count, 
 __device__ void build_tiles(const Params &p, DevState &st, long long *s_buf)
 {
     const int s = threadIdx.x;
-    const int n_act = s < st.n_slots ? p.n_active[st.cur * MAX_SLOTS + s] : 0;
-    const int n_sm = s < st.n_slots ? p.n_small[st.cur * MAX_SLOTS + s] : 0;
+    const int n_act = s < st.n_slots ? __ldcg(&p.n_active[st.cur * MAX_SLOTS + s]) : 0;
+    const int n_sm = s < st.n_slots ? __ldcg(&p.n_small[st.cur * MAX_SLOTS + s]) : 0;
     build_tiles_of(p, st, 0, n_act - n_sm, s_buf);
     build_tiles_of(p, st, 1, n_sm, s_buf);
     st.total_active = st.ts[0].total + st.ts[1].total;
@@ -961,7 +885,8 @@ __device__ void build_slots(const Params &p, DevState &st, long long *s_buf)
 }
 
 // input check: flags[0] = non-finite star coordinates / masses, flags[1] = pairs of coincident stars
-// (two stars at the same point make P(z) lose two roots: the degree claim 2N fails)
+// (two stars at the same point make P(z) lose two roots: the degree claim 2N fails),
+// flags[2] = masses that differ from masses[0] (0: an equal-mass field, which takes the lighter pair body)
 __global__ void k_check_stars(const double2 *__restrict__ stars, const double *__restrict__ masses, int N,
                               int *flags)
 {
@@ -972,6 +897,7 @@ __global__ void k_check_stars(const double2 *__restrict__ stars, const double *_
         me = stars[i];
         const double m = masses[i];
         if (!(fabs(me.x) <= 1e100) || !(fabs(me.y) <= 1e100) || !(fabs(m) <= 1e100)) atomicAdd(&flags[0], 1);
+        if (m != masses[0]) atomicAdd(&flags[2], 1);
     }
     int same = 0;
     for (int base = 0; base < N; base += BLOCK) {
@@ -999,9 +925,10 @@ __global__ void __launch_bounds__(FIN) k_init(Params p)
     if (threadIdx.x == 0) *p.state = st;
 }
 
-__global__ void __launch_bounds__(FIN) k_finalize(Params p)
+// Closes an iteration (run by the LAST CTA of k_apply_write, FIN threads): swaps the active lists, detects the end
+// of a step, writes the rows' diagnostics, builds the next step's slots and the tile tables of the next launch.
+__device__ void finalize_iteration(const Params &p, long long *s_buf)
 {
-    __shared__ long long s_buf[33];
     DevState st = *p.state;   // every thread carries the same copy and makes the same decisions
     if (st.done) return;
     const int s = threadIdx.x;
@@ -1015,8 +942,9 @@ __global__ void __launch_bounds__(FIN) k_finalize(Params p)
     st.n_outside = 0;
     int left = 0;
     if (s < st.n_slots) {
-        if (p.n_active[st.cur * MAX_SLOTS + s] > 0) p.slot_iters[s] = st.iter;
-        left = p.n_active[(st.cur ^ 1) * MAX_SLOTS + s];
+        // (written by other CTAs of this launch: read through L2)
+        if (__ldcg(&p.n_active[st.cur * MAX_SLOTS + s]) > 0) p.slot_iters[s] = st.iter;
+        left = __ldcg(&p.n_active[(st.cur ^ 1) * MAX_SLOTS + s]);
     }
     long long remaining;
     block_scan(left, &remaining, s_buf);
@@ -1041,6 +969,167 @@ __global__ void __launch_bounds__(FIN) k_finalize(Params p)
     if (s == 0) *p.state = st;
 }
 
+// ------------------------------------------------------------------------------------------------
+// apply: z_k -= Delta_k, freeze converged roots, compact the list of unfrozen roots IN ORDER (survivors that keep the
+// Aberth sum first, then the others), so the next iteration's tiles -- and with them the summation order of every
+// root -- do not depend on the timing of a launch: two runs give the same bits.
+// A slot's list is cut into chunks of APPLY_CHUNK entries, one CTA each:
+//   k_apply_count  counts the two kinds of survivors of every chunk (reads the steps only);
+//   k_apply_write  applies the steps and writes the survivors at the offsets the counts give; the last CTA of the
+//                  grid to finish (a ticket) then closes the iteration (finalize_iteration).
+// grid of both: (chunks of the longest list, max_slots)
+// ------------------------------------------------------------------------------------------------
+constexpr int APPLY_THREADS = FIN;   // the last CTA runs the state machine: one thread per slot
+constexpr int APPLY_ITEMS = 4;
+constexpr int APPLY_CHUNK = APPLY_THREADS * APPLY_ITEMS;
+constexpr int COUNT_THREADS = 256;
+
+__global__ void __launch_bounds__(COUNT_THREADS) k_apply_count(Params p)
+{
+    __shared__ int s_part[2][COUNT_THREADS / 32];
+    const DevState st = *p.state;
+    if (st.done) return;
+    const int slot = blockIdx.y, chunk = blockIdx.x;
+    if (slot >= st.n_slots) return;
+    const int n_act = p.n_active[st.cur * MAX_SLOTS + slot];
+    const int lo = chunk * APPLY_CHUNK, hi = min(n_act, lo + APPLY_CHUNK);
+    if (lo >= n_act) return;
+    const double2 *delta = p.delta + (long long)slot * p.n_r;
+    const bool guard = st.iter == 0 && trusted_step(p, st.step);
+    int n_large = 0, n_small = 0;
+    for (int pos = lo + threadIdx.x; pos < hi; pos += COUNT_THREADS) {
+        const double2 d = delta[pos];
+        const double d2 = d.x * d.x + d.y * d.y;
+        if (d2 <= 1.79769313486231570e308) {
+            const int kind = step_kind(d2, p.tol2, p.skip_below2, guard);
+            n_large += kind == 1;
+            n_small += kind == 2;
+        }
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        n_large += __shfl_xor_sync(0xffffffffu, n_large, o);
+        n_small += __shfl_xor_sync(0xffffffffu, n_small, o);
+    }
+    if ((threadIdx.x & 31) == 0) { s_part[0][threadIdx.x >> 5] = n_large; s_part[1][threadIdx.x >> 5] = n_small; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int a = 0, b = 0;
+        for (int w = 0; w < COUNT_THREADS / 32; ++w) { a += s_part[0][w]; b += s_part[1][w]; }
+        p.chunk_count[(size_t)slot * gridDim.x + chunk] = make_int2(a, b);
+    }
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(APPLY_THREADS) k_apply_write(Params p)
+{
+    __shared__ int s_warp[32];
+    __shared__ int s_total;
+    __shared__ long long s_buf[33];
+    __shared__ int s_last;
+    const DevState st = *p.state;
+    if (st.done) return;
+    const int slot = blockIdx.y, chunk = blockIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int n_act = slot < st.n_slots ? p.n_active[st.cur * MAX_SLOTS + slot] : 0;
+    const int c0 = chunk * APPLY_CHUNK;
+    if (c0 < n_act || (chunk == 0 && slot < st.n_slots)) {
+        // offsets of this chunk from the counts of the slot's chunks: large survivors first, then the small ones
+        const int n_chunks = (n_act + APPLY_CHUNK - 1) / APPLY_CHUNK;
+        int base_l = 0, base_s = 0, tot_l = 0, tot_s = 0;
+        for (int c = 0; c < n_chunks; ++c) {
+            const int2 v = p.chunk_count[(size_t)slot * gridDim.x + c];
+            if (c < chunk) { base_l += v.x; base_s += v.y; }
+            tot_l += v.x;
+            tot_s += v.y;
+        }
+        base_s += tot_l;
+        if (chunk == 0 && tid == 0) {
+            p.n_active[(st.cur ^ 1) * MAX_SLOTS + slot] = tot_l + tot_s;
+            p.n_small[(st.cur ^ 1) * MAX_SLOTS + slot] = tot_s;
+        }
+        if (c0 < n_act) {
+            const int *list = p.list + ((long long)st.cur * p.max_slots + slot) * p.n_r;
+            int *next = p.list + ((long long)(st.cur ^ 1) * p.max_slots + slot) * p.n_r;
+            const double2 *delta = p.delta + (long long)slot * p.n_r;
+            double2 *row = p.roots + p.slot_row[slot] * p.n_r;
+            float4 *slot_src = p.src + (size_t)slot * 2 * p.N_pad;
+            // First iteration of a trusted row: the steps were taken without the Aberth sum, i.e. they are Newton steps
+            // from the predicted seeds.  One below the skip threshold is applied as any confirming step is; a larger one
+            // says the prediction was not that good: it is NOT applied and the root gets a full Aberth iteration next.
+            const bool guard = st.iter == 0 && trusted_step(p, st.step);
+            int ks[APPLY_ITEMS];
+            int kind[APPLY_ITEMS];   // 0 frozen, 1 large, 2 small
+            int cnt = 0;
+#pragma unroll
+            for (int i = 0; i < APPLY_ITEMS; ++i) {
+                const int pos = c0 + tid * APPLY_ITEMS + i;
+                kind[i] = 0;
+                ks[i] = 0;
+                if (pos < n_act) {
+                    const int k = list[pos];
+                    const double2 d = delta[pos];
+                    const double d2 = d.x * d.x + d.y * d.y;
+                    if (d2 <= 1.79769313486231570e308) {   // finite step
+                        kind[i] = step_kind(d2, p.tol2, p.skip_below2, guard);
+                        if (!(guard && kind[i] == 1)) {     // (a rejected Newton step leaves z where it is)
+                            double2 z = row[k];
+                            z.x -= d.x;
+                            z.y -= d.y;
+                            row[k] = z;
+                            store_src<MODE>(slot_src, k, z);
+                        }
+                    } else {                                // NaN / Inf: freeze where it is, report
+                        atomicAdd(&p.state->degenerate, 1);
+                    }
+                    ks[i] = k;
+                    cnt += kind[i] == 1 ? 1 : (kind[i] == 2 ? (1 << 16) : 0);
+                }
+            }
+            int incl = cnt;   // inclusive scan over the warp, then over the warps (counts packed: large low, small high)
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int n = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += n;
+            }
+            if (lane == 31) s_warp[warp] = incl;
+            __syncthreads();
+            if (warp == 0) {
+                const int w = s_warp[lane];
+                int wi = w;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int n = __shfl_up_sync(0xffffffffu, wi, o);
+                    if (lane >= o) wi += n;
+                }
+                s_warp[lane] = wi - w;
+                if (lane == 31) s_total = wi;
+            }
+            __syncthreads();
+            const int excl = s_warp[warp] + incl - cnt;
+            int off_l = base_l + (excl & 0xffff), off_s = base_s + (excl >> 16);
+#pragma unroll
+            for (int i = 0; i < APPLY_ITEMS; ++i) {
+                if (kind[i] == 1) next[off_l++] = ks[i];
+                else if (kind[i] == 2) next[off_s++] = ks[i];
+            }
+        }
+    }
+    // ---- the last CTA to get here closes the iteration ----
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) {
+        const unsigned total = gridDim.x * gridDim.y;
+        const unsigned t = atomicAdd(p.ticket, 1u);
+        s_last = (t == total - 1);
+        if (s_last) *p.ticket = 0;   // for the next launch (ordered by the stream)
+    }
+    __syncthreads();
+    if (s_last) {
+        __threadfence();
+        finalize_iteration(p, s_buf);
+    }
+}
+
 // the kernels of one Aberth-sum mode / caustic fusion choice
 struct KernelSet {
     void (*prepare)(Params);
@@ -1052,15 +1141,19 @@ struct KernelSet {
 };
 
 template <int MODE>
-KernelSet kernel_set_mode(bool caus, bool fmm)
+KernelSet kernel_set_mode(bool caus, bool fmm, bool eqm)
 {
     constexpr int RR = MODE == MODE_F64 ? R_ROOTS_F64 : R_ROOTS_F32;
     KernelSet k;
-    k.prepare = k_prepare<MODE>; k.seed = k_seed<MODE>; k.apply = k_apply<MODE>;
+    k.prepare = k_prepare<MODE>; k.seed = k_seed<MODE>; k.apply = k_apply_write<MODE>;
     if (fmm) {
         k.compute = caus ? k_compute<MODE, true, false, true, RR> : k_compute<MODE, false, false, true, RR>;
         k.compute_noA = caus ? k_compute<MODE, true, false, false, RR> : k_compute<MODE, false, false, false, RR>;
         k.R = RR;
+    } else if (eqm) {
+        k.compute = caus ? k_compute<MODE, true, true, true, R_STARS, true> : k_compute<MODE, false, true, true, R_STARS, true>;
+        k.compute_noA = caus ? k_compute<MODE, true, true, false, R_STARS, true> : k_compute<MODE, false, true, false, R_STARS, true>;
+        k.R = R_STARS;
     } else {
         k.compute = caus ? k_compute<MODE, true, true, true, R_STARS> : k_compute<MODE, false, true, true, R_STARS>;
         k.compute_noA = caus ? k_compute<MODE, true, true, false, R_STARS> : k_compute<MODE, false, true, false, R_STARS>;
@@ -1069,9 +1162,9 @@ KernelSet kernel_set_mode(bool caus, bool fmm)
     return k;
 }
 
-KernelSet kernel_set(int mode, bool caus, bool fmm)
+KernelSet kernel_set(int mode, bool caus, bool fmm, bool eqm)
 {
-    return mode == MODE_F64 ? kernel_set_mode<MODE_F64>(caus, fmm) : kernel_set_mode<MODE_F32>(caus, fmm);
+    return mode == MODE_F64 ? kernel_set_mode<MODE_F64>(caus, fmm, eqm) : kernel_set_mode<MODE_F32>(caus, fmm, eqm);
 }
 
 }  // namespace
@@ -1134,6 +1227,93 @@ struct RunStream {
     }
 };
 
+// The chain regime: stars checked, one launch, one read-back (flags + counters), rows copied to the host buffers
+// of the _host entry points at the end (these fields are small).
+static int chain_solve(const double *star_xy, const double *masses, int64_t N, int n_r, double kappa_s, double gamma,
+                       int64_t num_phi, double tol, double skip_below, int max_iter, int max_iter_cold, int order,
+                       const std::vector<double2> &rot, int n_sub, const std::vector<long long> &first,
+                       const std::vector<long long> &centre, const std::vector<long long> &end, int max_steps,
+                       const double *init_roots, double *out_roots, double *out_caustics, int32_t *out_iters,
+                       int32_t *out_unconverged, mlcc_stats *out_stats, cudaStream_t stream, double *h_roots,
+                       double *h_caustics)
+{
+    NvtxRange nvtx_("mlcc: solve, chain regime (star check + one launch: cold rows and continuation steps run on chip)");
+    Workspace ws(stream);
+    double2 *d_rot = nullptr;
+    long long *d_plan = nullptr;
+    int *d_flags = nullptr;
+    unsigned char *d_counters = nullptr;
+    const size_t cbytes = chain_counters_bytes();
+    MLCC_CUDA(ws.alloc(&d_rot, (size_t)num_phi));
+    MLCC_CUDA(ws.alloc(&d_plan, (size_t)3 * n_sub));
+    MLCC_CUDA(ws.alloc(&d_flags, 4));
+    MLCC_CUDA(ws.alloc(&d_counters, cbytes));
+    static thread_local PinnedBlock tl_back;   // flags + counters come back through pinned memory
+    MLCC_CUDA(tl_back.reserve(2 * sizeof(int) + 8 + cbytes));
+    int *h_flags = static_cast<int *>(tl_back.p);
+    unsigned char *h_counters = static_cast<unsigned char *>(tl_back.p) + 16;
+    std::vector<long long> plan((size_t)3 * n_sub);
+    for (int c = 0; c < n_sub; ++c) { plan[c] = first[c]; plan[n_sub + c] = centre[c]; plan[2 * n_sub + c] = end[c]; }
+    MLCC_CUDA(cudaMemcpyAsync(d_rot, rot.data(), sizeof(double2) * (size_t)num_phi, cudaMemcpyHostToDevice, stream));
+    MLCC_CUDA(cudaMemcpyAsync(d_plan, plan.data(), sizeof(long long) * plan.size(), cudaMemcpyHostToDevice, stream));
+    MLCC_CUDA(cudaMemsetAsync(d_flags, 0, 4 * sizeof(int), stream));
+    Event ev0, ev1;
+    MLCC_CUDA(ev0.create());
+    MLCC_CUDA(ev1.create());
+    MLCC_CUDA(cudaEventRecord(ev0, stream));
+    k_check_stars<<<(unsigned)((N + BLOCK - 1) / BLOCK), BLOCK, 0, stream>>>(
+        reinterpret_cast<const double2 *>(star_xy), masses, (int)N, d_flags);
+    const int lrc = chain_launch(star_xy, masses, N, n_r, gamma, 1.0 - kappa_s, tol, skip_below, max_iter, max_iter_cold,
+                                 order, d_rot, init_roots, out_roots, out_caustics, out_iters, out_unconverged, n_sub,
+                                 d_plan, d_plan + n_sub, d_plan + 2 * n_sub, d_counters, stream);
+    if (lrc != MLCC_OK) return lrc;
+    MLCC_CUDA(cudaEventRecord(ev1, stream));
+    MLCC_CUDA(cudaMemcpyAsync(h_flags, d_flags, 2 * sizeof(int), cudaMemcpyDeviceToHost, stream));
+    MLCC_CUDA(cudaMemcpyAsync(h_counters, d_counters, cbytes, cudaMemcpyDeviceToHost, stream));
+    if (h_roots) {
+        const size_t bytes = (size_t)num_phi * n_r * 2 * sizeof(double);
+        MLCC_CUDA(cudaMemcpyAsync(h_roots, out_roots, bytes, cudaMemcpyDeviceToHost, stream));
+        if (h_caustics && out_caustics)
+            MLCC_CUDA(cudaMemcpyAsync(h_caustics, out_caustics, bytes, cudaMemcpyDeviceToHost, stream));
+    }
+    cudaError_t es = cudaStreamSynchronize(stream);
+    if (es == cudaSuccess) es = cudaGetLastError();
+    if (es != cudaSuccess) return cuda_fail(es, "critical-curve kernel (chain regime)", __FILE__, __LINE__);
+    if (h_flags[0]) return invalid("non-finite (or > 1e100) star position or mass");
+    if (h_flags[1]) {
+        set_last_error("coincident stars: P(z) loses roots (merge them into one star of the summed mass)");
+        return MLCC_ERR_DEGENERATE;
+    }
+    ChainRun run{};
+    chain_read_counters(h_counters, &run);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, ev0, ev1);
+    if (out_stats) {
+        out_stats->root_iterations = (int64_t)run.root_iterations;
+        out_stats->star_pairs = (int64_t)run.root_iterations * N;
+        out_stats->root_pairs = (int64_t)(run.root_iterations - run.root_iterations_noA) * (n_r - 1);
+        out_stats->kernel_launches = 2;   // star check, chain kernel
+        out_stats->total_iterations = run.max_iterations;   // the longest CTA's iterations: the critical path
+        out_stats->steps = max_steps + 1;
+        out_stats->subchains = n_sub;
+        out_stats->predictor_order = order;
+        out_stats->unconverged_rows = run.unconverged_rows;
+        out_stats->degenerate_roots = run.degenerate;
+        out_stats->solve_ms = ms;
+        out_stats->aberth_sum_precision = 64;
+        out_stats->regime = MLCC_REGIME_CHAIN;
+    }
+    if (run.degenerate > 0) {
+        set_last_error("NaN/Inf Aberth step: a root landed on a star or another root, or stars coincide");
+        return MLCC_ERR_DEGENERATE;
+    }
+    if (run.unconverged_rows > 0) {
+        set_last_error("some roots were still unfrozen at max_iter");
+        return MLCC_ERR_NOT_CONVERGED;
+    }
+    return MLCC_OK;
+}
+
 // h_roots / h_caustics (host-buffer entry points; may be null): PINNED host arrays of the shape of out_roots /
 // out_caustics.  Rows are final as soon as their step is over (nothing writes them again, the predictor only reads
 // them) and a sub-chain's finished rows are one interval that grows at both ends, so the rows each poll of the state
@@ -1161,14 +1341,16 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     }
     const int64_t phi_total = opt.phi_index_total > 0 ? opt.phi_index_total : num_phi;
     const int64_t phi_off = opt.phi_index_offset;
-    int order = opt.predictor_order < 0 ? 3 : opt.predictor_order;
+    int order = opt.predictor_order < 0 ? DEFAULT_ORDER_TILED : opt.predictor_order;
     if (order > MAX_ORDER) return invalid("predictor_order > 5");
     int min_T = opt.min_lanes_per_root <= 0 ? 1 : opt.min_lanes_per_root;
     if (min_T > CTA || (min_T & (min_T - 1))) return invalid("min_lanes_per_root must be a power of two <= 128");
     if (opt.num_subchains < 0 || opt.max_iter_cold < 0) return invalid("negative option");
     if (opt.aberth_sum_precision != 0 && opt.aberth_sum_precision != 32 && opt.aberth_sum_precision != 64)
         return invalid("aberth_sum_precision must be 0, 32 or 64");
-    const int mode = opt.aberth_sum_precision == 64 ? MODE_F64 : MODE_F32;
+    const int mode = opt.aberth_sum_precision == 32 ? MODE_F32 : MODE_F64;   // 0 = library default = FP64
+    if (opt.regime != MLCC_REGIME_AUTO && opt.regime != MLCC_REGIME_TILED && opt.regime != MLCC_REGIME_CHAIN)
+        return invalid("regime");
     if (!isfinite(opt.skip_aberth_sum_below)) return invalid("skip_aberth_sum_below");
     if (opt.trust_predictor != 0 && opt.trust_predictor != 1) return invalid("trust_predictor must be 0 or 1");
     if (opt.star_sum_mode != MLCC_STAR_SUMS_DIRECT && opt.star_sum_mode != MLCC_STAR_SUMS_FMM)
@@ -1186,10 +1368,45 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     }
     if (1.0 - kappa_s == 0.0 && gamma == 0.0) return invalid("kappa_s = 1 and gamma = 0");
 
+    // sheet polynomial: n_extra = deg H' = poly_n - 2 more roots per row
+    const int poly_n = opt.sheet_poly ? opt.sheet_poly_n : 0;
+    if (poly_n < 0 || poly_n > 512) return invalid("sheet_poly_n out of range");
+    if (poly_n > 0) {
+        for (int q = 0; q < poly_n; ++q)
+            if (!isfinite(opt.sheet_poly[q])) return invalid("sheet_poly has a non-finite coefficient");
+        if (opt.sheet_poly[poly_n - 1] == 0.0) return invalid("the last sheet_poly coefficient is zero");
+    }
+    const int n_extra = poly_n >= 3 ? poly_n - 2 : 0;
+    if (n_extra > 0 && !init_roots && !(opt.seed_radius > 0.0 && isfinite(opt.seed_radius)))
+        return invalid("seed_radius must be positive when the sheet polynomial adds roots");
+    if (2 * N + n_extra > (1ll << 30)) return invalid("too many roots");
+    const int n_r = (int)(2 * N) + n_extra;
+    // a stage pairs 256 stars with 512 root entries: enough (massless, far away) padding stars for all roots
+    const long long n_half = (n_r + 1) / 2 > N ? (n_r + 1) / 2 : N;
+    const int N_pad = (int)((n_half + S_TILE - 1) / S_TILE) * S_TILE;
+
+    // ---- which regime ----
+    // chain: one CTA per sub-chain, everything in shared memory (chain.cu); tiled: the launches below.
+    const bool use_fmm = opt.star_sum_mode == MLCC_STAR_SUMS_FMM;
+    const bool chain_able = !use_fmm && poly_n == 0 && opt.trust_predictor == 0 && opt.aberth_sum_precision != 32 &&
+                            opt.min_lanes_per_root <= 1;
+    int chain_cap = 0;
+    if (opt.regime != MLCC_REGIME_TILED && chain_able) chain_cap = chain_capacity(N, n_r, out_caustics != nullptr);
+    if (opt.regime == MLCC_REGIME_CHAIN && chain_cap < 1)
+        return invalid("regime = MLCC_REGIME_CHAIN needs direct star sums, no sheet polynomial, no trust_predictor, "
+                       "an FP64 Aberth sum and a field that fits shared memory (about 1200 stars)");
+    const bool use_chain = chain_cap >= 1 && (opt.regime == MLCC_REGIME_CHAIN || n_r <= CHAIN_AUTO_MAX_ROOTS);
+
     // plan
     std::vector<long long> first(MAX_SLOTS), centre(MAX_SLOTS), end(MAX_SLOTS);
     std::vector<int64_t> f64v(MAX_SLOTS), c64v(MAX_SLOTS), e64v(MAX_SLOTS);
     int want_sub = opt.num_subchains;
+    if (want_sub == 0 && use_chain) {
+        // one CTA per sub-chain, one wave of CTAs; a cold row costs about as much as two continued ones, so chains
+        // shorter than 8 rows are not worth their cold start
+        long long w = std::min<long long>(chain_cap, num_phi / 8);
+        want_sub = (int)std::max<long long>(1, std::min<long long>(w, MAX_SLOTS / 2));
+    }
     if (want_sub == 0 && opt.trust_predictor == 1 && opt.star_sum_mode == MLCC_STAR_SUMS_FMM) {
         // Continued rows cost O(N) here (far-field star sums, no Aberth sum): a step of the default plan is a handful
         // of short, latency-bound launches.  Four times as many rows per step amortise them; the price is four times
@@ -1212,24 +1429,16 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
         if (a > max_steps) max_steps = (int)a;
         if (b > max_steps) max_steps = (int)b;
     }
-    const int max_slots = 2 * n_sub > 1 ? 2 * n_sub : 1;
-    // sheet polynomial: n_extra = deg H' = poly_n - 2 more roots per row
-    const int poly_n = opt.sheet_poly ? opt.sheet_poly_n : 0;
-    if (poly_n < 0 || poly_n > 512) return invalid("sheet_poly_n out of range");
-    if (poly_n > 0) {
-        for (int q = 0; q < poly_n; ++q)
-            if (!isfinite(opt.sheet_poly[q])) return invalid("sheet_poly has a non-finite coefficient");
-        if (opt.sheet_poly[poly_n - 1] == 0.0) return invalid("the last sheet_poly coefficient is zero");
+    const int order_used = opt.predictor_order < 0 ? DEFAULT_ORDER_CHAIN : opt.predictor_order;
+    if (use_chain) {
+        const double sb = opt.skip_aberth_sum_below == 0.0 ? 1e-8 : opt.skip_aberth_sum_below;   // on at every N here
+        return chain_solve(star_xy, masses, N, n_r, kappa_s, gamma, num_phi, tol, sb, max_iter,
+                           opt.max_iter_cold > 0 ? opt.max_iter_cold : max_iter, order_used, rot, n_sub, first, centre,
+                           end, max_steps, init_roots, out_roots, out_caustics, out_iters, out_unconverged, out_stats,
+                           stream, h_roots, h_caustics);
     }
-    const int n_extra = poly_n >= 3 ? poly_n - 2 : 0;
-    if (n_extra > 0 && !init_roots && !(opt.seed_radius > 0.0 && isfinite(opt.seed_radius)))
-        return invalid("seed_radius must be positive when the sheet polynomial adds roots");
-    if (2 * N + n_extra > (1ll << 30)) return invalid("too many roots");
-    const int n_r = (int)(2 * N) + n_extra;
-    // a stage pairs 256 stars with 512 root entries: enough (massless, far away) padding stars for all roots
-    const long long n_half = (n_r + 1) / 2 > N ? (n_r + 1) / 2 : N;
-    const int N_pad = (int)((n_half + S_TILE - 1) / S_TILE) * S_TILE;
-
+    const int max_slots = 2 * n_sub > 1 ? 2 * n_sub : 1;
+    NvtxRange nvtx_("mlcc: solve, tiled regime");
     RunStream run_stream;            // declared before the workspace: destroyed after it
     MLCC_CUDA(run_stream.open(stream));
     stream = run_stream.run;
@@ -1270,15 +1479,17 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     MLCC_CUDA(cudaMemsetAsync(p.n_active, 0, sizeof(int) * 2 * MAX_SLOTS, stream));
     MLCC_CUDA(cudaMemsetAsync(p.n_small, 0, sizeof(int) * 2 * MAX_SLOTS, stream));
 
-    // input check (one small read-back before the solve)
+    // input check (one small read-back before the solve); flags[2] = 0 says every star has the mass masses[0]
+    int h_flags[3] = {0, 0, 0};
+    double mass0 = 0.0;
     {
         int *d_flags = nullptr;
-        MLCC_CUDA(ws.alloc(&d_flags, 2));
-        MLCC_CUDA(cudaMemsetAsync(d_flags, 0, 2 * sizeof(int), stream));
+        MLCC_CUDA(ws.alloc(&d_flags, 4));
+        MLCC_CUDA(cudaMemsetAsync(d_flags, 0, 4 * sizeof(int), stream));
         k_check_stars<<<(unsigned)((N + BLOCK - 1) / BLOCK), BLOCK, 0, stream>>>(
             reinterpret_cast<const double2 *>(star_xy), masses, (int)N, d_flags);
-        int h_flags[2] = {0, 0};
-        MLCC_CUDA(cudaMemcpyAsync(h_flags, d_flags, 2 * sizeof(int), cudaMemcpyDeviceToHost, stream));
+        MLCC_CUDA(cudaMemcpyAsync(h_flags, d_flags, 3 * sizeof(int), cudaMemcpyDeviceToHost, stream));
+        MLCC_CUDA(cudaMemcpyAsync(&mass0, masses, sizeof(double), cudaMemcpyDeviceToHost, stream));
         MLCC_CUDA(cudaStreamSynchronize(stream));
         MLCC_CUDA(cudaGetLastError());
         if (h_flags[0]) return invalid("non-finite (or > 1e100) star position or mass");
@@ -1288,8 +1499,8 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
         }
     }
 
-    const bool use_fmm = opt.star_sum_mode == MLCC_STAR_SUMS_FMM;
-    const KernelSet ks = kernel_set(mode, out_caustics != nullptr, use_fmm);
+    const bool eqm = h_flags[2] == 0;
+    const KernelSet ks = kernel_set(mode, out_caustics != nullptr, use_fmm, eqm);
     int blocks_per_sm = 0;
     MLCC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, ks.compute, CTA, 0));
     if (blocks_per_sm < 1) blocks_per_sm = 1;
@@ -1302,6 +1513,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     p.n_r = n_r;
     p.N_pad = N_pad;
     p.gamma = gamma;
+    p.mass0 = mass0;
     p.omk = 1.0 - kappa_s;
     p.tol2 = tol * tol;
     p.max_iter = max_iter;
@@ -1362,7 +1574,11 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     const int grid_seed = sms * 4;
     ks.prepare<<<grid_seed, BLOCK, 0, stream>>>(p);
     k_init<<<1, FIN, 0, stream>>>(p);
-    const int grid_apply = max_slots;
+    const int n_chunks = (n_r + APPLY_CHUNK - 1) / APPLY_CHUNK;
+    const dim3 grid_apply((unsigned)n_chunks, (unsigned)max_slots);
+    MLCC_CUDA(ws.alloc(&p.chunk_count, (size_t)n_chunks * max_slots));
+    MLCC_CUDA(ws.alloc(&p.ticket, 1));
+    MLCC_CUDA(cudaMemsetAsync(p.ticket, 0, sizeof(unsigned), stream));
     const dim3 grid_star((unsigned)((n_r + BLOCK - 1) / BLOCK), (unsigned)max_slots);
     // Upper bound on iteration groups, so that a device-side fault cannot spin the host forever.
     const long long max_groups = (long long)(max_steps + 1) * (long long)(p.max_iter > p.max_iter_cold ? p.max_iter : p.max_iter_cold) + 8;
@@ -1402,8 +1618,8 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
             }
             ks.compute<<<grid_compute, CTA, 0, stream>>>(p);
             if (skip_on) ks.compute_noA<<<grid_compute, CTA, 0, stream>>>(p);
+            k_apply_count<<<grid_apply, COUNT_THREADS, 0, stream>>>(p);
             ks.apply<<<grid_apply, APPLY_THREADS, 0, stream>>>(p);
-            k_finalize<<<1, FIN, 0, stream>>>(p);
         }
     };
     // Every launch of a chunk has the same arguments (the state lives on the device), so the chunk is captured once
@@ -1414,7 +1630,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
         // kernels are loaded lazily at their first launch, and loading is not allowed inside a capture: touch them first
         cudaFuncAttributes fa;
         const void *fns[] = {(const void *)ks.seed, (const void *)ks.compute, (const void *)ks.compute_noA,
-                             (const void *)ks.apply, (const void *)k_finalize, (const void *)k_star_sums,
+                             (const void *)ks.apply, (const void *)k_apply_count, (const void *)k_star_sums,
                              (const void *)k_star_sums_outside};
         for (const void *f : fns) cudaFuncGetAttributes(&fa, f);
         cudaGetLastError();
@@ -1428,7 +1644,9 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
         }
         if (!chunk_exec) cudaGetLastError();
     }
+    int steps_seen = 0;
     while (!finished && groups < max_groups + 2 * chunk) {
+        NvtxRange nvtx_chunk("mlcc: enqueue a chunk of 16 iteration groups (seed, compute, apply)");
         if (!chunk_exec || cudaGraphLaunch(chunk_exec, stream) != cudaSuccess) {
             if (chunk_exec) { cudaGetLastError(); cudaGraphExecDestroy(chunk_exec); chunk_exec = nullptr; }
             enqueue_chunk();
@@ -1442,6 +1660,13 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
             cudaError_t es = cudaEventSynchronize(ev_poll[which ^ 1]);
             if (es != cudaSuccess) { rc = cuda_fail(es, "cudaEventSynchronize", __FILE__, __LINE__); break; }
             if (h_state[which ^ 1].done) finished = true;
+            if (h_state[which ^ 1].step > steps_seen) {   // step 0 = the cold centre rows, then the continuation steps
+                char text[96];
+                snprintf(text, sizeof text, "mlcc: steps %d..%d finished (step 0 = cold rows)", steps_seen,
+                         h_state[which ^ 1].step - 1);
+                nvtxMarkA(text);
+                steps_seen = h_state[which ^ 1].step;
+            }
             copy_finished(h_state[which ^ 1].step);   // that snapshot is complete: every launch before it has run
         }
         which ^= 1;
@@ -1481,6 +1706,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
         out_stats->degenerate_roots = fin.degenerate;
         out_stats->solve_ms = ms;
         out_stats->aberth_sum_precision = mode == MODE_F64 ? 64 : 32;
+        out_stats->regime = MLCC_REGIME_TILED;
     }
     if (fin.degenerate > 0) {
         set_last_error("NaN/Inf Aberth step: a root landed on a star or another root, or stars coincide");

@@ -131,7 +131,7 @@ void mlcc_options_default(mlcc_options *opt)
     opt->trust_predictor = 0;
     opt->sheet_poly = nullptr;
     opt->sheet_poly_n = 0;
-    opt->reserved2_ = 0;
+    opt->regime = MLCC_REGIME_AUTO;
     opt->seed_radius = 0.0;
     opt->skip_aberth_sum_below = 0.0;
 }
@@ -139,6 +139,7 @@ void mlcc_options_default(mlcc_options *opt)
 int mlcc_star_field(uint64_t seed, int64_t N, double kappa_star, int mass_model, const double *mass_params,
                     double *star_xy, double *masses, double *out_radius, void *stream)
 {
+    NvtxRange nvtx_("mlcc_star_field");
     return star_field_impl(seed, N, kappa_star, mass_model, mass_params, 0.0, star_xy, masses, out_radius, nullptr,
                            static_cast<cudaStream_t>(stream));
 }
@@ -146,6 +147,7 @@ int mlcc_star_field(uint64_t seed, int64_t N, double kappa_star, int mass_model,
 int mlcc_star_field_rect(uint64_t seed, int64_t N, double kappa_star, double aspect, int mass_model,
                          const double *mass_params, double *star_xy, double *masses, double *out_corner, void *stream)
 {
+    NvtxRange nvtx_("mlcc_star_field_rect");
     if (!(aspect > 0.0)) {
         set_last_error("invalid argument: aspect must be positive");
         return MLCC_ERR_INVALID_ARG;
@@ -157,6 +159,7 @@ int mlcc_star_field_rect(uint64_t seed, int64_t N, double kappa_star, double asp
 int mlcc_critical_curves(const double *star_xy, const double *masses, int64_t N, double kappa_s, double gamma,
                          int64_t num_phi, double tol, int32_t max_iter, double *out_roots)
 {
+    NvtxRange nvtx_("mlcc_critical_curves");
     return critical_curves_impl(star_xy, masses, N, kappa_s, gamma, num_phi, tol, max_iter, out_roots, nullptr,
                                 nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
 }
@@ -166,6 +169,7 @@ int mlcc_critical_curves_ex(const double *star_xy, const double *masses, int64_t
                             const mlcc_options *opt, const double *init_roots, int32_t *out_iters,
                             int32_t *out_unconverged, mlcc_stats *out_stats, void *stream)
 {
+    NvtxRange nvtx_("mlcc_critical_curves_ex");
     return critical_curves_impl(star_xy, masses, N, kappa_s, gamma, num_phi, tol, max_iter, out_roots, nullptr,
                                 opt, init_roots, out_iters, out_unconverged, out_stats,
                                 static_cast<cudaStream_t>(stream));
@@ -176,6 +180,7 @@ int mlcc_curves_and_caustics(const double *star_xy, const double *masses, int64_
                              double *out_caustics, const mlcc_options *opt, const double *init_roots,
                              int32_t *out_iters, int32_t *out_unconverged, mlcc_stats *out_stats, void *stream)
 {
+    NvtxRange nvtx_("mlcc_curves_and_caustics");
     if (!out_caustics) return invalid("null pointer");
     return critical_curves_impl(star_xy, masses, N, kappa_s, gamma, num_phi, tol, max_iter, out_roots,
                                 out_caustics, opt, init_roots, out_iters, out_unconverged, out_stats,
@@ -185,6 +190,7 @@ int mlcc_curves_and_caustics(const double *star_xy, const double *masses, int64_
 int mlcc_caustics(const double *star_xy, const double *masses, int64_t N, double kappa_s, double gamma,
                   const double *points, int64_t P, double *out_caustics, void *stream)
 {
+    NvtxRange nvtx_("mlcc_caustics");
     return caustics_impl(star_xy, masses, N, kappa_s, gamma, points, P, out_caustics,
                          static_cast<cudaStream_t>(stream));
 }
@@ -197,6 +203,7 @@ int64_t mlcc_num_roots(int64_t N, int32_t sheet_poly_n)
 int mlcc_rect_sheet(double kappa_star, double c1, double c2, double s, double eps, int32_t t_in, double *out_coef,
                     int32_t capacity, double *out_gamma_shift)
 {
+    NvtxRange nvtx_("mlcc_rect_sheet");
     if (!out_coef || !out_gamma_shift) return -invalid("null pointer");
     if (!(kappa_star >= 0.0) || !(c1 > 0.0) || !(c2 > 0.0) || !isfinite(kappa_star + c1 + c2)) return -invalid("kappa_star, c1, c2");
     const double pi = 3.14159265358979323846264338327950288;
@@ -226,12 +233,14 @@ int mlcc_rect_sheet(double kappa_star, double c1, double c2, double s, double ep
 int mlcc_link_rows(const double *rows, int64_t S, int64_t n, int32_t *out_next, int32_t *out_bijective,
                    void *stream)
 {
+    NvtxRange nvtx_("mlcc_link_rows");
     return link_rows_impl(rows, S, n, out_next, out_bijective, static_cast<cudaStream_t>(stream));
 }
 
 int mlcc_crossing_map(const double *caustics, const int32_t *next, int64_t S, int64_t n, int closed, double x0,
                       double y0, double pixel, int32_t nx, int32_t ny, int32_t *out_map, void *stream)
 {
+    NvtxRange nvtx_("mlcc_crossing_map");
     return crossing_map_impl(caustics, next, S, n, closed, x0, y0, pixel, nx, ny, out_map,
                              static_cast<cudaStream_t>(stream));
 }
@@ -239,6 +248,7 @@ int mlcc_crossing_map(const double *caustics, const int32_t *next, int64_t S, in
 int mlcc_closed_loops(const int32_t *next, int64_t S, int64_t n, int32_t *out_chain_col, int32_t *out_chain_end,
                       int32_t *out_loop_id, int32_t *out_num_loops, void *stream)
 {
+    NvtxRange nvtx_("mlcc_closed_loops");
     return closed_loops_impl(next, S, n, out_chain_col, out_chain_end, out_loop_id, out_num_loops,
                              static_cast<cudaStream_t>(stream));
 }
@@ -246,18 +256,21 @@ int mlcc_closed_loops(const int32_t *next, int64_t S, int64_t n, int32_t *out_ch
 int mlcc_order_by_chain(const double *points, const int32_t *chain_col, int64_t S, int64_t n, double *out,
                         void *stream)
 {
+    NvtxRange nvtx_("mlcc_order_by_chain");
     return order_by_chain_impl(points, chain_col, S, n, out, static_cast<cudaStream_t>(stream));
 }
 
 int mlcc_distance_map(const int32_t *crossing_map, int32_t nx, int32_t ny, double pixel, double *out_distance,
                       int64_t *out_d2, void *stream)
 {
+    NvtxRange nvtx_("mlcc_distance_map");
     return distance_map_impl(crossing_map, nx, ny, pixel, out_distance, out_d2, static_cast<cudaStream_t>(stream));
 }
 
 int mlcc_directional_distance_map(const int32_t *crossing_map, int32_t nx, int32_t ny, double pixel, int32_t ux,
                                   int32_t uy, double *out_distance, void *stream)
 {
+    NvtxRange nvtx_("mlcc_directional_distance_map");
     return directional_distance_map_impl(crossing_map, nx, ny, pixel, ux, uy, out_distance,
                                          static_cast<cudaStream_t>(stream));
 }
@@ -265,6 +278,7 @@ int mlcc_directional_distance_map(const int32_t *crossing_map, int32_t nx, int32
 int mlcc_distance_histogram(const double *distance, const int32_t *crossing_map, int64_t num_pixels, double bin_width,
                             int32_t num_bins, int32_t num_counts, int64_t *out_hist, int64_t *out_left_out, void *stream)
 {
+    NvtxRange nvtx_("mlcc_distance_histogram");
     return distance_histogram_impl(distance, crossing_map, num_pixels, bin_width, num_bins, num_counts, out_hist,
                                    out_left_out, static_cast<cudaStream_t>(stream));
 }
@@ -273,6 +287,7 @@ int mlcc_vieta_residuals(const double *star_xy, const double *masses, int64_t N,
                          const double *roots, int64_t num_phi, int64_t phi_index_offset, int64_t phi_index_total,
                          double *out_e1, double *out_e2, void *stream)
 {
+    NvtxRange nvtx_("mlcc_vieta_residuals");
     return vieta_residuals_impl(star_xy, masses, N, kappa_s, gamma, roots, num_phi, phi_index_offset, phi_index_total,
                                 out_e1, out_e2, static_cast<cudaStream_t>(stream));
 }
@@ -282,6 +297,7 @@ int mlcc_detj_residuals(const double *star_xy, const double *masses, int64_t N, 
                         int64_t phi_index_total, double *out_residuals, double *out_row_newton, double *out_row_detj,
                         void *stream)
 {
+    NvtxRange nvtx_("mlcc_detj_residuals");
     return detj_residuals_impl(star_xy, masses, N, kappa_s, gamma, points, num_phi, n, phi_index_offset,
                                phi_index_total, out_residuals, out_row_newton, out_row_detj,
                                static_cast<cudaStream_t>(stream));
@@ -290,6 +306,7 @@ int mlcc_detj_residuals(const double *star_xy, const double *masses, int64_t N, 
 int mlcc_star_sums(const double *star_xy, const double *masses, int64_t N, const double *points, int64_t P,
                    int mode, int fmm_order, int fmm_stars_per_node, double *out_sums, void *stream)
 {
+    NvtxRange nvtx_("mlcc_star_sums");
     return star_sums_impl(star_xy, masses, N, points, P, mode, fmm_order, fmm_stars_per_node, out_sums,
                           static_cast<cudaStream_t>(stream));
 }
@@ -297,6 +314,7 @@ int mlcc_star_sums(const double *star_xy, const double *masses, int64_t N, const
 int mlcc_match_root_sets(const double *a, const double *b, int64_t S, int64_t n, double rel_tol,
                          double *out_max_err, int32_t *out_bijective, void *stream)
 {
+    NvtxRange nvtx_("mlcc_match_root_sets");
     return match_root_sets_impl(a, b, S, n, rel_tol, out_max_err, out_bijective,
                                 static_cast<cudaStream_t>(stream));
 }
@@ -304,6 +322,7 @@ int mlcc_match_root_sets(const double *a, const double *b, int64_t S, int64_t n,
 int mlcc_plan_subchains(int64_t N, int64_t num_phi, int32_t num_subchains, int32_t capacity,
                         int64_t *first_row, int64_t *centre_row, int64_t *end_row)
 {
+    NvtxRange nvtx_("mlcc_plan_subchains");
     if (!first_row || !centre_row || !end_row) return -MLCC_ERR_INVALID_ARG;
     return plan_subchains_host(N, num_phi, num_subchains, capacity, first_row, centre_row, end_row);
 }
@@ -313,6 +332,7 @@ int mlcc_curves_and_caustics_host(const double *star_xy, const double *masses, i
                                   const mlcc_options *opt, double *out_roots, double *out_caustics,
                                   mlcc_stats *out_stats)
 {
+    NvtxRange nvtx_("mlcc_curves_and_caustics_host");
     if (!star_xy || !masses || !out_roots) return invalid("null pointer");
     if (N < 1 || N > (1 << 28)) return invalid("N out of range");
     if (num_phi < 1) return invalid("num_phi < 1");
@@ -346,6 +366,7 @@ int mlcc_curves_and_caustics_host(const double *star_xy, const double *masses, i
 int mlcc_critical_curves_host(const double *star_xy, const double *masses, int64_t N, double kappa_s,
                               double gamma, int64_t num_phi, double tol, int32_t max_iter, double *out_roots)
 {
+    NvtxRange nvtx_("mlcc_critical_curves_host");
     return mlcc_curves_and_caustics_host(star_xy, masses, N, kappa_s, gamma, num_phi, tol, max_iter, nullptr,
                                          out_roots, nullptr, nullptr);
 }
@@ -353,6 +374,7 @@ int mlcc_critical_curves_host(const double *star_xy, const double *masses, int64
 int mlcc_caustics_host(const double *star_xy, const double *masses, int64_t N, double kappa_s, double gamma,
                        const double *points, int64_t P, double *out_caustics)
 {
+    NvtxRange nvtx_("mlcc_caustics_host");
     if (!star_xy || !masses) return invalid("null pointer");
     if (N < 1 || N > (1 << 29)) return invalid("N out of range");
     if (P < 0) return invalid("P < 0");

@@ -174,6 +174,186 @@ __global__ void __launch_bounds__(BLOCK) k_match(const double2 *__restrict__ a, 
     }
 }
 
+// The same matching with the bins in SHARED memory (sets of up to ~27 000 points: cell table and sorted indices
+// are 8 bytes per point): one CTA of 1024 threads per set, counting sort with shared-memory atomics, block-wide scan
+// by warp shuffles, the bijection test by a bit per b_j (n marks on n slots without a repeat cover every slot).
+// The global-scratch kernel above stays for larger sets.
+constexpr int MBLOCK = 1024;
+
+__device__ __forceinline__ double block_reduce_m(double v, bool take_max, double *s_red /*[33]*/)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int o = 16; o > 0; o >>= 1) {
+        const double t = __shfl_xor_sync(0xffffffffu, v, o);
+        v = take_max ? fmax(v, t) : fmin(v, t);
+    }
+    __syncthreads();
+    if (lane == 0) s_red[warp] = v;
+    __syncthreads();
+    if (warp == 0) {
+        double w = s_red[lane];
+        for (int o = 16; o > 0; o >>= 1) {
+            const double t = __shfl_xor_sync(0xffffffffu, w, o);
+            w = take_max ? fmax(w, t) : fmin(w, t);
+        }
+        if (lane == 0) s_red[32] = w;
+    }
+    __syncthreads();
+    return s_red[32];
+}
+
+__global__ void __launch_bounds__(MBLOCK) k_match_smem(const double2 *__restrict__ a, const double2 *__restrict__ b,
+                                                       long long S, int n, double rel_tol, int G,
+                                                       double *out_max_err, int *out_bijective,
+                                                       long long b_shift, int *out_index)
+{
+    extern __shared__ int s_dyn[];
+    __shared__ double s_red[33];
+    __shared__ int s_part[MBLOCK / 32 + 1];
+    __shared__ int s_flag;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int ncell = G * G;
+    int *cell_start = s_dyn;                       // [ncell + 2]
+    int *sorted = cell_start + ncell + 2;          // [n]
+    unsigned *mask = reinterpret_cast<unsigned *>(sorted + n);   // [(n + 31) / 32]
+    const int n_words = (n + 31) >> 5;
+
+    for (long long s = blockIdx.x; s < S; s += gridDim.x) {
+        const double2 *as = a + s * n, *bs = b + ((s + b_shift) % S) * n;
+        // ---- bounding box of b, finiteness of a and b ----
+        double xmin = 1e308, xmax = -1e308, ymin = 1e308, ymax = -1e308, bad = 0.0;
+        for (int j = tid; j < n; j += MBLOCK) {
+            const double2 q = bs[j], q2 = as[j];
+            xmin = fmin(xmin, q.x); xmax = fmax(xmax, q.x);
+            ymin = fmin(ymin, q.y); ymax = fmax(ymax, q.y);
+            if (!(fabs(q.x) <= 1e300) || !(fabs(q.y) <= 1e300) || !(fabs(q2.x) <= 1e300) || !(fabs(q2.y) <= 1e300)) bad = 1.0;
+        }
+        xmin = block_reduce_m(xmin, false, s_red); xmax = block_reduce_m(xmax, true, s_red);
+        ymin = block_reduce_m(ymin, false, s_red); ymax = block_reduce_m(ymax, true, s_red);
+        bad = block_reduce_m(bad, true, s_red);
+        if (bad > 0.0) {
+            if (tid == 0) { if (out_max_err) out_max_err[s] = INFINITY; out_bijective[s] = 0; }
+            if (out_index) for (int i = tid; i < n; i += MBLOCK) out_index[s * n + i] = -1;
+            continue;
+        }
+        const double wx = xmax - xmin, wy = ymax - ymin;
+        const double hx = wx > 0.0 ? wx / G : 1.0, hy = wy > 0.0 ? wy / G : 1.0;
+        const double inv_hx = 1.0 / hx, inv_hy = 1.0 / hy;
+        const double hmin = fmin(hx, hy);
+        // ---- counting sort of b into cells ----
+        for (int c = tid; c < ncell + 2; c += MBLOCK) cell_start[c] = 0;
+        for (int w = tid; w < n_words; w += MBLOCK) mask[w] = 0u;
+        __syncthreads();
+        for (int j = tid; j < n; j += MBLOCK) {
+            const double2 q = bs[j];
+            const int c = cell_coord(q.y, ymin, inv_hy, G) * G + cell_coord(q.x, xmin, inv_hx, G);
+            atomicAdd(&cell_start[c + 1], 1);
+        }
+        __syncthreads();
+        {   // inclusive scan of cell_start[1 .. ncell]: cell_start[c + 1] = points in cells 0 .. c
+            const int chunk = (ncell + MBLOCK - 1) / MBLOCK;
+            const int lo = 1 + tid * chunk, hi = min(ncell + 1, lo + chunk);
+            int sum = 0;
+            for (int c = lo; c < hi; ++c) sum += cell_start[c];
+            int incl = sum;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += t;
+            }
+            if (lane == 31) s_part[warp] = incl;
+            __syncthreads();
+            if (warp == 0) {
+                const int w = s_part[lane];
+                int wi = w;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int t = __shfl_up_sync(0xffffffffu, wi, o);
+                    if (lane >= o) wi += t;
+                }
+                s_part[lane] = wi - w;
+            }
+            __syncthreads();
+            int run = s_part[warp] + incl - sum;
+            for (int c = lo; c < hi; ++c) { run += cell_start[c]; cell_start[c] = run; }
+            if (tid == 0) cell_start[ncell + 1] = n;
+            __syncthreads();
+        }
+        // scatter from the back: every insertion into cell c takes slot --cell_start[c + 1]; afterwards
+        // cell_start[c + 1] is the FIRST slot of cell c and cell_start[c + 2] one past its last
+        for (int j = tid; j < n; j += MBLOCK) {
+            const double2 q = bs[j];
+            const int c = cell_coord(q.y, ymin, inv_hy, G) * G + cell_coord(q.x, xmin, inv_hx, G);
+            sorted[atomicSub(&cell_start[c + 1], 1) - 1] = j;
+        }
+        __syncthreads();
+        // ---- nearest b for every a ----
+        double max_d2 = 0.0;
+        int ok = 1;
+        for (int i = tid; i < n; i += MBLOCK) {
+            const double2 p = as[i];
+            const int cx = cell_coord(p.x, xmin, inv_hx, G), cy = cell_coord(p.y, ymin, inv_hy, G);
+            double best = INFINITY;
+            int bj = -1;
+            int r_done = 0;
+            for (int r = 1; r <= 4; ++r) {
+                for (int yy = cy - r; yy <= cy + r; ++yy) {
+                    if (yy < 0 || yy >= G) continue;
+                    const bool edge_row = abs(yy - cy) == r;
+                    // r = 1: the whole 3-cell row is one contiguous range of `sorted`; r > 1: the whole row on the ring's
+                    // top and bottom, its two end cells otherwise
+                    for (int part = 0; part < 2; ++part) {
+                        int xa, xb;
+                        if (r == 1 || edge_row) { if (part) break; xa = cx - r; xb = cx + r; }
+                        else { xa = xb = part ? cx + r : cx - r; }
+                        xa = max(xa, 0);
+                        xb = min(xb, G - 1);
+                        if (xa > xb) continue;
+                        const int t0 = cell_start[yy * G + xa + 1], t1 = cell_start[yy * G + xb + 2];
+                        for (int t = t0; t < t1; ++t) {
+                            const int j = sorted[t];
+                            const double2 q = bs[j];
+                            const double dx = p.x - q.x, dy = p.y - q.y;
+                            const double d2 = dx * dx + dy * dy;
+                            if (d2 < best || (d2 == best && j < bj)) { best = d2; bj = j; }
+                        }
+                    }
+                }
+                r_done = r;
+                const double reach = r * hmin;
+                if (best <= reach * reach) break;
+                if (cx - r <= 0 && cy - r <= 0 && cx + r >= G - 1 && cy + r >= G - 1) break;  // whole grid seen
+            }
+            const double reach = r_done * hmin;
+            const bool whole = (cx - r_done <= 0 && cy - r_done <= 0 && cx + r_done >= G - 1 && cy + r_done >= G - 1);
+            if (!(best <= reach * reach) && !whole) {   // rare: nothing close, look at everything
+                for (int j = 0; j < n; ++j) {
+                    const double2 q = bs[j];
+                    const double dx = p.x - q.x, dy = p.y - q.y;
+                    const double d2 = dx * dx + dy * dy;
+                    if (d2 < best || (d2 == best && j < bj)) { best = d2; bj = j; }
+                }
+            }
+            max_d2 = fmax(max_d2, best);
+            if (out_index) out_index[s * n + i] = bj;
+            if (bj >= 0) {
+                const unsigned bit = 1u << (bj & 31);
+                if (atomicOr(&mask[bj >> 5], bit) & bit) ok = 0;     // b_j taken twice: not a bijection
+                const double2 q = bs[bj];
+                const double lim = rel_tol * (1.0 + sqrt(q.x * q.x + q.y * q.y));
+                if (!(sqrt(best) <= lim)) ok = 0;
+            } else {
+                ok = 0;
+            }
+        }
+        max_d2 = block_reduce_m(max_d2, true, s_red);
+        const int all_ok = __syncthreads_and(ok);
+        if (tid == 0) { if (out_max_err) out_max_err[s] = sqrt(max_d2); out_bijective[s] = all_ok ? 1 : 0; }
+        __syncthreads();
+    }
+    (void)s_flag;
+}
+
 // ---- completeness certificate: Vieta's first two sums of every row ----
 // P(z; phi) = F(z, phi) prod (z - z_i)^2 has degree 2N and leading coefficient -c(phi); its next two
 // coefficients give  sum_k z_k = 2 sum_i z_i  and  sum_k z_k^2 = 2 sum_i z_i^2 + 2 (sum_i m_i)/c(phi).
@@ -309,8 +489,26 @@ static int match_launch(const double *a, const double *b, int64_t S, int64_t n, 
     if (G < 1) G = 1;
     if (G > 2048) G = 2048;
     const long long ncell = (long long)G * G;
-    const long long stride = (ncell + 1) + ncell + 2 * n;
     const int sms = device_sm_count();
+    // sets whose bins fit shared memory: one 1024-thread CTA per set, everything but the points on chip
+    const size_t smem = ((size_t)ncell + 2 + (size_t)n + (size_t)((n + 31) / 32)) * sizeof(int);
+    int dev = 0, max_optin = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (smem + 2048 <= (size_t)max_optin) {
+        MLCC_CUDA(cudaFuncSetAttribute(k_match_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int per_sm = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_match_smem, MBLOCK, smem) != cudaSuccess || per_sm < 1)
+            per_sm = 1;
+        long long grid = (long long)per_sm * sms;
+        if (grid > S) grid = S;
+        k_match_smem<<<(int)grid, MBLOCK, smem, stream>>>(reinterpret_cast<const double2 *>(a),
+                                                          reinterpret_cast<const double2 *>(b), (long long)S, (int)n,
+                                                          rel_tol, G, out_max_err, out_bijective, b_shift, out_index);
+        MLCC_CUDA(cudaGetLastError());
+        return MLCC_OK;
+    }
+    const long long stride = (ncell + 1) + ncell + 2 * n;
     // latency-bound CTAs (global-memory counting sort and ring search): as many as stay resident
     int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_match, BLOCK, 0) != cudaSuccess || per_sm < 1) per_sm = 2;

@@ -1,6 +1,7 @@
 // mlcc_common.cuh — shared host/device helpers of libmlcc (product path; not used by oracle/).
 #pragma once
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>
 #include <stdint.h>
 #include <stdio.h>
 #include <string>
@@ -100,6 +101,18 @@ struct PinnedBlock {
 };
 
 int device_sm_count();
+
+// NVTX range on the calling host thread (SURVEY.md §5 "Tracing"): every C-ABI entry point opens one named after the
+// call; the solver adds one per phase of its work (set-up, every enqueued chunk of iterations, the final read-back)
+// and a mark whenever a poll of the device state shows that further steps of the continuation have finished.  The
+// iterations themselves run from a device-side state machine, so per-step ranges exist only as those marks.
+// Header-only NVTX 3: no tool attached = a no-op call.
+struct NvtxRange {
+    explicit NvtxRange(const char *name) { nvtxRangePushA(name); }
+    NvtxRange(const NvtxRange &) = delete;
+    NvtxRange &operator=(const NvtxRange &) = delete;
+    ~NvtxRange() { nvtxRangePop(); }
+};
 
 // ---- device arithmetic ------------------------------------------------------------------------
 #ifdef __CUDACC__

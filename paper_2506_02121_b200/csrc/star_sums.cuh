@@ -75,6 +75,47 @@ __device__ __forceinline__ void pair_star(double zx, double zy, double2 s, doubl
     a.s3y = fma(uy, h, a.s3y);
 }
 
+// The same for a field of EQUAL masses m_i = m0 (BASELINE.json configs 1, 2, 5): the sums are accumulated
+// unweighted and scaled once at the end (star_sums_scale), 20 FP64 instructions per pair instead of 24:
+//   S1 += w,  S2/m0 += w^2,  S3/m0 += w^3,  Sm/m0 = S1.
+// Where S1 is not wanted (WITH_S1 = false) but the caustic point is, w is added into the Sm fields instead.
+// With m0 = 1 the results are bit-identical to pair_star (every product by the mass is exact there).
+template <bool CAUS, bool WITH_S1 = true>
+__device__ __forceinline__ void pair_star_eq(double zx, double zy, double2 s, StarAcc &a)
+{
+    const double dx = zx - s.x;
+    const double dy = s.y - zy;
+    const double r2 = fma(dy, dy, dx * dx);
+    const double inv = rcp_full(r2);
+    const double wx = dx * inv;
+    const double wy = dy * inv;
+    if (WITH_S1) {
+        a.s1x += wx;
+        a.s1y += wy;
+    } else if (CAUS) {
+        a.smx += wx;
+        a.smy += wy;
+    }
+    const double A = wx * wx;
+    const double B = wy * wy;
+    const double g = fma(-3.0, B, A);
+    const double h = fma(3.0, A, -B);
+    a.s2x += A - B;
+    a.s2h = fma(wx, wy, a.s2h);
+    a.s3x = fma(wx, g, a.s3x);
+    a.s3y = fma(wy, h, a.s3y);
+}
+template <bool CAUS, bool WITH_S1 = true>
+__device__ __forceinline__ void star_sums_scale(StarAcc &a, double m0)
+{
+    if (CAUS) {
+        a.smx = m0 * (WITH_S1 ? a.s1x : a.smx);
+        a.smy = m0 * (WITH_S1 ? a.s1y : a.smy);
+    }
+    a.s2x *= m0; a.s2h *= m0;
+    a.s3x *= m0; a.s3y *= m0;
+}
+
 // P(u) = sum_l a[l] u^l with its first two derivatives by one Horner pass (synthetic division):
 // returns P, P', P''/2.
 __device__ __forceinline__ void horner3(const double2 *__restrict__ a, int n, double ux, double uy,

@@ -47,7 +47,7 @@ def test_options_default_and_struct_layout(lib):
     o = api.options()
     assert o.struct_size == C.sizeof(api.mlcc_options) == 88
     assert o.predictor_order == -1 and o.num_subchains == 0 and o.phi_index_total == 0
-    assert C.sizeof(api.mlcc_stats) == 64
+    assert C.sizeof(api.mlcc_stats) == 72
 
 
 @pytest.mark.parametrize("N,num_phi,req", [(10, 1000, 0), (200, 4000, 0), (2000, 5000, 0), (10000, 10000, 0),

@@ -91,17 +91,25 @@ def test_star_field_seed_and_defaults(api, orc):
 # ---------------------------------------------------------------------------------------------
 # a1-a6 critical curves, a7 caustics: full grids where the oracle finishes in seconds
 # ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("regime", [1, 2])
 @pytest.mark.parametrize("name", ["cfg1", "cfg2"])
-def test_curves_and_caustics_full_grid(api, orc, name):
+def test_curves_and_caustics_full_grid(api, orc, name, regime):
+    """Full grids of cfg1 / cfg2 against the oracle, in both kernel regimes (1 = tiled launches, 2 = one CTA per
+    sub-chain: mlcc_options.regime)."""
     cfg = CONFIGS[name]
     xy, m, R = field(orc, cfg)
     ref, it_ref, un_ref = orc.critical_curves(xy, m, cfg.kappa_s, cfg.gamma, cfg.num_phi, cfg.tol, cfg.max_iter)
     assert un_ref.sum() == 0
     roots, iters, unconv, stats = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, cfg.num_phi,
-                                                         cfg.tol, cfg.max_iter)
+                                                         cfg.tol, cfg.max_iter, opt=api.options(regime=regime))
+    assert stats.regime == regime
     assert int(unconv.sum()) == 0 and stats.unconverged_rows == 0 and stats.degenerate_roots == 0
     assert int(iters.min()) >= 1 and int(iters.max()) <= cfg.max_iter
     assert stats.root_iterations >= cfg.num_phi * 2 * cfg.N
+    again, _, _, _ = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, cfg.num_phi, cfg.tol, cfg.max_iter,
+                                            opt=api.options(regime=regime))
+    assert torch.equal(again, roots)                      # fixed summation order: two runs give the same bits
+    certify_every_row(api, dev(xy), dev(m), cfg, roots)
     g = roots.cpu().numpy()
     assert_rows_match(orc, g, ref)
     # caustics: GPU roots -> GPU caustics, oracle roots -> oracle caustics, compared through the matching
@@ -114,7 +122,10 @@ def test_curves_and_caustics_full_grid(api, orc, name):
     assert np.abs(w_same - w_ref).max() <= 1e-12 * (1 + np.abs(w_ref).max())
     # default-options entry point on the default stream
     r2 = api.critical_curves(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, cfg.num_phi, cfg.tol, cfg.max_iter)
-    assert torch.equal(r2, roots)
+    if regime == 2:                                       # the regime AUTO picks for these fields
+        assert torch.equal(r2, roots)
+    else:
+        assert_rows_match(orc, r2.cpu().numpy(), ref)
 
 
 # ---------------------------------------------------------------------------------------------
@@ -327,6 +338,73 @@ def test_bench_configuration_full_size_cfg4(api, orc):
 
 
 # ---------------------------------------------------------------------------------------------
+# the chain regime (one CTA per sub-chain, chain.cu): sizes that exercise every pass shape and edge
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N,num_phi,nsub", [(1, 1, 0), (1, 7, 0), (2, 33, 2), (3, 64, 0), (17, 101, 5), (64, 40, 0),
+                                            (129, 96, 3), (300, 50, 0), (640, 24, 0), (1200, 12, 2)])
+def test_chain_regime_sizes_and_edges(api, orc, N, num_phi, nsub):
+    """Fields from one star (two roots, fewer roots than lanes: T-lane passes) to the largest that fits shared memory
+    (N = 1200), grids that do not divide into the sub-chains, one-row sub-chains: root sets and fused caustic points
+    against the oracle, diagnostics, and the tiled regime on the same input."""
+    cfg = CONFIGS["cfg2"]
+    xy, m, R = orc.star_field(11, N, cfg.kappa_star, 1, (0.08, 1.0, 2.35))
+    if N == 1:
+        xy = xy + np.array([[0.37, -0.21]])            # keep the single star (and its seeds) off the real axis
+    dxy, dm = dev(xy), dev(m)
+    opt = api.options(regime=2, num_subchains=nsub)
+    roots, caus, iters, unconv, st = api.curves_and_caustics(dxy, dm, cfg.kappa_s, cfg.gamma, num_phi, cfg.tol, cfg.max_iter,
+                                                             opt=opt)
+    assert st.regime == 2 and st.kernel_launches == 2 and st.unconverged_rows == 0 and st.degenerate_roots == 0
+    assert int(unconv.sum()) == 0 and int(iters.min()) >= 1
+    assert st.root_iterations >= num_phi * 2 * N and st.star_pairs == st.root_iterations * N
+    if N <= 300:
+        ref, _, un = orc.critical_curves(xy, m, cfg.kappa_s, cfg.gamma, num_phi, cfg.tol, cfg.max_iter)
+    else:
+        ref = np.concatenate([orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, num_phi, [j], cfg.tol, cfg.max_iter)[0]
+                              for j in range(num_phi)])
+    assert_rows_match(orc, roots.cpu().numpy(), ref)
+    w_ref = orc.caustics(xy, m, cfg.kappa_s, cfg.gamma, ref)
+    g, w = roots.cpu().numpy(), caus.cpu().numpy()
+    for j in range(num_phi):
+        assert_caustics_match(g[j], w[j], ref[j], w_ref[j])
+    c2 = api.caustics(dxy, dm, cfg.kappa_s, cfg.gamma, roots)
+    assert float((caus - c2).abs().max()) <= 1e-11
+    tiled, _, _, st1 = api.critical_curves_ex(dxy, dm, cfg.kappa_s, cfg.gamma, num_phi, cfg.tol, cfg.max_iter,
+                                              opt=api.options(regime=1, num_subchains=nsub))
+    assert st1.regime == 1
+    err, bij = api.match_root_sets(roots, tiled, 1e-10)
+    assert bool(bij.all())
+
+
+def test_chain_regime_limits_and_reports(api, orc):
+    """What the chain regime refuses (fields beyond shared memory, far-field sums, a sheet polynomial, the FP32 Aberth
+    sum when forced), what AUTO then does, and its max_iter / NaN reports."""
+    cfg = CONFIGS["cfg2"]
+    xy, m, R = field(orc, cfg)
+    dxy, dm = dev(xy), dev(m)
+    for bad in (dict(star_sum_mode=api.MLCC_STAR_SUMS_FMM), dict(trust_predictor=1), dict(aberth_sum_precision=32)):
+        with pytest.raises(api.MlccError):
+            api.critical_curves_ex(dxy, dm, cfg.kappa_s, cfg.gamma, 16, opt=api.options(regime=2, **bad))
+        _, _, _, st = api.critical_curves_ex(dxy, dm, cfg.kappa_s, cfg.gamma, 16, opt=api.options(**bad))
+        assert st.regime == 1                                       # AUTO falls back to the tiled regime
+    big = CONFIGS["cfg3"]
+    bxy, bm, _ = field(orc, big)
+    with pytest.raises(api.MlccError):
+        api.critical_curves_ex(dev(bxy), dev(bm), big.kappa_s, big.gamma, 4, opt=api.options(regime=2))
+    # max_iter: unconverged roots are counted per row, everything is written, the status says so
+    r, it, un, st = api.critical_curves_ex(dxy, dm, cfg.kappa_s, cfg.gamma, 40, cfg.tol, 2, opt=api.options(regime=2),
+                                           strict=False)
+    assert st.status == api.MLCC_ERR_NOT_CONVERGED and st.unconverged_rows > 0 and int(un.max()) > 0
+    assert int(it.max()) == 2 and bool(torch.isfinite(r).all())
+    assert st.unconverged_rows == int((un > 0).sum())
+    # an initial guess that sits on a star gives a NaN step: frozen and reported, nothing hangs
+    init = torch.cat([dxy, dxy]).contiguous()
+    r, it, un, st = api.critical_curves_ex(dxy, dm, cfg.kappa_s, cfg.gamma, 8, cfg.tol, cfg.max_iter,
+                                           opt=api.options(regime=2), init_roots=init, strict=False)
+    assert st.status == api.MLCC_ERR_DEGENERATE and st.degenerate_roots > 0
+
+
+# ---------------------------------------------------------------------------------------------
 # options do not change the answer (the iteration path is not part of the contract)
 # ---------------------------------------------------------------------------------------------
 def test_options_do_not_change_the_root_sets(api, orc):
@@ -336,15 +414,18 @@ def test_options_do_not_change_the_root_sets(api, orc):
     ref, _, _ = orc.critical_curves(xy, m, cfg.kappa_s, cfg.gamma, num_phi)
     dxy, dm = dev(xy), dev(m)
     seen_iters = {}
-    for order in range(0, 6):
-        for nsub in (1, 3, 16):
-            r, it, un, st = api.critical_curves_ex(dxy, dm, cfg.kappa_s, cfg.gamma, num_phi,
-                                                   opt=api.options(num_subchains=nsub, predictor_order=order))
-            assert st.subchains == nsub and st.predictor_order == order and int(un.sum()) == 0
-            assert_rows_match(orc, r.cpu().numpy(), ref)
-            seen_iters[(order, nsub)] = st.root_iterations
-    # the predictor only removes work
-    assert seen_iters[(3, 1)] < seen_iters[(0, 1)]
+    for regime in (1, 2):
+        for order in range(0, 6):
+            for nsub in (1, 3, 16):
+                r, it, un, st = api.critical_curves_ex(dxy, dm, cfg.kappa_s, cfg.gamma, num_phi,
+                                                       opt=api.options(num_subchains=nsub, predictor_order=order,
+                                                                       regime=regime))
+                assert st.subchains == nsub and st.predictor_order == order and int(un.sum()) == 0
+                assert st.regime == regime
+                assert_rows_match(orc, r.cpu().numpy(), ref)
+                seen_iters[(regime, order, nsub)] = st.root_iterations
+        # the predictor only removes work
+        assert seen_iters[(regime, 3, 1)] < seen_iters[(regime, 0, 1)]
     for T in (1, 2, 4, 8, 16, 32, 64, 128):
         for prec in (32, 64):
             r, it, un, st = api.critical_curves_ex(dxy, dm, cfg.kappa_s, cfg.gamma, num_phi,
@@ -366,8 +447,8 @@ def test_aberth_sum_precision_changes_the_path_not_the_roots(api, orc, name, num
     out = {}
     for prec in (32, 64):
         r, it, unc, st = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, num_phi, cfg.tol,
-                                                cfg.max_iter, opt=api.options(aberth_sum_precision=prec))
-        assert int(unc.sum()) == 0 and st.aberth_sum_precision == prec
+                                                cfg.max_iter, opt=api.options(aberth_sum_precision=prec, regime=1))
+        assert int(unc.sum()) == 0 and st.aberth_sum_precision == prec and st.regime == 1
         assert_rows_match(orc, r.cpu().numpy(), ref)
         out[prec] = (r, st)
     # the two paths agree with each other far inside the tolerance, and cost about the same work
@@ -919,7 +1000,7 @@ def test_trust_predictor_starts_rows_with_newton_steps(api, orc, name, num_phi):
     a, _, _, sa = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, min(num_phi, 200), cfg.tol, cfg.max_iter,
                                          opt=api.options(predictor_order=0, trust_predictor=1))
     b, _, _, sb = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, min(num_phi, 200), cfg.tol, cfg.max_iter,
-                                         opt=api.options(predictor_order=0, skip_aberth_sum_below=1e-8))
+                                         opt=api.options(predictor_order=0, skip_aberth_sum_below=1e-8, regime=1))
     assert torch.equal(a, b) and sa.root_pairs == sb.root_pairs
     with pytest.raises(api.MlccError):
         api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, 8, opt=api.options(trust_predictor=2))
