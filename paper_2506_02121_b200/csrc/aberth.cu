@@ -562,7 +562,12 @@ __global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Para
         const int slot = lo;
         const long long row = p.slot_row[slot];
         const float4 *slot_src = p.src + (size_t)slot * n_src;
-        if (STAGES && tid == 0) {   // first stage of this tile
+        // Tiles whose roots are spread over the WHOLE CTA (T = CTA: the straggler iterations of a step, a handful of
+        // unfrozen roots) read their sources straight from global memory (L2): every thread has only N_pad / CTA
+        // sources, so the staged pipeline would be a chain of n_stage copy latencies (43 us per launch at N = 10^4)
+        // with nothing to overlap them; independent loads take a few microseconds.
+        const bool direct = STAGES && T == CTA;
+        if (STAGES && !direct && tid == 0) {   // first stage of this tile
             const unsigned b = g & 1u;
             mbar_expect_tx(&s_full[b], STAGE_TX);
             if (STARS) {
@@ -602,7 +607,7 @@ __global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Para
             fx[r] = fy[r] = make_float2(0.f, 0.f);
         }
 
-        for (int t = 0; t < n_stage; ++t, ++g) {
+        for (int t = 0; t < (direct ? 0 : n_stage); ++t, ++g) {
             const unsigned b = g & 1u;
             if (tid == 0 && t + 1 < n_stage) {   // prefetch: buffer b^1 was last read in stage g-1, closed by a barrier
                 const unsigned nb = b ^ 1u;
@@ -664,6 +669,53 @@ __global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Para
                 }
             }
             __syncthreads();   // everyone is done with buffer b before it is refilled
+        }
+        if (direct && valid) {
+            // thread `tid` takes the sources tid, tid + CTA, ... (star j with the root entries 2j, 2j + 1, as a stage
+            // pairs them); N_pad is a multiple of 2 CTA
+#pragma unroll 2
+            for (int j0 = tid; j0 < p.N_pad; j0 += 2 * CTA) {
+                double2 sxy[2];
+                double sm[2];
+                float4 e0[2], e1[2];
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    const int j = j0 + u * CTA;
+                    sxy[u] = make_double2(0.0, 0.0);
+                    sm[u] = 0.0;
+                    e0[u] = e1[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (STARS) {
+                        sxy[u] = __ldg(&p.stars_pad[j]);
+                        if (!EQM) sm[u] = __ldg(&p.mass_pad[j]);
+                    }
+                    if (ROOTS) {
+                        e0[u] = __ldg(&slot_src[2 * j]);
+                        e1[u] = __ldg(&slot_src[2 * j + 1]);
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        if (STARS) {
+                            if (EQM) pair_star_eq<CAUS, ROOTS>(zx[r], zy[r], sxy[u], acc[r]);
+                            else pair_star<CAUS, ROOTS>(zx[r], zy[r], sxy[u], sm[u], acc[r]);
+                        }
+                        if (ROOTS && MODE == MODE_F64) {
+                            const double2 ra = make_double2(__hiloint2double(__float_as_int(e0[u].y), __float_as_int(e0[u].x)),
+                                                            __hiloint2double(__float_as_int(e0[u].w), __float_as_int(e0[u].z)));
+                            const double2 rb = make_double2(__hiloint2double(__float_as_int(e1[u].y), __float_as_int(e1[u].x)),
+                                                            __hiloint2double(__float_as_int(e1[u].w), __float_as_int(e1[u].z)));
+                            pair_root_f64(zx[r], zy[r], ra, ax[r], ay[r]);
+                            pair_root_f64(zx[r], zy[r], rb, bx[r], by[r]);
+                        } else if (ROOTS) {
+                            pair_root2_f32(make_float2(zxh[r], zxh[r]), make_float2(zyh[r], zyh[r]),
+                                           make_float2(zxl[r], zxl[r]), make_float2(zyl[r], zyl[r]), e0[u], e1[u],
+                                           fx[r], fy[r]);
+                        }
+                    }
+                }
+            }
         }
         // ---- this thread's partial sums: v = (2 S1 - A, S2, S3, Sm), or (-A) alone without STARS ----
         double v[R][NV];

@@ -376,6 +376,27 @@ def test_chain_regime_sizes_and_edges(api, orc, N, num_phi, nsub):
     assert bool(bij.all())
 
 
+@pytest.mark.parametrize("regime,N,num_phi", [(1, 300, 24), (2, 300, 24), (1, 2500, 6)])
+def test_equal_mass_fields_take_the_lighter_pair_body(api, orc, regime, N, num_phi):
+    """A field whose stars all have the mass m0 runs the equal-mass pair body (unweighted sums scaled by m0 at the end,
+    star_sums.cuh).  m0 = 2.5 (not 1, so the scaling is not the identity), both regimes, roots and fused caustic points
+    against the oracle; one star made heavier switches back to the general body with the same contract."""
+    cfg = CONFIGS["cfg2"]
+    xy, _, R = orc.star_field(3, N, cfg.kappa_star, 0, None)
+    for m in (np.full(N, 2.5), np.concatenate([np.full(N - 1, 2.5), [2.75]])):
+        roots, caus, it, un, st = api.curves_and_caustics(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, num_phi, cfg.tol,
+                                                          cfg.max_iter, opt=api.options(regime=regime))
+        assert st.regime == regime and int(un.sum()) == 0
+        ref = np.concatenate([orc.critical_curve_rows(xy, m, cfg.kappa_s, cfg.gamma, num_phi, [j], cfg.tol, cfg.max_iter)[0]
+                              for j in range(num_phi)])
+        assert_rows_match(orc, roots.cpu().numpy(), ref)
+        w_ref = orc.caustics(xy, m, cfg.kappa_s, cfg.gamma, ref)
+        g, w = roots.cpu().numpy(), caus.cpu().numpy()
+        for j in range(num_phi):
+            assert_caustics_match(g[j], w[j], ref[j], w_ref[j])
+        certify_every_row(api, dev(xy), dev(m), cfg, roots)
+
+
 def test_chain_regime_limits_and_reports(api, orc):
     """What the chain regime refuses (fields beyond shared memory, far-field sums, a sheet polynomial, the FP32 Aberth
     sum when forced), what AUTO then does, and its max_iter / NaN reports."""
