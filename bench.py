@@ -143,6 +143,23 @@ class ClockSampler:
                 pass
             time.sleep(self.period_ms / 1000.0)
 
+    def sample_now(self):
+        """One synchronous sample (used at both ends of a timed region, so that regions shorter than the sampling
+        period still carry the clocks they ran at)."""
+        if self.proc != "nvml":
+            return
+        nv, h = self.nvml, self.handle
+        try:
+            row = [str(self.gpu), str(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)), str(self.smax),
+                   str(nv.nvmlDeviceGetPowerUsage(h) / 1000.0), "", "", "", "", ""]
+            mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+            for bit, col in ((nv.nvmlClocksThrottleReasonHwSlowdown, 5), (nv.nvmlClocksThrottleReasonHwThermalSlowdown, 6),
+                             (nv.nvmlClocksThrottleReasonSwThermalSlowdown, 7), (nv.nvmlClocksThrottleReasonSwPowerCap, 8)):
+                row[col] = "Active" if (mask & bit) else "Not Active"
+            self.rows.append((time.time(), row))
+        except Exception:
+            pass
+
     def _read(self):
         for line in self.proc.stdout:
             self.rows.append((time.time(), [c.strip() for c in line.split(",")]))
@@ -370,7 +387,9 @@ def time_workload(api, torch, dist, world, sampler, cfg, num_phi, opt, phi_off, 
     barrier()
     t_begin = time.time()
     ev0.record()
-    for _ in range(steps):
+    for i_step in range(steps):
+        if sampler is not None and i_step == steps - 1:
+            sampler.sample_now()          # launches of the earlier steps are still running: a sample under load
         st = wb.step()
         f = flop_model(cfg, st, star_sums, st.aberth_sum_precision)
         acc["solve_ms"] += st.solve_ms
@@ -379,6 +398,8 @@ def time_workload(api, torch, dist, world, sampler, cfg, num_phi, opt, phi_off, 
         for k in ("fp64", "fp32", "hw_fp64", "survey"):
             acc[k] += f[k]
     ev1.record()
+    if sampler is not None:
+        sampler.sample_now()              # the device is still working through the last step's launches
     barrier()
     t_end = time.time()
     ms = ev0.elapsed_time(ev1)
@@ -392,7 +413,7 @@ def time_workload(api, torch, dist, world, sampler, cfg, num_phi, opt, phi_off, 
     return wb, acc
 
 
-def roofline_of(acc, peak64, peak32, mode):
+def roofline_of(acc, peak64, peak32, mode, survey_ok=True):
     s = acc["solve_ms"] * 1e-3
     if s <= 0:
         return {}
@@ -402,7 +423,7 @@ def roofline_of(acc, peak64, peak32, mode):
             "fp32_algorithmic_tflops": f32, "fp32_frac": (f32 / peak32 if peak32 else None) if mode == 32 else 0.0,
             "combined_frac": ((f64 / peak64 if peak64 else 0.0) + (f32 / peak32 if (peak32 and mode == 32) else 0.0)),
             "hw_fp64_frac_model": acc["hw_fp64"] / s / 1e12 / peak64 if peak64 else None,
-            "frac_with_survey_accounting": acc["survey"] / s / 1e12 / peak64 if (peak64 and mode != 32) else None}
+            "frac_with_survey_accounting": acc["survey"] / s / 1e12 / peak64 if (peak64 and mode != 32 and survey_ok) else None}
 
 
 def ncu_capture_summary():
@@ -513,7 +534,7 @@ def main():
     sm_count = props.multi_processor_count
     sm_max_mhz = (acc["clocks"] or {}).get("sm_max_mhz") or 1965.0
     nominal64 = sm_count * 64 * 2 * sm_max_mhz * 1e6 / 1e12     # SMs x FP64 lanes x 2 flop x max SM clock
-    rf = roofline_of(acc, peak64, peak32, mode)
+    rf = roofline_of(acc, peak64, peak32, mode, survey_ok=(args.star_sums == "direct" and not args.trust_predictor))
     ncu = ncu_capture_summary() if (args.workload == "cfg4" and args.star_sums == "direct") else None
     kernel = "mlcc::k_chain (chain regime)" if st.regime == api.MLCC_REGIME_CHAIN else "mlcc::k_compute (Aberth iteration, tiled regime)"
     roofline = {"bound": "alu", "kernel": kernel,
@@ -615,7 +636,8 @@ def main():
                    "root_iterations_per_root": st2.root_iterations / float(num_phi * n_r),
                    "root_iterations_with_aberth_sum_per_root": st2.root_pairs / float(n_r - 1) / float(num_phi * n_r),
                    "unconverged_rows": st2.unconverged_rows, "clocks": acc2["clocks"]}
-            out.update(roofline_of(acc2, peak64, peak32, st2.aberth_sum_precision))
+            out.update(roofline_of(acc2, peak64, peak32, st2.aberth_sum_precision,
+                                   survey_ok=(star_sums == "direct" and not kw.get("trust_predictor"))))
             del wb2
             torch.cuda.empty_cache()
             return out

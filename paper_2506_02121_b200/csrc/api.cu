@@ -337,26 +337,29 @@ int mlcc_curves_and_caustics_host(const double *star_xy, const double *masses, i
     if (N < 1 || N > (1 << 28)) return invalid("N out of range");
     if (num_phi < 1) return invalid("num_phi < 1");
     const size_t n_pts = (size_t)num_phi * (size_t)mlcc_num_roots(N, (opt && opt->sheet_poly) ? opt->sheet_poly_n : 0);
-    DeviceBuffer d_xy, d_m, d_roots, d_caus;
-    MLCC_CUDA(d_xy.alloc(sizeof(double) * 2 * (size_t)N));
-    MLCC_CUDA(d_m.alloc(sizeof(double) * (size_t)N));
-    MLCC_CUDA(d_roots.alloc(sizeof(double) * 2 * n_pts));
-    if (out_caustics) MLCC_CUDA(d_caus.alloc(sizeof(double) * 2 * n_pts));
-    MLCC_CUDA(cudaMemcpyAsync(d_xy.p, star_xy, sizeof(double) * 2 * (size_t)N, cudaMemcpyHostToDevice, 0));
-    MLCC_CUDA(cudaMemcpyAsync(d_m.p, masses, sizeof(double) * (size_t)N, cudaMemcpyHostToDevice, 0));
+    // device copies from the stream-ordered pool (kept cached between calls: mlcc_common.cuh keep_pool_memory; a
+    // cudaMalloc / cudaFree pair of 6.4 GB per call cost 0.2-0.3 s at cfg4)
+    Workspace hws(nullptr);
+    double *d_xy = nullptr, *d_m = nullptr, *d_roots = nullptr, *d_caus = nullptr;
+    MLCC_CUDA(hws.alloc(&d_xy, 2 * (size_t)N));
+    MLCC_CUDA(hws.alloc(&d_m, (size_t)N));
+    MLCC_CUDA(hws.alloc(&d_roots, 2 * n_pts));
+    if (out_caustics) MLCC_CUDA(hws.alloc(&d_caus, 2 * n_pts));
+    MLCC_CUDA(cudaMemcpyAsync(d_xy, star_xy, sizeof(double) * 2 * (size_t)N, cudaMemcpyHostToDevice, 0));
+    MLCC_CUDA(cudaMemcpyAsync(d_m, masses, sizeof(double) * (size_t)N, cudaMemcpyHostToDevice, 0));
     // Pinned (or registered) host outputs receive the finished rows while the solve runs; pageable ones would make
     // every copy block the host thread that feeds the launches, so they are copied once, at the end.
     const bool overlap = host_is_pinned(out_roots) && (!out_caustics || host_is_pinned(out_caustics));
-    const int rc = critical_curves_impl(d_xy.as<double>(), d_m.as<double>(), N, kappa_s, gamma, num_phi, tol,
-                                        max_iter, d_roots.as<double>(), out_caustics ? d_caus.as<double>() : nullptr,
+    const int rc = critical_curves_impl(d_xy, d_m, N, kappa_s, gamma, num_phi, tol,
+                                        max_iter, d_roots, out_caustics ? d_caus : nullptr,
                                         opt, nullptr, nullptr, nullptr, out_stats, nullptr,
                                         overlap ? out_roots : nullptr, overlap ? out_caustics : nullptr);
     if (rc != MLCC_OK && rc != MLCC_ERR_NOT_CONVERGED && rc != MLCC_ERR_DEGENERATE) return rc;
     const std::string keep = g_last_error;
     if (!overlap) {
-        MLCC_CUDA(cudaMemcpyAsync(out_roots, d_roots.p, sizeof(double) * 2 * n_pts, cudaMemcpyDeviceToHost, 0));
+        MLCC_CUDA(cudaMemcpyAsync(out_roots, d_roots, sizeof(double) * 2 * n_pts, cudaMemcpyDeviceToHost, 0));
         if (out_caustics)
-            MLCC_CUDA(cudaMemcpyAsync(out_caustics, d_caus.p, sizeof(double) * 2 * n_pts, cudaMemcpyDeviceToHost, 0));
+            MLCC_CUDA(cudaMemcpyAsync(out_caustics, d_caus, sizeof(double) * 2 * n_pts, cudaMemcpyDeviceToHost, 0));
     }
     MLCC_CUDA(cudaStreamSynchronize(0));
     if (rc != MLCC_OK) g_last_error = keep;

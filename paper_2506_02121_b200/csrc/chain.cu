@@ -29,6 +29,9 @@
 namespace mlcc {
 namespace {
 
+#ifndef MLCC_CHAIN_MIN_CTAS
+#define MLCC_CHAIN_MIN_CTAS 2
+#endif
 constexpr int CR = 2;                 // list entries per thread
 constexpr int MAX_ORDER = 5;
 constexpr double TINY = 1e-300;       // |d|^2 + TINY: the pair of a root with itself contributes exactly 0
@@ -215,7 +218,7 @@ __device__ __forceinline__ void chain_pass(const ChainParams &p, double m0, int 
 }
 
 template <bool CAUS>
-__global__ void __launch_bounds__(256, 2) k_chain(ChainParams p)
+__global__ void __launch_bounds__(256, MLCC_CHAIN_MIN_CTAS) k_chain(ChainParams p)
 {
     extern __shared__ __align__(16) unsigned char s_raw[];
     __shared__ unsigned long long s_buf[33];
@@ -300,24 +303,29 @@ __global__ void __launch_bounds__(256, 2) k_chain(ChainParams p)
             // entry over the T lanes of its group.  Full passes use RR = 2, T = 1 (each shared-memory read of a source
             // serves two roots); what is left is cut so that no thread idles through a whole pass: one entry per
             // thread, then the remainder spread over T lanes per entry. ----
-            for (int base = 0; base < n_act;) {
-                const int left = n_act - base;
-                int rr = 2, T = 1;
-                if (4 * left >= 7 * NT) {                       // >= 1.75 NT entries: a full (or nearly full) pass
-                } else if (left > NT) {                         // one entry per thread
-                    rr = 1;
-                } else {                                        // the rest: T lanes per entry
-                    T = 2;
-                    while (T < 32 && left * (2 * T) <= NT * 2) T <<= 1;
+            // The entries that keep the Aberth sum and those that do not cost different amounts per entry, so the two
+            // groups get passes of their own: inside a pass every thread then does the same work.
+            for (int seg = 0; seg < 2; ++seg) {
+                const int seg_end = seg == 0 ? n_large : n_act;
+                for (int base = seg == 0 ? 0 : n_large; base < seg_end;) {
+                    const int left = seg_end - base;
+                    int rr = 2, T = 1;
+                    if (4 * left >= 7 * NT) {                       // >= 1.75 NT entries: a full (or nearly full) pass
+                    } else if (left > NT) {                         // one entry per thread
+                        rr = 1;
+                    } else {                                        // the rest: T lanes per entry
+                        T = 2;
+                        while (T < 32 && left * (2 * T) <= NT * 2) T <<= 1;
+                    }
+                    if (eqm) {
+                        if (rr == 2) chain_pass<CAUS, 2, true>(p, m0, base, T, seg_end, n_large, list, s_xy, s_m, s_z, s_delta, row_s);
+                        else chain_pass<CAUS, 1, true>(p, m0, base, T, seg_end, n_large, list, s_xy, s_m, s_z, s_delta, row_s);
+                    } else {
+                        if (rr == 2) chain_pass<CAUS, 2, false>(p, m0, base, T, seg_end, n_large, list, s_xy, s_m, s_z, s_delta, row_s);
+                        else chain_pass<CAUS, 1, false>(p, m0, base, T, seg_end, n_large, list, s_xy, s_m, s_z, s_delta, row_s);
+                    }
+                    base += rr * NT / T;
                 }
-                if (eqm) {
-                    if (rr == 2) chain_pass<CAUS, 2, true>(p, m0, base, T, n_act, n_large, list, s_xy, s_m, s_z, s_delta, row_s);
-                    else chain_pass<CAUS, 1, true>(p, m0, base, T, n_act, n_large, list, s_xy, s_m, s_z, s_delta, row_s);
-                } else {
-                    if (rr == 2) chain_pass<CAUS, 2, false>(p, m0, base, T, n_act, n_large, list, s_xy, s_m, s_z, s_delta, row_s);
-                    else chain_pass<CAUS, 1, false>(p, m0, base, T, n_act, n_large, list, s_xy, s_m, s_z, s_delta, row_s);
-                }
-                base += rr * NT / T;
             }
             __syncthreads();
             // ---- apply the steps, freeze, compact in order: survivors with the Aberth sum first, then the others ----
