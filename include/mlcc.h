@@ -72,7 +72,7 @@ enum { MLCC_STAR_SUMS_DIRECT = 0, MLCC_STAR_SUMS_FMM = 1 };
  *        sources through shared memory (any N; the path for N >~ 10^3).
  * CHAIN: one CTA owns a sub-chain and runs all its rows and iterations out of shared memory, one launch per call
  *        (fields of up to about 1200 stars; direct star sums, disc fields, FP64 Aberth sum, no trust_predictor).
- * AUTO:  CHAIN where it applies and n_r <= 2400, else TILED.  The root sets are the same within the parity
+ * AUTO:  CHAIN where it applies and n_r <= 2000, else TILED.  The root sets are the same within the parity
  *        tolerance; the bits differ (other summation order).                                              */
 enum { MLCC_REGIME_AUTO = 0, MLCC_REGIME_TILED = 1, MLCC_REGIME_CHAIN = 2 };
 
@@ -82,9 +82,11 @@ typedef struct mlcc_options {
     int32_t num_subchains;    /* sub-chains grown concurrently from their centre rows outwards
                                  (PAPER.md:211-213); 0 = chosen from N and num_phi                  */
     int32_t predictor_order;  /* seeds of a new row: 0 = the previous row's roots;
-                                 p >= 1 = polynomial extrapolation through the last p+1 rows of the
-                                 chain (result-preserving: only the starting guess changes); max 5;
-                                 -1 = library default                                               */
+                                 p >= 1 = polynomial extrapolation through up to p+1 rows of the chain, the
+                                 order chosen root by root: terms are added only while they still fall by a
+                                 factor two from one order to the next, so a rough or noisy history falls
+                                 back towards the previous row's root (result-preserving: only the starting
+                                 guess changes); max 8; -1 = library default (8)                     */
     int32_t max_iter_cold;    /* iteration cap of the cold-started centre rows; 0 = max_iter        */
     int64_t phi_index_offset; /* row j has phase phi = 2 pi (j + phi_index_offset) / phi_index_total */
     int64_t phi_index_total;  /* 0 = num_phi (the half-open grid over [0, 2 pi))                     */

@@ -35,6 +35,7 @@
 //   * Jacobi: updates go to a side buffer and are applied by `apply`, which also refreshes the
 //     per-slot source copy of the row and compacts the list of unfrozen roots in order.
 #include "star_sums.cuh"
+#include "predictor.cuh"
 
 #include <math.h>
 #include <stdlib.h>
@@ -61,7 +62,7 @@ namespace {
 
 // Fields of up to this many roots per phase go to the chain regime when they fit it (mlcc_options.regime = AUTO);
 // measured crossover: DESIGN.md "Kernel regimes".
-constexpr int CHAIN_AUTO_MAX_ROOTS = 2400;
+constexpr int CHAIN_AUTO_MAX_ROOTS = 2000;
 
 constexpr int CTA = 128;          // threads per CTA of the compute kernel
 #ifndef MLCC_ROOTS_PER_THREAD
@@ -79,13 +80,12 @@ constexpr int R_ROOTS_F64 = 4;
 constexpr int S_TILE = 256;       // stars per stage; a stage also holds the 2*S_TILE roots paired with them
 constexpr int STAGE_BYTES = S_TILE * 16 + S_TILE * 8 + 2 * S_TILE * 16;
 constexpr int BLOCK = 256;        // threads per CTA of the small kernels
-constexpr int MAX_ORDER = 5;      // highest predictor order
-// Library defaults of the predictor order (mlcc_options.predictor_order = -1), by measurement (R18): the
-// higher the order, the more roots are within tol of their seed and freeze in the first iteration (cfg4: 79 % at
-// order 3, 96 % at order 4, 98 % at order 5), but the extrapolation weights (sum |c_q| = 15, 31, 63) also amplify the
-// rounding of the stored rows, which leaves more stragglers iterations behind in the large fields.
-constexpr int DEFAULT_ORDER_TILED = 4;
-constexpr int DEFAULT_ORDER_CHAIN = 5;
+constexpr int MAX_ORDER = PRED_MAX_ORDER;      // highest predictor order
+// Library default of the predictor's HIGHEST order (mlcc_options.predictor_order = -1); the order actually used is
+// chosen root by root (predictor.cuh), so a high cap costs nothing where the history is rough or noisy.  Measured
+// (R18): cfg4 5.47 / 5.01 / 4.94 / 4.92 s per set at caps 3 / 4 / 5 / 8, cfg5 25.1 / 22.4 / 21.7 s at 4 / 5 / 8.
+constexpr int DEFAULT_ORDER_TILED = PRED_MAX_ORDER;
+constexpr int DEFAULT_ORDER_CHAIN = PRED_MAX_ORDER;
 constexpr int MAX_SLOTS = 1024;   // most slots in one step (2 per sub-chain)
 constexpr double TINY = 1e-300;   // added to |d|^2 (FP64 root pairs): makes the self pair finite
 constexpr float TINYF = 1e-30f;   // same for the FP32 root pairs
@@ -327,9 +327,6 @@ __global__ void k_prepare(Params p)
 // ------------------------------------------------------------------------------------------------
 // seed kernel: starting values of every slot's new row + identity active lists
 // ------------------------------------------------------------------------------------------------
-__constant__ double c_coef[MAX_ORDER + 1][MAX_ORDER + 1] = {
-    {1, 0, 0, 0, 0, 0},          {2, -1, 0, 0, 0, 0},          {3, -3, 1, 0, 0, 0},
-    {4, -6, 4, -1, 0, 0},        {5, -10, 10, -5, 1, 0},       {6, -15, 20, -15, 6, -1}};
 
 template <int MODE>
 __global__ void k_seed(Params p)
@@ -363,13 +360,11 @@ __global__ void k_seed(Params p)
             long long room = (dir > 0) ? (row - p.sub_first[sub]) : (p.sub_end[sub] - 1 - row);
             long long avail = min((long long)(2 * st.step - 1), room);
             int order = (int)min((long long)p.order, avail - 1);
-            double zx = 0.0, zy = 0.0;
-            for (int q = order; q >= 0; --q) {
-                const double2 v = p.roots[(row - (long long)dir * (q + 1)) * p.n_r + k];
-                zx = fma(c_coef[order][q], v.x, zx);
-                zy = fma(c_coef[order][q], v.y, zy);
-            }
-            z = make_double2(zx, zy);
+            double2 v[PRED_MAX_ORDER + 1];
+#pragma unroll
+            for (int q = 0; q <= PRED_MAX_ORDER; ++q)
+                v[q] = q <= order ? p.roots[(row - (long long)dir * (q + 1)) * p.n_r + k] : make_double2(0.0, 0.0);
+            z = predict_adaptive(v, order);
         }
         p.roots[row * p.n_r + k] = z;
         store_src<MODE>(p.src + (size_t)slot * 2 * p.N_pad, k, z);
@@ -1394,7 +1389,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     const int64_t phi_total = opt.phi_index_total > 0 ? opt.phi_index_total : num_phi;
     const int64_t phi_off = opt.phi_index_offset;
     int order = opt.predictor_order < 0 ? DEFAULT_ORDER_TILED : opt.predictor_order;
-    if (order > MAX_ORDER) return invalid("predictor_order > 5");
+    if (order > MAX_ORDER) return invalid("predictor_order > 8");
     int min_T = opt.min_lanes_per_root <= 0 ? 1 : opt.min_lanes_per_root;
     if (min_T > CTA || (min_T & (min_T - 1))) return invalid("min_lanes_per_root must be a power of two <= 128");
     if (opt.num_subchains < 0 || opt.max_iter_cold < 0) return invalid("negative option");

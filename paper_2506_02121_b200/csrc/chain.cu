@@ -21,6 +21,7 @@
 //     iteration), combined by shuffles in a fixed order: two runs give the same bits.
 // All arithmetic is FP64; the reciprocal of the Aberth sum is the 20-bit seed (R19), that of the star sums full.
 #include "star_sums.cuh"
+#include "predictor.cuh"
 
 #include <math.h>
 #include <algorithm>
@@ -30,15 +31,14 @@ namespace mlcc {
 namespace {
 
 #ifndef MLCC_CHAIN_MIN_CTAS
-#define MLCC_CHAIN_MIN_CTAS 2
+#define MLCC_CHAIN_MIN_CTAS 1
+#endif
+#ifndef MLCC_CHAIN_MAX_THREADS
+#define MLCC_CHAIN_MAX_THREADS 512
 #endif
 constexpr int CR = 2;                 // list entries per thread
-constexpr int MAX_ORDER = 5;
 constexpr double TINY = 1e-300;       // |d|^2 + TINY: the pair of a root with itself contributes exactly 0
 
-__constant__ double c_pred[MAX_ORDER + 1][MAX_ORDER + 1] = {
-    {1, 0, 0, 0, 0, 0},          {2, -1, 0, 0, 0, 0},          {3, -3, 1, 0, 0, 0},
-    {4, -6, 4, -1, 0, 0},        {5, -10, 10, -5, 1, 0},       {6, -15, 20, -15, 6, -1}};
 
 struct ChainCounters {
     unsigned long long root_iterations;       // unfrozen roots updated, summed over iterations, rows and sub-chains
@@ -218,7 +218,7 @@ __device__ __forceinline__ void chain_pass(const ChainParams &p, double m0, int 
 }
 
 template <bool CAUS>
-__global__ void __launch_bounds__(256, MLCC_CHAIN_MIN_CTAS) k_chain(ChainParams p)
+__global__ void __launch_bounds__(MLCC_CHAIN_MAX_THREADS, MLCC_CHAIN_MIN_CTAS) k_chain(ChainParams p)
 {
     extern __shared__ __align__(16) unsigned char s_raw[];
     __shared__ unsigned long long s_buf[33];
@@ -275,13 +275,12 @@ __global__ void __launch_bounds__(256, MLCC_CHAIN_MIN_CTAS) k_chain(ChainParams 
                         z.x += (k < N) ? 1.0 : -1.0;
                     }
                 } else {
-                    double zx = 0.0, zy = 0.0;
-                    for (int q = order; q >= 0; --q) {
-                        const double2 v = __ldcg(&p.roots[(row - (long long)dir * (q + 1)) * n_r + k]);
-                        zx = fma(c_pred[order][q], v.x, zx);
-                        zy = fma(c_pred[order][q], v.y, zy);
-                    }
-                    z = make_double2(zx, zy);
+                    double2 v[PRED_MAX_ORDER + 1];
+#pragma unroll
+                    for (int q = 0; q <= PRED_MAX_ORDER; ++q)
+                        v[q] = q <= order ? __ldcg(&p.roots[(row - (long long)dir * (q + 1)) * n_r + k])
+                                          : make_double2(0.0, 0.0);
+                    z = predict_adaptive(v, order);
                 }
                 s_z[set * n_r + k] = z;
                 s_list[n_act + k] = set * n_r + k;
@@ -458,7 +457,7 @@ int chain_threads(int64_t n_r)
     long long nt = (2 * n_r * 4 + CR - 1) / CR;
     nt = (nt + 31) / 32 * 32;
     if (nt < 32) nt = 32;
-    if (nt > 256) nt = 256;
+    if (nt > MLCC_CHAIN_MAX_THREADS) nt = MLCC_CHAIN_MAX_THREADS;
     return (int)nt;
 }
 

@@ -191,7 +191,7 @@ __device__ __forceinline__ double block_reduce_m(double v, bool take_max, double
     if (lane == 0) s_red[warp] = v;
     __syncthreads();
     if (warp == 0) {
-        double w = s_red[lane];
+        double w = lane < (int)(blockDim.x >> 5) ? s_red[lane] : v;   // (v: this lane's own warp result, a member of the set)
         for (int o = 16; o > 0; o >>= 1) {
             const double t = __shfl_xor_sync(0xffffffffu, w, o);
             w = take_max ? fmax(w, t) : fmin(w, t);
@@ -211,7 +211,7 @@ __global__ void __launch_bounds__(MBLOCK) k_match_smem(const double2 *__restrict
     __shared__ double s_red[33];
     __shared__ int s_part[MBLOCK / 32 + 1];
     __shared__ int s_flag;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, NTH = blockDim.x, nwarps = NTH >> 5;
     const int ncell = G * G;
     int *cell_start = s_dyn;                       // [ncell + 2]
     int *sorted = cell_start + ncell + 2;          // [n]
@@ -222,7 +222,7 @@ __global__ void __launch_bounds__(MBLOCK) k_match_smem(const double2 *__restrict
         const double2 *as = a + s * n, *bs = b + ((s + b_shift) % S) * n;
         // ---- bounding box of b, finiteness of a and b ----
         double xmin = 1e308, xmax = -1e308, ymin = 1e308, ymax = -1e308, bad = 0.0;
-        for (int j = tid; j < n; j += MBLOCK) {
+        for (int j = tid; j < n; j += NTH) {
             const double2 q = bs[j], q2 = as[j];
             xmin = fmin(xmin, q.x); xmax = fmax(xmax, q.x);
             ymin = fmin(ymin, q.y); ymax = fmax(ymax, q.y);
@@ -233,7 +233,7 @@ __global__ void __launch_bounds__(MBLOCK) k_match_smem(const double2 *__restrict
         bad = block_reduce_m(bad, true, s_red);
         if (bad > 0.0) {
             if (tid == 0) { if (out_max_err) out_max_err[s] = INFINITY; out_bijective[s] = 0; }
-            if (out_index) for (int i = tid; i < n; i += MBLOCK) out_index[s * n + i] = -1;
+            if (out_index) for (int i = tid; i < n; i += NTH) out_index[s * n + i] = -1;
             continue;
         }
         const double wx = xmax - xmin, wy = ymax - ymin;
@@ -241,17 +241,17 @@ __global__ void __launch_bounds__(MBLOCK) k_match_smem(const double2 *__restrict
         const double inv_hx = 1.0 / hx, inv_hy = 1.0 / hy;
         const double hmin = fmin(hx, hy);
         // ---- counting sort of b into cells ----
-        for (int c = tid; c < ncell + 2; c += MBLOCK) cell_start[c] = 0;
-        for (int w = tid; w < n_words; w += MBLOCK) mask[w] = 0u;
+        for (int c = tid; c < ncell + 2; c += NTH) cell_start[c] = 0;
+        for (int w = tid; w < n_words; w += NTH) mask[w] = 0u;
         __syncthreads();
-        for (int j = tid; j < n; j += MBLOCK) {
+        for (int j = tid; j < n; j += NTH) {
             const double2 q = bs[j];
             const int c = cell_coord(q.y, ymin, inv_hy, G) * G + cell_coord(q.x, xmin, inv_hx, G);
             atomicAdd(&cell_start[c + 1], 1);
         }
         __syncthreads();
         {   // inclusive scan of cell_start[1 .. ncell]: cell_start[c + 1] = points in cells 0 .. c
-            const int chunk = (ncell + MBLOCK - 1) / MBLOCK;
+            const int chunk = (ncell + NTH - 1) / NTH;
             const int lo = 1 + tid * chunk, hi = min(ncell + 1, lo + chunk);
             int sum = 0;
             for (int c = lo; c < hi; ++c) sum += cell_start[c];
@@ -264,7 +264,7 @@ __global__ void __launch_bounds__(MBLOCK) k_match_smem(const double2 *__restrict
             if (lane == 31) s_part[warp] = incl;
             __syncthreads();
             if (warp == 0) {
-                const int w = s_part[lane];
+                const int w = lane < nwarps ? s_part[lane] : 0;
                 int wi = w;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
@@ -281,7 +281,7 @@ __global__ void __launch_bounds__(MBLOCK) k_match_smem(const double2 *__restrict
         }
         // scatter from the back: every insertion into cell c takes slot --cell_start[c + 1]; afterwards
         // cell_start[c + 1] is the FIRST slot of cell c and cell_start[c + 2] one past its last
-        for (int j = tid; j < n; j += MBLOCK) {
+        for (int j = tid; j < n; j += NTH) {
             const double2 q = bs[j];
             const int c = cell_coord(q.y, ymin, inv_hy, G) * G + cell_coord(q.x, xmin, inv_hx, G);
             sorted[atomicSub(&cell_start[c + 1], 1) - 1] = j;
@@ -290,7 +290,7 @@ __global__ void __launch_bounds__(MBLOCK) k_match_smem(const double2 *__restrict
         // ---- nearest b for every a ----
         double max_d2 = 0.0;
         int ok = 1;
-        for (int i = tid; i < n; i += MBLOCK) {
+        for (int i = tid; i < n; i += NTH) {
             const double2 p = as[i];
             const int cx = cell_coord(p.x, xmin, inv_hx, G), cy = cell_coord(p.y, ymin, inv_hy, G);
             double best = INFINITY;
@@ -497,12 +497,16 @@ static int match_launch(const double *a, const double *b, int64_t S, int64_t n, 
     cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     if (smem + 2048 <= (size_t)max_optin) {
         MLCC_CUDA(cudaFuncSetAttribute(k_match_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        // small sets: fewer threads per CTA, more CTAs per SM
+        int threads = (int)((n + 31) / 32) * 32;
+        if (threads < 64) threads = 64;
+        if (threads > MBLOCK) threads = MBLOCK;
         int per_sm = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_match_smem, MBLOCK, smem) != cudaSuccess || per_sm < 1)
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_match_smem, threads, smem) != cudaSuccess || per_sm < 1)
             per_sm = 1;
         long long grid = (long long)per_sm * sms;
         if (grid > S) grid = S;
-        k_match_smem<<<(int)grid, MBLOCK, smem, stream>>>(reinterpret_cast<const double2 *>(a),
+        k_match_smem<<<(int)grid, threads, smem, stream>>>(reinterpret_cast<const double2 *>(a),
                                                           reinterpret_cast<const double2 *>(b), (long long)S, (int)n,
                                                           rel_tol, G, out_max_err, out_bijective, b_shift, out_index);
         MLCC_CUDA(cudaGetLastError());

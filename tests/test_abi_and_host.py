@@ -4,6 +4,7 @@ argument validation that is decided before any CUDA call."""
 import ctypes as C
 import os
 import re
+import sys
 
 import numpy as np
 import pytest
@@ -199,3 +200,31 @@ def test_rect_sheet_polynomial_reproduces_eq_b2(lib, orc):
     L = lib
     assert L.mlcc_rect_sheet(0.4, -1.0, 2.0, 1.5, 1e-9, 0, coef5.ctypes.data, 6, C.byref(C.c_double())) < 0
     assert L.mlcc_rect_sheet(0.4, 3.0, 2.0, 1.5, 1e-9, 0, coef5.ctypes.data, 6, C.byref(C.c_double())) < 0   # capacity
+
+
+def test_bench_host_arithmetic():
+    """bench.py's host-side bookkeeping (no GPU): the stride of the in-step det J sample reproduces the sampled rows'
+    phases exactly, and the per-pipe roofline splits the counters the way the line says it does."""
+    import types
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_2506_02121_b200.configs import CONFIGS
+    for total, off in ((10000, 0), (4000, 0), (5000, 0), (2000, 0), (1000, 0), (20000, 10000), (80000, 30000), (7, 0)):
+        d = bench.detj_stride(total, off)
+        assert 1 <= d <= 64 and total % d == 0 and off % d == 0
+        # row q*d of the rank (grid row q*d + off) has phase 2 pi (q + off/d) / (total/d)
+        q = 3
+        assert abs((q * d + off) / total - (q + off // d) / (total // d)) < 1e-15
+    assert bench.detj_stride(10000, 0) == 50
+    cfg = CONFIGS["cfg4"]
+    n_r = 2 * cfg.N
+    st = types.SimpleNamespace(root_iterations=1000, root_pairs=900 * (n_r - 1), aberth_sum_precision=64)
+    f64 = bench.flop_model(cfg, st, "direct", 64)
+    f32 = bench.flop_model(cfg, st, "direct", 32)
+    star = 27.0 * cfg.N * 900 + 25.0 * cfg.N * 100
+    assert f64["fp32"] == 0.0 and abs(f64["fp64"] - (star + 10.0 * st.root_pairs)) < 1.0
+    assert abs(f32["fp64"] - star) < 1.0 and abs(f32["fp32"] - 10.0 * st.root_pairs) < 1.0
+    acc = {"solve_ms": 1000.0, "fp64": f32["fp64"], "fp32": f32["fp32"], "hw_fp64": f32["hw_fp64"], "survey": f32["survey"]}
+    rf = bench.roofline_of(acc, 37.0, 70.0, 32)
+    assert abs(rf["combined_frac"] - (rf["fp64_frac"] + rf["fp32_frac"])) < 1e-15 and rf["fp32_frac"] > 0
+    assert bench.roofline_of(dict(acc, fp32=0.0), 37.0, 70.0, 64)["fp32_frac"] == 0.0

@@ -397,6 +397,36 @@ def test_equal_mass_fields_take_the_lighter_pair_body(api, orc, regime, N, num_p
         certify_every_row(api, dev(xy), dev(m), cfg, roots)
 
 
+def test_predictor_order_is_chosen_root_by_root(api, orc):
+    """DESIGN.md R18: the extrapolation order is capped by the option and chosen per root from the size of the backward
+    differences.  What can be observed through the C-ABI: any cap gives the oracle's root sets; a higher cap never
+    costs root-iterations on a smooth grid; and a grid coarse enough that two chains come close (cfg1 at 50 phases,
+    2 pi / 50 per row) still converges everywhere with the highest cap, within a few iterations per row."""
+    cfg = CONFIGS["cfg2"]
+    xy, m, R = field(orc, cfg)
+    dxy, dm = dev(xy), dev(m)
+    num_phi = 600
+    ref, _, _ = orc.critical_curves(xy, m, cfg.kappa_s, cfg.gamma, num_phi)
+    work = {}
+    for cap in (0, 2, 5, 8):
+        r, it, un, st = api.critical_curves_ex(dxy, dm, cfg.kappa_s, cfg.gamma, num_phi,
+                                               opt=api.options(predictor_order=cap, num_subchains=2, regime=1))
+        assert int(un.sum()) == 0 and st.predictor_order == cap
+        assert_rows_match(orc, r.cpu().numpy(), ref)
+        work[cap] = st.root_iterations
+    assert work[8] <= work[5] <= work[2] <= work[0]
+    with pytest.raises(api.MlccError):
+        api.critical_curves_ex(dxy, dm, cfg.kappa_s, cfg.gamma, 8, opt=api.options(predictor_order=9))
+    c1 = CONFIGS["cfg1"]
+    xy1, m1, _ = field(orc, c1)
+    for regime in (1, 2):
+        r, it, un, st = api.critical_curves_ex(dev(xy1), dev(m1), c1.kappa_s, c1.gamma, 50,
+                                               opt=api.options(num_subchains=1, regime=regime))
+        ref1, _, _ = orc.critical_curves(xy1, m1, c1.kappa_s, c1.gamma, 50)
+        assert int(un.sum()) == 0 and int(it.max()) <= 12
+        assert_rows_match(orc, r.cpu().numpy(), ref1)
+
+
 def test_chain_regime_limits_and_reports(api, orc):
     """What the chain regime refuses (fields beyond shared memory, far-field sums, a sheet polynomial, the FP32 Aberth
     sum when forced), what AUTO then does, and its max_iter / NaN reports."""
@@ -436,7 +466,7 @@ def test_options_do_not_change_the_root_sets(api, orc):
     dxy, dm = dev(xy), dev(m)
     seen_iters = {}
     for regime in (1, 2):
-        for order in range(0, 6):
+        for order in (0, 1, 2, 3, 5, 8):
             for nsub in (1, 3, 16):
                 r, it, un, st = api.critical_curves_ex(dxy, dm, cfg.kappa_s, cfg.gamma, num_phi,
                                                        opt=api.options(num_subchains=nsub, predictor_order=order,
