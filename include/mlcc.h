@@ -132,8 +132,9 @@ typedef struct mlcc_options {
                                  which multiplies F ~ F' dz in the denominator, cannot move the step by
                                  more than |dz|^2 |2 S1 - A| (reading R27).  The first iteration of every row always has A, and so
                                  has every root whose last step was larger.  0 = library default
-                                 (1e-8 for N >= 512; off for smaller fields, which are launch bound,
-                                 unless trust_predictor is set); negative = never skip.              */
+                                 (1e-8 in the chain regime and, in the tiled regime, for N >= 512: smaller
+                                 fields are launch bound there and the extra launch costs more than it
+                                 saves, unless trust_predictor is set); negative = never skip.       */
 } mlcc_options;
 
 /* Counters of one mlcc_critical_curves_ex call (host struct, filled on return). */
