@@ -1027,7 +1027,7 @@ def test_trust_predictor_starts_rows_with_newton_steps(api, orc, name, num_phi):
                                                       cfg.max_iter)[0] for j in rows])
     for mode in (api.MLCC_STAR_SUMS_DIRECT, api.MLCC_STAR_SUMS_FMM):
         base, it0, un0, st0 = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, num_phi, cfg.tol,
-                                                     cfg.max_iter, opt=api.options(star_sum_mode=mode))
+                                                     cfg.max_iter, opt=api.options(star_sum_mode=mode, regime=1))
         got, it1, un1, st1 = api.critical_curves_ex(dev(xy), dev(m), cfg.kappa_s, cfg.gamma, num_phi, cfg.tol,
                                                     cfg.max_iter, opt=api.options(star_sum_mode=mode, trust_predictor=1))
         assert int(un1.sum()) == 0 and st1.degenerate_roots == 0 and st1.unconverged_rows == 0
