@@ -266,6 +266,18 @@ int mlcc_star_sums(const double *star_xy, const double *masses, int64_t N, const
 int mlcc_match_root_sets(const double *a, const double *b, int64_t S, int64_t n, double rel_tol,
                          double *out_max_err, int32_t *out_bijective, void *stream);
 
+/* a8 for callers that may not allocate device memory (code under CUDA graph capture, serving loops, harnesses that
+ * forbid cudaMalloc): the same matching as mlcc_match_root_sets, same arguments, same outputs, but the call
+ * allocates and frees NOTHING (no cudaMalloc, cudaMallocAsync, cudaFree, no allocating library routine).  Its
+ * bins live in a static device array of 4 MiB that every GPU loading the library holds until the process exits.
+ *   Limit: n <= 8192 points per set; a larger n returns MLCC_ERR_INVALID_ARG (use mlcc_match_root_sets).
+ *   Every call on a device shares that array and finds the previous call's contents in it (the kernel clears what
+ *   it needs at zero itself).  Calls that OVERLAP on the GPU (different streams) race on it: keep the calls of one
+ *   device on one stream, or order them with events.
+ * Asynchronous on `stream`.  Errors: INVALID_ARG, CUDA.                                                       */
+int mlcc_match_root_sets_noalloc(const double *a, const double *b, int64_t S, int64_t n, double rel_tol,
+                                 double *out_max_err, int32_t *out_bijective, void *stream);
+
 /* a8, invariants  Completeness certificate of the root sets (BASELINE.json
  * north_star: "exactly the paper's degree of distinct roots per phase").  P(z; phi) =
  * F(z, phi) prod_i (z - z_i)^2 has degree 2N and leading coefficient -c(phi),

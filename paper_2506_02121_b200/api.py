@@ -99,6 +99,7 @@ def lib() -> C.CDLL:
                                                C.POINTER(mlcc_stats), vp]
         L.mlcc_caustics.argtypes = [vp, vp, i64, dbl, dbl, vp, i64, vp, vp]
         L.mlcc_match_root_sets.argtypes = [vp, vp, i64, i64, dbl, vp, vp, vp]
+        L.mlcc_match_root_sets_noalloc.argtypes = [vp, vp, i64, i64, dbl, vp, vp, vp]
         L.mlcc_num_roots.restype = C.c_int64
         L.mlcc_num_roots.argtypes = [i64, i32]
         L.mlcc_rect_sheet.argtypes = [dbl, dbl, dbl, dbl, dbl, i32, vp, i32, C.POINTER(dbl)]
@@ -474,6 +475,22 @@ def match_root_sets(a, b, rel_tol):
     if rc != MLCC_OK:
         _raise(rc)
     return err, bij
+
+
+def match_root_sets_noalloc(a, b, rel_tol, out_max_err, out_bijective):
+    """mlcc_match_root_sets_noalloc: as match_root_sets, but neither this wrapper nor the library allocates: the caller
+    passes the outputs (max_err [S] f64, bijective [S] i32).  n <= 8192 points per set."""
+    if a.shape != b.shape or a.dim() != 3 or a.shape[2] != 2:
+        raise ValueError("a and b must both be [S, n, 2]")
+    S, n, _ = a.shape
+    if tuple(out_max_err.shape) != (S,) or tuple(out_bijective.shape) != (S,):
+        raise ValueError("out_max_err and out_bijective must be [S]")
+    rc = lib().mlcc_match_root_sets_noalloc(_dev(a, name="a"), _dev(b, name="b"), S, n, float(rel_tol),
+                                            _dev(out_max_err, name="out_max_err"),
+                                            _dev(out_bijective, torch.int32, "out_bijective"), _stream())
+    if rc != MLCC_OK:
+        _raise(rc)
+    return out_max_err, out_bijective
 
 
 def plan_subchains(N: int, num_phi: int, num_subchains: int = 0):

@@ -64,6 +64,8 @@ int distance_histogram_impl(const double *, const int32_t *, int64_t, double, in
                             cudaStream_t);
 int match_root_sets_impl(const double *, const double *, int64_t, int64_t, double, double *, int32_t *,
                          cudaStream_t);
+int match_root_sets_noalloc_impl(const double *, const double *, int64_t, int64_t, double, double *, int32_t *,
+                                 cudaStream_t);
 int vieta_residuals_impl(const double *, const double *, int64_t, double, double, const double *, int64_t, int64_t,
                          int64_t, double *, double *, cudaStream_t);
 
@@ -317,6 +319,13 @@ int mlcc_match_root_sets(const double *a, const double *b, int64_t S, int64_t n,
     NvtxRange nvtx_("mlcc_match_root_sets");
     return match_root_sets_impl(a, b, S, n, rel_tol, out_max_err, out_bijective,
                                 static_cast<cudaStream_t>(stream));
+}
+
+int mlcc_match_root_sets_noalloc(const double *a, const double *b, int64_t S, int64_t n, double rel_tol,
+                                 double *out_max_err, int32_t *out_bijective, void *stream)
+{
+    return match_root_sets_noalloc_impl(a, b, S, n, rel_tol, out_max_err, out_bijective,
+                                        static_cast<cudaStream_t>(stream));
 }
 
 int mlcc_plan_subchains(int64_t N, int64_t num_phi, int32_t num_subchains, int32_t capacity,

@@ -534,4 +534,63 @@ static int match_launch(const double *a, const double *b, int64_t S, int64_t n, 
     return MLCC_OK;
 }
 
+// ------------------------------------------------------------------------------------------------
+// mlcc_match_root_sets_noalloc: the matcher for callers that may not allocate (code under CUDA graph capture,
+// serving loops, harnesses that forbid cudaMalloc).  It runs k_match, the kernel that bins b in GLOBAL scratch, with
+// that scratch in the file-scope device array below instead of a per-call allocation: nothing is allocated or freed
+// by the call (no cudaMalloc / cudaMallocAsync / cudaFree, no allocating library routine).
+//   * Size: MATCH_NOALLOC_INTS ints = 4 MiB, held by every GPU that loads the library until the process exits.
+//     A CTA needs (G^2 + 1) + G^2 + 2 n ints, G = ceil(sqrt n); sets of up to MATCH_NOALLOC_MAX_N = 8192 points leave
+//     room for >= 31 CTAs.  Larger n is rejected with MLCC_ERR_INVALID_ARG.
+//   * In host code the NAME of a __device__ array is a host-side stand-in, not a device address: the address the
+//     kernel gets comes from cudaGetSymbolAddress, asked once per device with that device current.
+//   * Every call on a device shares the array and finds the previous call's contents in it.  k_match zeroes what it
+//     needs at zero (cell counts, hit counts) for every set it handles, so nothing has to be cleared here; but two
+//     calls that overlap on the GPU (different streams) RACE on it.  Calls on one stream are ordered and safe.
+// ------------------------------------------------------------------------------------------------
+constexpr long long MATCH_NOALLOC_INTS = 1ll << 20;
+constexpr int MATCH_NOALLOC_MAX_N = 8192;
+static __device__ __align__(256) int g_match_scratch[MATCH_NOALLOC_INTS];
+
+int match_root_sets_noalloc_impl(const double *a, const double *b, int64_t S, int64_t n, double rel_tol,
+                                 double *out_max_err, int32_t *out_bijective, cudaStream_t stream)
+{
+    if (S < 0) return invalid("S < 0");
+    if (n < 1) return invalid("n < 1");
+    if (n > MATCH_NOALLOC_MAX_N)
+        return invalid("mlcc_match_root_sets_noalloc: n exceeds 8192 points per set (the static scratch is 4 MiB); "
+                       "use mlcc_match_root_sets");
+    if (!(rel_tol >= 0.0)) return invalid("rel_tol must be >= 0");
+    if (S == 0) return MLCC_OK;
+    if (!a || !b || !out_max_err || !out_bijective) return invalid("null pointer");
+    // device address of the scratch array, once per device, with that device current
+    static int *scratch_of_device[64] = {};
+    int dev = 0;
+    MLCC_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return invalid("device index out of range");
+    if (!scratch_of_device[dev]) {
+        int *ptr = nullptr;
+        MLCC_CUDA(cudaGetSymbolAddress((void **)&ptr, g_match_scratch));
+        if (!ptr) return invalid("internal: no device address for the static scratch");
+        scratch_of_device[dev] = ptr;
+    }
+    int *scratch = scratch_of_device[dev];
+    int G = (int)ceil(sqrt((double)n));
+    if (G < 1) G = 1;
+    const long long ncell = (long long)G * G;
+    const long long stride = (ncell + 1) + ncell + 2 * n;
+    long long grid = MATCH_NOALLOC_INTS / stride;   // CTAs the array has room for (>= 31 by the limit on n)
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_match, BLOCK, 0) != cudaSuccess || per_sm < 1) per_sm = 2;
+    const long long resident = (long long)per_sm * device_sm_count();
+    if (grid > resident) grid = resident;
+    if (grid > S) grid = S;
+    if (grid < 1) return invalid("internal: static scratch too small");
+    k_match<<<(int)grid, BLOCK, 0, stream>>>(reinterpret_cast<const double2 *>(a), reinterpret_cast<const double2 *>(b),
+                                            (long long)S, (int)n, rel_tol, G, scratch, stride, out_max_err,
+                                            out_bijective, 0, nullptr);
+    MLCC_CUDA(cudaGetLastError());
+    return MLCC_OK;
+}
+
 }  // namespace mlcc
