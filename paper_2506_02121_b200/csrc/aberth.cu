@@ -1225,9 +1225,13 @@ int plan_subchains_host(int64_t N, int64_t num_phi, int32_t num_subchains, int32
     if (N < 1 || num_phi < 1 || num_subchains < 0) return -MLCC_ERR_INVALID_ARG;
     int64_t n = num_subchains;
     if (n == 0) {
-        // enough slots (2 per sub-chain) to keep ~3e5 roots in flight, but chains at least 16 rows long
+        // enough slots (2 per sub-chain) to keep ~4.8e5 roots in flight, but chains at least 16 rows long.  More rows
+        // per step mean fewer steps, and every step ends with two or three launches for a handful of straggler roots
+        // (~80 us each, whatever the field); more sub-chains mean more cold rows (~7.6 full row-iterations each).
+        // Measured on B200, seconds per curve set at 3e5 / 4.8e5 / 6.4e5 / 9.6e5 roots in flight: cfg4 4.919 / 4.855 /
+        // 4.856 / 4.882, cfg3 0.1175 / 0.1162 / 0.1188 / 0.1250.
         const int64_t n_r = 2 * N;
-        int64_t slots = (300000 + n_r - 1) / n_r;
+        int64_t slots = (480000 + n_r - 1) / n_r;
         n = (slots + 1) / 2;
         const int64_t by_len = num_phi / 16;
         if (n > by_len) n = by_len;
@@ -1456,11 +1460,11 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     }
     if (want_sub == 0 && opt.trust_predictor == 1 && opt.star_sum_mode == MLCC_STAR_SUMS_FMM) {
         // Continued rows cost O(N) here (far-field star sums, no Aberth sum): a step of the default plan is a handful
-        // of short, latency-bound launches.  Four times as many rows per step amortise them; the price is four times
-        // as many cold rows (measured on cfg4: 0.53 s per set with the default plan, 0.34 s with four times it).
+        // of short, latency-bound launches.  More rows per step amortise them; the price is as many more cold rows
+        // (measured on cfg4: 0.53 s per set with 8 sub-chains, 0.34 s with 32; 2.5 times the default plan is 30).
         const int base = plan_subchains_host(N, num_phi, 0, MAX_SLOTS / 2, f64v.data(), c64v.data(), e64v.data());
         if (base >= 1) {
-            long long w = 4ll * base;
+            long long w = 5ll * base / 2;
             if (w > num_phi / 16) w = num_phi / 16;
             if (w > MAX_SLOTS / 2) w = MAX_SLOTS / 2;
             want_sub = (int)(w > base ? w : base);
