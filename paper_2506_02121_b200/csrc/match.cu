@@ -310,12 +310,24 @@ __global__ void __launch_bounds__(MBLOCK) k_match_smem(const double2 *__restrict
                         xb = min(xb, G - 1);
                         if (xa > xb) continue;
                         const int t0 = cell_start[yy * G + xa + 1], t1 = cell_start[yy * G + xb + 2];
-                        for (int t = t0; t < t1; ++t) {
-                            const int j = sorted[t];
-                            const double2 q = bs[j];
-                            const double dx = p.x - q.x, dy = p.y - q.y;
-                            const double d2 = dx * dx + dy * dy;
-                            if (d2 < best || (d2 == best && j < bj)) { best = d2; bj = j; }
+                        // four candidates per pass: their gathers from b are independent loads in flight together
+                        // (the kernel is bound by the latency of these L2 reads); compared in list order as before
+                        for (int t = t0; t < t1; t += 4) {
+                            int jj[4];
+                            double2 qq[4];
+#pragma unroll
+                            for (int u = 0; u < 4; ++u) jj[u] = sorted[min(t + u, t1 - 1)];
+#pragma unroll
+                            for (int u = 0; u < 4; ++u) qq[u] = bs[jj[u]];
+#pragma unroll
+                            for (int u = 0; u < 4; ++u) {
+                                if (t + u < t1) {
+                                    const int j = jj[u];
+                                    const double dx = p.x - qq[u].x, dy = p.y - qq[u].y;
+                                    const double d2 = dx * dx + dy * dy;
+                                    if (d2 < best || (d2 == best && j < bj)) { best = d2; bj = j; }
+                                }
+                            }
                         }
                     }
                 }
