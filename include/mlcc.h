@@ -72,7 +72,8 @@ enum { MLCC_STAR_SUMS_DIRECT = 0, MLCC_STAR_SUMS_FMM = 1 };
  *        sources through shared memory (any N; the path for N >~ 10^3).
  * CHAIN: one CTA owns a sub-chain and runs all its rows and iterations out of shared memory, one launch per call
  *        (fields of up to about 1200 stars; direct star sums, disc fields, FP64 Aberth sum, no trust_predictor).
- * AUTO:  CHAIN where it applies and n_r <= 2000, else TILED.  The root sets are the same within the parity
+ * AUTO:  CHAIN where it applies and n_r <= 2400 (all that fits shared memory), else TILED.
+ *        The root sets are the same within the parity
  *        tolerance; the bits differ (other summation order).                                              */
 enum { MLCC_REGIME_AUTO = 0, MLCC_REGIME_TILED = 1, MLCC_REGIME_CHAIN = 2 };
 

@@ -62,7 +62,7 @@ namespace {
 
 // Fields of up to this many roots per phase go to the chain regime when they fit it (mlcc_options.regime = AUTO);
 // measured crossover: DESIGN.md "Kernel regimes".
-constexpr int CHAIN_AUTO_MAX_ROOTS = 2000;
+constexpr int CHAIN_AUTO_MAX_ROOTS = 2400;
 
 constexpr int CTA = 128;          // threads per CTA of the compute kernel
 #ifndef MLCC_ROOTS_PER_THREAD

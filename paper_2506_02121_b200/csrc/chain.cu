@@ -16,9 +16,9 @@
 //     shared memory; the only global traffic is the finished rows (16 B per root and per caustic point) and the
 //     predictor's reads of the chain's last rows (L2 hits: this CTA wrote them);
 //   * an iteration is: pair loops -> __syncthreads -> apply + ordered compaction -> __syncthreads;
-//   * a thread owns R = 2 adjacent list entries (each shared-memory read of a source serves both) and T lanes of a
-//     warp split the sources of one root when fewer roots than threads are unfrozen (T = 1 .. 32, chosen per
-//     iteration), combined by shuffles in a fixed order: two runs give the same bits.
+//   * the unfrozen entries are worked off in passes that keep every thread busy: two adjacent entries per thread
+//     (each shared-memory read of a source serves both) while there are that many, one per thread, then T lanes of
+//     a warp per entry (T = 2 .. 32), combined by shuffles in a fixed order: two runs give the same bits.
 // All arithmetic is FP64; the reciprocal of the Aberth sum is the 20-bit seed (R19), that of the star sums full.
 #include "star_sums.cuh"
 #include "predictor.cuh"
@@ -128,7 +128,7 @@ __device__ __forceinline__ void chain_pass(const ChainParams &p, double m0, int 
     if (valid[0]) {
         // star sums (S1 only where the Aberth sum is used)
         if (large[0]) {
-#pragma unroll 2
+#pragma unroll (RR == 1 ? 4 : 2)
             for (int j = sub; j < N; j += T) {
                 const double2 s = s_xy[j];
                 const double m = EQM ? 0.0 : s_m[j];
@@ -139,7 +139,7 @@ __device__ __forceinline__ void chain_pass(const ChainParams &p, double m0, int 
                 }
             }
         } else {
-#pragma unroll 2
+#pragma unroll (RR == 1 ? 4 : 2)
             for (int j = sub; j < N; j += T) {
                 const double2 s = s_xy[j];
                 const double m = EQM ? 0.0 : s_m[j];
@@ -299,22 +299,25 @@ __global__ void __launch_bounds__(MLCC_CHAIN_MAX_THREADS, MLCC_CHAIN_MIN_CTAS) k
             int *next = s_list + (cur ^ 1) * 2 * n_r;
             const int n_large = n_act - n_small;
             // ---- pair loops.  A pass gives every lane group RR adjacent list entries and splits the sources of an
-            // entry over the T lanes of its group.  Full passes use RR = 2, T = 1 (each shared-memory read of a source
-            // serves two roots); what is left is cut so that no thread idles through a whole pass: one entry per
-            // thread, then the remainder spread over T lanes per entry. ----
+            // entry over the T lanes of its group (the schedule of the passes is below). ----
             // The entries that keep the Aberth sum and those that do not cost different amounts per entry, so the two
             // groups get passes of their own: inside a pass every thread then does the same work.
             for (int seg = 0; seg < 2; ++seg) {
                 const int seg_end = seg == 0 ? n_large : n_act;
                 for (int base = seg == 0 ? 0 : n_large; base < seg_end;) {
                     const int left = seg_end - base;
-                    int rr = 2, T = 1;
-                    if (4 * left >= 7 * NT) {                       // >= 1.75 NT entries: a full (or nearly full) pass
-                    } else if (left > NT) {                         // one entry per thread
-                        rr = 1;
-                    } else {                                        // the rest: T lanes per entry
+                    // Passes that keep every thread busy: two entries per thread while at least 2 NT are left, one entry
+                    // per thread while at least NT are left, then the remainder over T lanes per entry with T the
+                    // largest power of two that still gives every thread a share (a remainder above NT / 2 takes two
+                    // such passes).  A pass in which some warps have nothing to do makes them wait at the barrier for
+                    // its whole length (ncu: 23 % of the warp samples of cfg2 sat there with the earlier schedule).
+                    int rr = 1, T = 1;
+                    if (left >= 2 * NT) {
+                        rr = 2;
+                    } else if (left >= NT) {
+                    } else {
                         T = 2;
-                        while (T < 32 && left * (2 * T) <= NT * 2) T <<= 1;
+                        while (T < 32 && left * (2 * T) <= NT) T <<= 1;
                     }
                     if (eqm) {
                         if (rr == 2) chain_pass<CAUS, 2, true>(p, m0, base, T, seg_end, n_large, list, s_xy, s_m, s_z, s_delta, row_s);

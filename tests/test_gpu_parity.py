@@ -580,8 +580,10 @@ def test_ragged_sizes_span_tiles(api, orc):
         xy, m, R = orc.star_field(11, N, 0.35, 1)
         ref, _, un = orc.critical_curves(xy, m, 0.05, 0.3, num_phi)
         assert un.sum() == 0
-        r, it, unc, st = api.critical_curves_ex(dev(xy), dev(m), 0.05, 0.3, num_phi)
-        assert_rows_match(orc, r.cpu().numpy(), ref)
+        for regime in (1, 2):        # the tiled kernel's stages, and the chain regime that AUTO picks at these sizes
+            r, it, unc, st = api.critical_curves_ex(dev(xy), dev(m), 0.05, 0.3, num_phi, opt=api.options(regime=regime))
+            assert st.regime == regime
+            assert_rows_match(orc, r.cpu().numpy(), ref)
         pts = np.random.default_rng(N).normal(size=(777, 2)) * R
         w = api.caustics(dev(xy), dev(m), 0.05, 0.3, dev(pts)).cpu().numpy()
         wr = orc.caustics(xy, m, 0.05, 0.3, pts)
