@@ -228,3 +228,32 @@ def test_bench_host_arithmetic():
     rf = bench.roofline_of(acc, 37.0, 70.0, 32)
     assert abs(rf["combined_frac"] - (rf["fp64_frac"] + rf["fp32_frac"])) < 1e-15 and rf["fp32_frac"] > 0
     assert bench.roofline_of(dict(acc, fp32=0.0), 37.0, 70.0, 64)["fp32_frac"] == 0.0
+
+
+def test_reference_arm_prints_the_contract_line():
+    """`bench.py --impl reference` (the oracle on the host cores, no GPU): one JSON line with the keys the driver reads,
+    the value being the full-set rate extrapolated from a cold row and continued rows, labelled as such."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--workload", "cfg1",
+                        "--gpus", "1", "--steps", "2", "--warmup", "1"], capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.strip()]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["metric"] == "converged critical-curve roots/s" and d["unit"] == "roots/s"
+    assert d["higher_is_better"] is True and d["n_gpus"] == 1 and d["steps"] == 2 and d["warmup"] == 1
+    assert d["value"] > 0 and d["ms_per_step"] > 0 and d["vs_baseline"] is None and d["dtype"] == "f64"
+    assert d["config"]["workload"].startswith("cfg1") and d["config"]["extrapolated"] is True
+    cb = d["cpu_baseline"]
+    assert cb["kind"] == "oracle" and cb["cores"] >= 1 and cb["value"] == d["value"] and cb["extrapolated"] is True
+    assert cb["seconds_per_cold_row"] > 0 and cb["seconds_per_continued_row"] > 0
+    assert abs(cb["extrapolated_full_set_s"] - (cb["seconds_per_cold_row"] + 999 * cb["seconds_per_continued_row"])) < 1e-9
+    assert d["e2e"] == {"value": d["value"], "unit": "roots/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    assert d["gpu_launches"] == 0
+    # ranks other than 0 do no work and print nothing
+    r1 = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--workload", "cfg1",
+                         "--steps", "1", "--warmup", "0"], capture_output=True, text=True, env=dict(env, RANK="1", WORLD_SIZE="2"),
+                        timeout=300)
+    assert r1.returncode == 0 and r1.stdout.strip() == ""
