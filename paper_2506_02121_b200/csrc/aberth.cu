@@ -105,9 +105,11 @@ struct TileSet {
 };
 
 struct DevState {
-    int step;             // current step: 0 = cold centre rows, s >= 1 = rows centre +/- s
-    int iter;             // iterations done in this step
-    int n_slots;          // slots active in this step
+    int step;             // newest step started: 0 = cold centre rows, s >= 1 = rows centre +/- s
+    int iter;             // (unused)
+    int n_slots;          // slot indices in use: gens * s2 (a slot with slot_step < 0 is free)
+    int steps_final;      // every row of the steps below this one is final (no slot of theirs is live)
+    int newest_roots;     // roots of the rows the newest step started with
     int done;             // all steps finished
     int need_seed;        // the seed kernel must write starting values for this step
     int cur;              // which of the two active lists is current
@@ -161,7 +163,10 @@ struct Params {
     long long *slot_row;      // [MAX_SLOTS] row solved by the slot in this step
     int *slot_sub;            // [MAX_SLOTS] sub-chain of the slot
     int *slot_dir;            // [MAX_SLOTS] -1, +1 (0 = centre)
-    int *slot_iters;          // [MAX_SLOTS] iteration at which the slot last had unfrozen roots
+    int *slot_iters;          // [MAX_SLOTS] iterations done on the slot's row
+    int *slot_step;           // [MAX_SLOTS] step the slot's row belongs to, -1 = the slot is free
+    int gens;                 // generations of slots that can be live at once (1 = lock-step)
+    int s2;                   // slots per generation: 2 n_sub (sub-chain c: 2c downward / centre, 2c + 1 upward)
     int *n_active;            // [2][MAX_SLOTS]
     int *tile_start;          // [2 kernels][2][MAX_SLOTS + 1] first coarse / first fine tile of each slot
     int *coarse_roots;        // [2 kernels][MAX_SLOTS] roots of the slot covered by its coarse tiles
@@ -333,11 +338,14 @@ __global__ void k_seed(Params p)
 {
     const DevState st = *p.state;
     if (st.done || !st.need_seed) return;
-    const long long total = (long long)st.n_slots * p.n_r;
+    // the rows of the step that has just started sit in the slot block of its generation
+    const int blk = (st.step % p.gens) * p.s2;
+    const long long total = (long long)p.s2 * p.n_r;
     for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
          idx += (long long)gridDim.x * blockDim.x) {
-        const int slot = (int)(idx / p.n_r);
-        const int k = (int)(idx - (long long)slot * p.n_r);
+        const int slot = blk + (int)(idx / p.n_r);
+        const int k = (int)(idx - (long long)(slot - blk) * p.n_r);
+        if (p.slot_step[slot] != st.step) continue;   // no row of this step in that slot
         const long long row = p.slot_row[slot];
         double2 z;
         if (st.step == 0) {
@@ -894,9 +902,10 @@ __device__ void build_tiles(const Params &p, DevState &st, long long *s_buf)
     st.total_active = st.ts[0].total + st.ts[1].total;
 }
 
-// The slots of step st.step: thread c looks after sub-chain c (n_sub <= MAX_SLOTS / 2); the slots keep the
-// order (sub-chain, downward before upward).  Every thread returns with the same st.
-__device__ void build_slots(const Params &p, DevState &st, long long *s_buf)
+// Starts step st.step: thread c looks after sub-chain c (n_sub <= MAX_SLOTS / 2).  The rows of the step take the
+// slot block of the step's generation, (st.step % gens) * s2 + {2c: downward (or the centre row), 2c + 1: upward};
+// st.cur is the list the next launches read.  Every thread returns with the same st.
+__device__ void spawn_step(const Params &p, DevState &st, long long *s_buf)
 {
     const int c = threadIdx.x;
     int has_dn = 0, has_up = 0;
@@ -912,22 +921,26 @@ __device__ void build_slots(const Params &p, DevState &st, long long *s_buf)
             has_up = row_up < p.sub_end[c];
         }
     }
-    long long n;
-    int at = (int)block_scan(has_dn + has_up, &n, s_buf);
-    if (has_dn) { p.slot_row[at] = row_dn; p.slot_sub[at] = c; p.slot_dir[at] = st.step == 0 ? 0 : -1; ++at; }
-    if (has_up) { p.slot_row[at] = row_up; p.slot_sub[at] = c; p.slot_dir[at] = +1; }
-    st.n_slots = (int)n;
-    if (threadIdx.x < st.n_slots) {
-        p.n_active[st.cur * MAX_SLOTS + threadIdx.x] = p.n_r;
-        p.n_active[(st.cur ^ 1) * MAX_SLOTS + threadIdx.x] = 0;
-        // a new row: every root gets the Aberth sum, unless the step's seeds are trusted (then none does at first)
-        p.n_small[st.cur * MAX_SLOTS + threadIdx.x] = trusted_step(p, st.step) ? p.n_r : 0;
-        p.n_small[(st.cur ^ 1) * MAX_SLOTS + threadIdx.x] = 0;
-        p.slot_iters[threadIdx.x] = 0;
+    const int blk = (st.step % p.gens) * p.s2;
+    // a new row: every root gets the Aberth sum, unless the step's seeds are trusted (then none does at first)
+    const int n_small0 = trusted_step(p, st.step) ? p.n_r : 0;
+    for (int q = 0; q < 2; ++q) {
+        if (!(q == 0 ? has_dn : has_up)) continue;
+        const int slot = blk + 2 * c + q;
+        p.slot_row[slot] = q == 0 ? row_dn : row_up;
+        p.slot_sub[slot] = c;
+        p.slot_dir[slot] = q == 0 ? (st.step == 0 ? 0 : -1) : +1;
+        p.slot_step[slot] = st.step;
+        p.slot_iters[slot] = 0;
+        p.n_active[st.cur * MAX_SLOTS + slot] = p.n_r;
+        p.n_active[(st.cur ^ 1) * MAX_SLOTS + slot] = 0;
+        p.n_small[st.cur * MAX_SLOTS + slot] = n_small0;
+        p.n_small[(st.cur ^ 1) * MAX_SLOTS + slot] = 0;
     }
-    st.iter = 0;
+    long long n;
+    block_scan(has_dn + has_up, &n, s_buf);
+    st.newest_roots = (int)(n * p.n_r);
     st.need_seed = 1;
-    if (n == 0) st.done = 1;
     __syncthreads();   // the counts are read back by build_tiles
 }
 
@@ -963,53 +976,83 @@ __global__ void __launch_bounds__(FIN) k_init(Params p)
 {
     __shared__ long long s_buf[33];
     DevState st;
-    st.step = 0; st.iter = 0; st.n_slots = 0; st.done = 0; st.need_seed = 1; st.cur = 0;
+    st.step = 0; st.iter = 0; st.n_slots = p.gens * p.s2; st.done = 0; st.need_seed = 1; st.cur = 0;
+    st.steps_final = 0; st.newest_roots = 0;
     st.ts[0] = TileSet{1, 1, 0, 0, 0, 0}; st.ts[1] = TileSet{1, 1, 0, 0, 0, 0};
     st.total_active = 0; st.total_iterations = 0;
     st.unconverged_rows = 0; st.degenerate = 0; st.n_outside = 0; st.root_iterations_noA = 0; st.root_iterations = 0; st.launches_used = 0;
-    build_slots(p, st, s_buf);
+    p.slot_step[threadIdx.x] = -1;   // FIN = MAX_SLOTS threads: every slot free (n_active / n_small were zeroed by the host)
+    __syncthreads();
+    spawn_step(p, st, s_buf);
     build_tiles(p, st, s_buf);
     if (threadIdx.x == 0) *p.state = st;
 }
 
-// Closes an iteration (run by the LAST CTA of k_apply_write, FIN threads): swaps the active lists, detects the end
-// of a step, writes the rows' diagnostics, builds the next step's slots and the tile tables of the next launch.
+// Closes an iteration (run by the LAST CTA of k_apply_write, FIN threads).  Every live slot has been iterated once:
+// a slot whose list is empty (or that has used up its iterations) is finished -- its row's diagnostics are written
+// and the slot is freed; the next step is STARTED as soon as (a) the slot block of its generation is free and (b) the
+// newest step has almost no survivor with a large step left (at most one root in 1024; the cold step must be
+// finished altogether): the few roots of older rows that still need iterations are carried along as extra slots of
+// the same launches instead of holding up the whole step.  A row seeded from a predecessor that
+// is still moving by < 1e-8 gets a seed that is off by as much: only the starting guess sees it.
 __device__ void finalize_iteration(const Params &p, long long *s_buf)
 {
     DevState st = *p.state;   // every thread carries the same copy and makes the same decisions
     if (st.done) return;
     const int s = threadIdx.x;
     // the iteration that just ran
-    st.iter += 1;
     st.total_iterations += 1;
     st.root_iterations += st.total_active;
     st.root_iterations_noA += st.ts[1].total;
     st.launches_used += 1;
     st.need_seed = 0;
     st.n_outside = 0;
-    int left = 0;
-    if (s < st.n_slots) {
+    int my_step = -1, unconv = 0, large = 0;
+    if (s < st.n_slots && (my_step = p.slot_step[s]) >= 0) {
+        const int it = p.slot_iters[s] + 1;
+        p.slot_iters[s] = it;
         // (written by other CTAs of this launch: read through L2)
-        if (__ldcg(&p.n_active[st.cur * MAX_SLOTS + s]) > 0) p.slot_iters[s] = st.iter;
-        left = __ldcg(&p.n_active[(st.cur ^ 1) * MAX_SLOTS + s]);
-    }
-    long long remaining;
-    block_scan(left, &remaining, s_buf);
-    st.cur ^= 1;
-    const int cap = (st.step == 0) ? p.max_iter_cold : p.max_iter;
-    if (remaining == 0 || st.iter >= cap) {
-        // step finished: per-row diagnostics, then the next step's slots
-        if (s < st.n_slots) {
+        const int left = __ldcg(&p.n_active[(st.cur ^ 1) * MAX_SLOTS + s]);
+        const int cap = (my_step == 0) ? p.max_iter_cold : p.max_iter;
+        if (left == 0 || it >= cap) {            // the row is finished
             const long long row = p.slot_row[s];
-            if (p.out_iters) p.out_iters[row] = p.slot_iters[s];
+            if (p.out_iters) p.out_iters[row] = it;
             if (p.out_unconverged) p.out_unconverged[row] = left;
+            if (left > 0) {
+                unconv = 1;
+                p.n_active[(st.cur ^ 1) * MAX_SLOTS + s] = 0;
+                p.n_small[(st.cur ^ 1) * MAX_SLOTS + s] = 0;
+            }
+            p.slot_step[s] = -1;
+            my_step = -1;
+        } else if (my_step == st.step) {
+            large = left - __ldcg(&p.n_small[(st.cur ^ 1) * MAX_SLOTS + s]);
         }
-        long long unconverged;
-        block_scan(left > 0 ? 1 : 0, &unconverged, s_buf);
-        st.unconverged_rows += (int)unconverged;
+    }
+    // live slots per generation (step - g, g = 0 .. gens - 1 <= 2) in 16-bit fields, unconverged rows above them
+    long long packed = (long long)unconv << 48;
+    if (my_step >= 0) packed += 1ll << (16 * (st.step - my_step));
+    long long tot_packed, tot_large;
+    block_scan(packed, &tot_packed, s_buf);
+    block_scan(large, &tot_large, s_buf);
+    st.unconverged_rows += (int)(tot_packed >> 48);
+    const int live_g[3] = {(int)(tot_packed & 0xffff), (int)((tot_packed >> 16) & 0xffff), (int)((tot_packed >> 32) & 0xffff)};
+    const int live_total = live_g[0] + live_g[1] + live_g[2];
+    st.cur ^= 1;
+    st.steps_final = st.step + 1;
+    for (int g = 0; g < p.gens; ++g)
+        if (live_g[g] > 0) st.steps_final = st.step - g;
+    bool spawn = false;
+    if (st.step < p.max_steps) {
+        const bool block_free = live_g[p.gens - 1] == 0;   // the slot block of step + 1 is that of step + 1 - gens
+        const bool newest_ok = st.step == 0 ? live_total == 0 : tot_large <= (long long)(st.newest_roots >> 10);
+        spawn = block_free && newest_ok;
+    }
+    if (spawn) {
         st.step += 1;
-        if (st.step > p.max_steps) { st.done = 1; st.n_slots = 0; }
-        else build_slots(p, st, s_buf);
+        spawn_step(p, st, s_buf);
+    } else if (st.step >= p.max_steps && live_total == 0) {
+        st.done = 1;
     }
     if (!st.done) build_tiles(p, st, s_buf);
     __syncthreads();   // every thread has read *p.state
@@ -1042,7 +1085,7 @@ __global__ void __launch_bounds__(COUNT_THREADS) k_apply_count(Params p)
     const int lo = chunk * APPLY_CHUNK, hi = min(n_act, lo + APPLY_CHUNK);
     if (lo >= n_act) return;
     const double2 *delta = p.delta + (long long)slot * p.n_r;
-    const bool guard = st.iter == 0 && trusted_step(p, st.step);
+    const bool guard = p.slot_iters[slot] == 0 && trusted_step(p, p.slot_step[slot]);
     int n_large = 0, n_small = 0;
     for (int pos = lo + threadIdx.x; pos < hi; pos += COUNT_THREADS) {
         const double2 d = delta[pos];
@@ -1103,7 +1146,7 @@ __global__ void __launch_bounds__(APPLY_THREADS) k_apply_write(Params p)
             // First iteration of a trusted row: the steps were taken without the Aberth sum, i.e. they are Newton steps
             // from the predicted seeds.  One below the skip threshold is applied as any confirming step is; a larger one
             // says the prediction was not that good: it is NOT applied and the root gets a full Aberth iteration next.
-            const bool guard = st.iter == 0 && trusted_step(p, st.step);
+            const bool guard = p.slot_iters[slot] == 0 && trusted_step(p, p.slot_step[slot]);
             int ks[APPLY_ITEMS];
             int kind[APPLY_ITEMS];   // 0 frozen, 1 large, 2 small
             int cnt = 0;
@@ -1488,7 +1531,11 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
                            end, max_steps, init_roots, out_roots, out_caustics, out_iters, out_unconverged, out_stats,
                            stream, h_roots, h_caustics);
     }
-    const int max_slots = 2 * n_sub > 1 ? 2 * n_sub : 1;
+    // up to three generations of slots live at once: the rows of the newest step, and what is left of the two before
+    const int s2 = 2 * n_sub;
+    int gens = 3;
+    while (gens > 1 && gens * s2 > MAX_SLOTS) --gens;
+    const int max_slots = gens * s2;
     NvtxRange nvtx_("mlcc: solve, tiled regime");
     RunStream run_stream;            // declared before the workspace: destroyed after it
     MLCC_CUDA(run_stream.open(stream));
@@ -1508,6 +1555,7 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
         (e = ws.alloc(&p.slot_sub, MAX_SLOTS)) != cudaSuccess ||
         (e = ws.alloc(&p.slot_dir, MAX_SLOTS)) != cudaSuccess ||
         (e = ws.alloc(&p.slot_iters, MAX_SLOTS)) != cudaSuccess ||
+        (e = ws.alloc(&p.slot_step, MAX_SLOTS)) != cudaSuccess ||
         (e = ws.alloc(&p.n_active, 2 * MAX_SLOTS)) != cudaSuccess ||
         (e = ws.alloc(&p.tile_start, 4 * (MAX_SLOTS + 1))) != cudaSuccess ||
         (e = ws.alloc(&p.coarse_roots, 2 * MAX_SLOTS)) != cudaSuccess ||
@@ -1601,6 +1649,8 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
     p.sub_end = d_plan + 2 * n_sub;
     p.max_steps = max_steps;
     p.max_slots = max_slots;
+    p.gens = gens;
+    p.s2 = s2;
 
     Event ev0, ev1, ev_poll[2];
     MLCC_CUDA(ev0.create());
@@ -1711,14 +1761,14 @@ int critical_curves_impl(const double *star_xy, const double *masses, int64_t N,
             cudaError_t es = cudaEventSynchronize(ev_poll[which ^ 1]);
             if (es != cudaSuccess) { rc = cuda_fail(es, "cudaEventSynchronize", __FILE__, __LINE__); break; }
             if (h_state[which ^ 1].done) finished = true;
-            if (h_state[which ^ 1].step > steps_seen) {   // step 0 = the cold centre rows, then the continuation steps
+            if (h_state[which ^ 1].steps_final > steps_seen) {   // step 0 = the cold centre rows, then the continuation steps
                 char text[96];
                 snprintf(text, sizeof text, "mlcc: steps %d..%d finished (step 0 = cold rows)", steps_seen,
-                         h_state[which ^ 1].step - 1);
+                         h_state[which ^ 1].steps_final - 1);
                 nvtxMarkA(text);
-                steps_seen = h_state[which ^ 1].step;
+                steps_seen = h_state[which ^ 1].steps_final;
             }
-            copy_finished(h_state[which ^ 1].step);   // that snapshot is complete: every launch before it has run
+            copy_finished(h_state[which ^ 1].steps_final);   // that snapshot is complete: every launch before it has run
         }
         which ^= 1;
     }

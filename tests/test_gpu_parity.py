@@ -427,6 +427,34 @@ def test_predictor_order_is_chosen_root_by_root(api, orc):
         assert_rows_match(orc, r.cpu().numpy(), ref1)
 
 
+@pytest.mark.parametrize("max_iter", [1, 2, 3, 6])
+def test_tiled_regime_iteration_cap_and_many_subchains(api, orc, max_iter):
+    """The tiled regime's driver (rows of several steps in flight at once: DESIGN.md "Driver") at its edges: an iteration
+    cap that stops rows early -- every row reports its own count of unfrozen roots, everything is written and finite,
+    the call says NOT_CONVERGED -- and plans with so many sub-chains that only two generations, or one (lock-step), of
+    slots fit: same root sets as the oracle."""
+    cfg = CONFIGS["cfg2"]
+    xy, m, R = field(orc, cfg)
+    dxy, dm = dev(xy), dev(m)
+    num_phi = 96
+    r, it, un, st = api.critical_curves_ex(dxy, dm, cfg.kappa_s, cfg.gamma, num_phi, cfg.tol, max_iter,
+                                           opt=api.options(regime=1, num_subchains=3), strict=False)
+    assert st.regime == 1 and bool(torch.isfinite(r).all())
+    assert st.status == api.MLCC_ERR_NOT_CONVERGED and st.unconverged_rows == int((un > 0).sum()) > 0
+    assert int(it.max()) == max_iter and int(it.min()) >= 1
+    again, it2, un2, _ = api.critical_curves_ex(dxy, dm, cfg.kappa_s, cfg.gamma, num_phi, cfg.tol, max_iter,
+                                                opt=api.options(regime=1, num_subchains=3), strict=False)
+    assert torch.equal(again, r) and torch.equal(it2, it) and torch.equal(un2, un)
+    if max_iter == 6:
+        ref, _, _ = orc.critical_curves(xy, m, cfg.kappa_s, cfg.gamma, 1100)
+        for nsub in (200, 400, 512):        # 3, 2 and 1 generations of slots
+            full, itf, unf, stf = api.critical_curves_ex(dxy, dm, cfg.kappa_s, cfg.gamma, 1100,
+                                                         opt=api.options(regime=1, num_subchains=nsub))
+            assert stf.subchains == nsub and int(unf.sum()) == 0
+            assert_rows_match(orc, full.cpu().numpy(), ref)
+            certify_every_row(api, dxy, dm, cfg, full)
+
+
 def test_chain_regime_limits_and_reports(api, orc):
     """What the chain regime refuses (fields beyond shared memory, far-field sums, a sheet polynomial, the FP32 Aberth
     sum when forced), what AUTO then does, and its max_iter / NaN reports."""
