@@ -11,11 +11,13 @@
 // Organisation (DESIGN.md "Driver" and "Kernels"):
 //   * The rows [0, num_phi) are cut into sub-chains; each sub-chain cold-starts its centre row from
 //     z_i +/- 1 and then grows towards both ends.  One "step"
-//     advances every growing direction ("slot") by one row; all slots of a step are iterated
-//     together by the same kernels, so the grid is full even when 2N is small.
-//   * A device-side state machine (DevState) decides what each launch does; the host only enqueues
-//     [seed, compute, apply, finalize] groups and polls one flag per chunk.  No host round trip
-//     sits inside the iteration loop.
+//     starts one new row in every growing direction; a row being solved occupies a "slot", and all
+//     live slots are iterated together by the same kernels, so the grid is full even when 2N is small.
+//     Steps are pipelined: the next one starts as soon as the newest has (almost) only nearly
+//     converged roots left, and the stragglers of older rows ride along as extra slots.
+//   * A device-side state machine (DevState, finalize_iteration) decides what each launch does; the
+//     host only enqueues [seed, compute, compute without A, apply count, apply write] groups and polls
+//     one flag per chunk.  No host round trip sits inside the iteration loop.
 //   * compute: persistent CTAs of 128 threads pull tiles of unfrozen roots from an atomic counter.
 //     A thread owns R roots (R = 2), and a root's sums are split over T threads (T = 1..128): the
 //     T shares sit in different warps whenever T <= 4, so every shared-memory read of the pair loop
@@ -32,8 +34,8 @@
 //   * Far-field mode: k_star_sums evaluates the star sums of every unfrozen root
 //     from the near stars and the node's Taylor series (star_sums.cuh, fmm.cu); the compute kernel
 //     then sums root pairs only (R = 8).
-//   * Jacobi: updates go to a side buffer and are applied by `apply`, which also refreshes the
-//     per-slot source copy of the row and compacts the list of unfrozen roots in order.
+//   * Jacobi: updates go to a side buffer and are applied by the apply kernels, which also refresh the
+//     per-slot source copy of the row and compact the list of unfrozen roots in order.
 #include "star_sums.cuh"
 #include "predictor.cuh"
 
