@@ -455,6 +455,57 @@ def test_tiled_regime_iteration_cap_and_many_subchains(api, orc, max_iter):
             certify_every_row(api, dxy, dm, cfg, full)
 
 
+def test_random_shapes_both_regimes_certified_and_against_oracle(api, orc):
+    """48 seeded random problems (N 1..300, 1..700 phases, plans from one sub-chain to one per row, every option that
+    keeps the root sets): the tiled regime is reproducible bit for bit, every row passes the det J and Vieta
+    certificates, the chain regime finds the same root sets, and where the oracle finishes at once (N <= 64,
+    <= 64 phases) so does the oracle."""
+    rng = np.random.default_rng(20250602)
+    with_oracle = stuck = 0
+    for case in range(48):
+        N = int(rng.choice([1, 2, 3, 5, 17, 40, 64, 100, 129, 200, 257, 300]))
+        num_phi = int(rng.choice([1, 2, 3, 7, 16, 33, 64, 100, 257, 400, 700]))
+        kappa_star, kappa_s, gamma = rng.uniform(0.05, 0.6), rng.uniform(0.0, 0.6), rng.uniform(-0.6, 0.6)
+        nsub = min(int(rng.choice([0, 0, 1, 2, 3, 5, 8, 50, 170, 200, 342, 400, 512])), num_phi)
+        kw = [dict(), dict(trust_predictor=1), dict(star_sum_mode=api.MLCC_STAR_SUMS_FMM), dict(aberth_sum_precision=32),
+              dict(predictor_order=int(rng.integers(0, 9))),
+              dict(trust_predictor=1, star_sum_mode=api.MLCC_STAR_SUMS_FMM)][int(rng.integers(0, 6))]
+        what = (case, N, num_phi, nsub, kw)
+        xy, m, R = orc.star_field(int(rng.integers(0, 1 << 30)), N, kappa_star, int(rng.integers(0, 2)), None)
+        dxy, dm = dev(xy), dev(m)
+        opt = api.options(regime=1, num_subchains=nsub, **kw)
+        r1, c1, it1, un1, st1 = api.curves_and_caustics(dxy, dm, kappa_s, gamma, num_phi, 1e-12, 60, opt=opt, strict=False)
+        r2, c2, it2, un2, _ = api.curves_and_caustics(dxy, dm, kappa_s, gamma, num_phi, 1e-12, 60, opt=opt, strict=False)
+        assert torch.equal(r1, r2) and torch.equal(c1, c2) and torch.equal(it1, it2) and torch.equal(un1, un2), what
+        if st1.status == api.MLCC_ERR_NOT_CONVERGED:
+            # DESIGN.md R6: one star makes F real in z - z_1, the seeds z_1 +- 1 are real, and where the two roots are
+            # imaginary (phi = 0 with |gamma| > 1 - kappa_s) the iterates never leave the axis.  The oracle, which
+            # follows the paper's seeds too, must fail on the same rows, and so must the chain regime.
+            assert N == 1, what
+            _, _, un_ref = orc.critical_curves(xy, m, kappa_s, gamma, num_phi, 1e-12, 60)
+            assert np.array_equal(un1.cpu().numpy() > 0, un_ref > 0), what
+            _, _, _, un3, st3 = api.curves_and_caustics(dxy, dm, kappa_s, gamma, num_phi, 1e-12, 60, strict=False,
+                                                        opt=api.options(regime=2, num_subchains=nsub))
+            assert st3.status == api.MLCC_ERR_NOT_CONVERGED and torch.equal(un3 > 0, un1 > 0), what
+            stuck += 1
+            continue
+        assert st1.regime == 1 and st1.unconverged_rows == 0 and int(it1.min()) >= 1, what
+        assert bool(torch.isfinite(r1).all()) and bool(torch.isfinite(c1).all()), what
+        row_newton, row_detj, _ = api.detj_residuals(dxy, dm, kappa_s, gamma, r1)
+        assert float(row_detj.max()) <= 1.0 and float(row_newton.max()) <= 1e-10, what
+        e1, e2 = api.vieta_residuals(dxy, dm, kappa_s, gamma, r1)
+        assert float(e1.max()) <= 1e-11 and float(e2.max()) <= 1e-11, what
+        r3, _, _, _, st3 = api.curves_and_caustics(dxy, dm, kappa_s, gamma, num_phi, 1e-12, 60,
+                                                   opt=api.options(regime=2, num_subchains=nsub))
+        err, bij = api.match_root_sets(r1, r3, ROOT_TOL)
+        assert st3.regime == 2 and bool(bij.all()), (what, float(err.max()))
+        if N <= 64 and num_phi <= 64:
+            ref = orc.critical_curves(xy, m, kappa_s, gamma, num_phi, 1e-12, 80)[0]
+            assert_rows_match(orc, r1.cpu().numpy(), ref)
+            with_oracle += 1
+    assert with_oracle >= 8 and stuck <= 2
+
+
 def test_chain_regime_limits_and_reports(api, orc):
     """What the chain regime refuses (fields beyond shared memory, far-field sums, a sheet polynomial, the FP32 Aberth
     sum when forced), what AUTO then does, and its max_iter / NaN reports."""
