@@ -533,6 +533,8 @@ __global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Para
     const int tid = threadIdx.x;
     const int n_stage = STAGES ? p.N_pad / S_TILE : 0;
     const int n_src = 2 * p.N_pad;
+    // sources of the last stage that are not padding (a stage pairs star j with the root entries 2j, 2j + 1)
+    const int last_cnt = max(p.N, (p.n_r + 1) / 2) - (n_stage - 1) * S_TILE;
     const int *n_active = p.n_active + st.cur * MAX_SLOTS;
 
     if (tid == 0) {
@@ -556,6 +558,7 @@ __global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Para
         const int sub = tid / G;
         const int local = tid - sub * G;
         const int n_it = S_TILE / T;         // pair-loop iterations per stage (even, >= 2)
+        const int n_it_last = min(n_it, ((last_cnt + T - 1) / T + 1) & ~1);   // the last stage stops at its padding
         const int tile_roots = R * G;
         const int *tab = p.tile_start + (2 * K + (fine ? 1 : 0)) * (MAX_SLOTS + 1);
         const int tt = fine ? tile - ts.n_coarse : tile;
@@ -628,7 +631,8 @@ __global__ void __launch_bounds__(CTA, STARS ? MLCC_MIN_CTAS : 4) k_compute(Para
                 const Stage &sg = s_stage[b];
                 // blocks of 2 sources x R roots: independent (1 star + 2 roots) bodies with no exit in
                 // between, so that their dependent chains (|d|^2 -> reciprocal -> powers) interleave
-                for (int i = 0; i < n_it; i += 2) {
+                const int n_it_t = t + 1 < n_stage ? n_it : n_it_last;
+                for (int i = 0; i < n_it_t; i += 2) {
 #pragma unroll
                     for (int u = 0; u < 2; ++u) {
                         const int j = sub + (i + u) * T;
