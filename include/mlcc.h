@@ -101,7 +101,7 @@ typedef struct mlcc_options {
                                    default: every pair of the iteration is FP64 arithmetic);
                                    32 = double-single FP32 (z = hi + lo, differences exact to
                                    ~2^-23 |z_k - z_r|, packed f32x2 instructions; tiled regime only;
-                                   about 7 % faster at N = 10^4).  Star sums (F, F') are FP64 in both. */
+                                   about 9 % faster at N = 10^4).  Star sums (F, F') are FP64 in both. */
     int32_t star_sum_mode;    /* MLCC_STAR_SUMS_DIRECT (default) or MLCC_STAR_SUMS_FMM               */
     int32_t fmm_order;        /* Taylor order of the node series (1..63); 0 = 31                     */
     int32_t fmm_stars_per_node; /* mean stars per grid node (the grid has ~N / this many nodes);
